@@ -1,0 +1,149 @@
+/*
+ * pairhmm_b200.h -- C ABI of libpairhmm_b200.so: batch PairHMM forward on one NVIDIA B200 (sm_100a).
+ *
+ * What the library computes (reference/PAPER.md = arxiv/paper_2606_25738, "Endeavor"):
+ *   for every (read, haplotype) pair of a batch, the PairHMM forward likelihood
+ *       L = sum_{j=1..k} ( M_{l,j} + I_{l,j} ) / C                        (Eq.4)
+ *   of the three-state recurrence (Eq.2) started from Eq.1 with the
+ *   emission prior of Eq.3 and per-read-position transition probabilities derived
+ *   from the insertion / deletion / gap-continuation qualities (Listing 2
+ *   :293-295).  The kernels evaluate the paper's row-wise reformulation (Eq.6-7, PAPER.md:99-121,
+ *   D eliminated / carried as a running weighted sum) as a skewed systolic wavefront; the result
+ *   is the same number.  Output is log10 L (the paper returns the raw scaled sum).
+ *
+ * Conventions
+ *   - "host" / "device" below says where a pointer must live.  Device buffers are allocated by
+ *     the caller (e.g. through PyTorch); the library only reads inputs and writes the outputs.
+ *   - Bases are bytes compared literally (Eq.3: r_i == h_j); the workloads use ASCII A,C,G,T.
+ *     Only the low 2 bits after the mapping A->0 C->1 G->2 T->3 are used on the device; any other
+ *     byte is mapped to a code that matches nothing in the other sequence ('N' matches nothing,
+ *     DESIGN.md reading G17) -- on the read side it is code 4, on the haplotype side it is "no bit set".
+ *   - Qualities are RAW Phred bytes 0..93 (NOT ASCII+33; reading G5):
+ *        eps = 10^(-Qbase/10), iota = 10^(-Qins/10), delta = 10^(-Qdel/10), gamma = 10^(-Qgcp/10);
+ *        T_MM = 1-iota-delta, T_MI = iota, T_MD = delta, T_II = T_DD = gamma, T_IM = T_DM = 1-gamma,
+ *     all taken at the read position (row) of the cell being written.  Precondition: iota+delta < 1.
+ *   - All calls are thread-compatible per context (one context = one caller at a time).
+ *   - Every function returns PHMM_OK (0) or a negative PHMM_E_* code; nothing throws or aborts.
+ *     A call that fails argument validation writes nothing.
+ */
+#ifndef PAIRHMM_B200_H
+#define PAIRHMM_B200_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define PHMM_VERSION 1
+
+/* error codes */
+#define PHMM_OK 0
+#define PHMM_E_ARG (-1)          /* null pointer, negative size, unknown precision */
+#define PHMM_E_OFFSETS (-2)      /* offsets not monotone, or a pair index out of range */
+#define PHMM_E_EMPTY (-3)        /* a pair references a read or haplotype of length 0 */
+#define PHMM_E_TOOLONG (-4)      /* a sequence exceeds PHMM_MAX_LEN */
+#define PHMM_E_CUDA (-5)         /* a CUDA runtime call failed (see phmm_last_cuda_error) */
+#define PHMM_E_NOMEM (-6)        /* host or device allocation failed */
+#define PHMM_E_UNSUPPORTED (-7)  /* device is not sm_100, or option not supported */
+
+#define PHMM_MAX_LEN (1 << 24)   /* longest read / haplotype accepted, in bases */
+
+/* precision modes of phmm_forward_batch */
+#define PHMM_FP32_RESCUE 0 /* fp32 recurrence; pairs whose fp32 result underflows are redone in fp64 */
+#define PHMM_FP64 1        /* fp64 recurrence for every pair */
+
+/* bits of the per-pair output flags */
+#define PHMM_FLAG_RESCUED 1u /* PHMM_FP32_RESCUE only: pair was recomputed in fp64 */
+#define PHMM_FLAG_LONG 2u    /* pair went through the multi-warp / multi-CTA rescaled wavefront path */
+
+typedef struct phmm_ctx phmm_ctx; /* opaque; owns workspaces, internal streams, the last stats */
+
+/* Tunables; zero-initialise and set `size = sizeof(phmm_options)`, fields left 0 take defaults. */
+typedef struct phmm_options {
+    uint32_t size;
+    /* fp32 rescue criterion (reading G16): the fp32 pass runs with scale constant
+     * C = 2^120; a pair is redone in fp64 iff its scaled sum is not finite or is
+     * < 2^rescue_log2_threshold.  Default -90  (<=> L < 2^-210 ~ 10^-63.2). */
+    int32_t rescue_log2_threshold;
+    /* haplotypes longer than this many bases use the long (CTA-chain) path; default 1280 */
+    int32_t long_min_hap_len;
+    /* target number of read rows per short-path task (a task streams several reads of one
+     * haplotype through one lane group); default 3072 */
+    int32_t task_rows;
+    /* upper bound, in bytes, for the per-read row-constant table built per launch group; batches
+     * needing more are processed in several slices.  Default 8 GiB. */
+    int64_t max_table_bytes;
+} phmm_options;
+
+/* One batch, CSR layout, natural order (a read, a haplotype and four
+ * read-length quality strings per pair; here reads and haplotypes are stored once and pairs
+ * reference them by index). */
+typedef struct phmm_batch {
+    int64_t n_reads, n_haps, n_pairs;
+    const int64_t* h_read_off;   /* host,   n_reads+1: byte offset of each read in the d_* read arrays */
+    const int64_t* h_hap_off;    /* host,   n_haps+1 : byte offset of each haplotype in d_hap_bases */
+    const uint8_t* d_read_bases; /* device, h_read_off[n_reads] bytes */
+    const uint8_t* d_qual_base;  /* device, same length: raw Phred base qualities */
+    const uint8_t* d_qual_ins;   /* device, same length: insertion gap-open qualities */
+    const uint8_t* d_qual_del;   /* device, same length: deletion gap-open qualities */
+    const uint8_t* d_qual_gcp;   /* device, same length: gap-continuation qualities */
+    const uint8_t* d_hap_bases;  /* device, h_hap_off[n_haps] bytes */
+    const int32_t* h_pair_read;  /* host,   n_pairs: read index of each pair */
+    const int32_t* h_pair_hap;   /* host,   n_pairs: haplotype index of each pair */
+} phmm_batch;
+
+/* Counters of the most recent phmm_forward_batch / phmm_forward_batch_host on a context. */
+typedef struct phmm_stats {
+    int64_t n_pairs;
+    int64_t cells;              /* sum over pairs of read_len * hap_len (the TCUPS numerator) */
+    int64_t n_short_pairs;      /* pairs run by the sub-warp systolic kernel */
+    int64_t n_long_pairs;       /* pairs run by the CTA-chain wavefront kernel */
+    int64_t n_rescued;          /* PHMM_FP32_RESCUE: pairs recomputed in fp64 (valid after the stream is synchronised) */
+    int64_t short_cells;        /* real cells of the short-path pairs */
+    int64_t short_padded_cells; /* lane-cells the short kernel actually swept (padding, fill/drain included) */
+    int64_t n_kernel_launches;  /* kernels enqueued by the call */
+    int64_t table_bytes;        /* row-constant table size of the call */
+    double host_batch_ms;       /* host time spent in the batcher */
+    int32_t n_short_warps;      /* warp tasks of the short kernel */
+    int32_t n_slices;
+} phmm_stats;
+
+/* Create a context on CUDA device `device`.  opt may be NULL.  Fails with PHMM_E_UNSUPPORTED on a
+ * device whose compute capability is not 10.x. */
+int phmm_create(phmm_ctx** ctx, int device, const phmm_options* opt);
+int phmm_destroy(phmm_ctx* ctx);
+
+/* log10 likelihood of every pair of `b`, in the caller's pair order.
+ *   precision    PHMM_FP32_RESCUE or PHMM_FP64
+ *   d_out_log10  device, n_pairs doubles (written)
+ *   d_out_flags  device, n_pairs bytes (written; may be NULL)
+ *   cuda_stream  a cudaStream_t (NULL = legacy default stream).  The call enqueues all device work on
+ *                it (internally forked streams are joined back) and returns without synchronising
+ *                the device; outputs are valid once the caller has synchronised `cuda_stream`.
+ * The host batcher ("batched according to their lengths") runs inside the call.
+ * For valid input every output is finite. */
+int phmm_forward_batch(phmm_ctx* ctx, const phmm_batch* b, int precision, double* d_out_log10,
+                       uint8_t* d_out_flags, void* cuda_stream);
+
+/* Same computation with ALL buffers on the host (the d_* members of `b` are host pointers, out
+ * pointers are host): the library copies the payload to the device, runs phmm_forward_batch, copies
+ * the results back and synchronises.  This is the end-to-end entry ("with transfer"). */
+int phmm_forward_batch_host(phmm_ctx* ctx, const phmm_batch* b, int precision, double* h_out_log10,
+                            uint8_t* h_out_flags);
+
+int phmm_get_stats(phmm_ctx* ctx, phmm_stats* out);
+const char* phmm_strerror(int code);
+/* cudaError_t value of the last failing CUDA call on this context (0 if none). */
+int phmm_last_cuda_error(phmm_ctx* ctx);
+
+/* Measured non-tensor arithmetic peak of the device, used as roofline denominator (BASELINE.json
+ * north_star: "fraction of the FP32 (and FP64) non-tensor roofline").  kind: 0 = scalar FFMA,
+ * 1 = packed FFMA2 (fma.rn.f32x2), 2 = DFMA.  Writes TFLOP/s (2 flops per lane-FMA) of a kernel of
+ * independent FMA chains, best of `reps` launches, timed with CUDA events. */
+int phmm_measure_peak(int device, int kind, int reps, double* out_tflops);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PAIRHMM_B200_H */

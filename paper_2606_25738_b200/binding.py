@@ -1,0 +1,216 @@
+"""Thin ctypes binding over libpairhmm_b200.so (include/pairhmm_b200.h).
+
+Argument marshalling only: every step of the PairHMM forward path runs inside the library's CUDA
+kernels.  PyTorch is used for device memory and streams.  There is NO CPU fallback: if the shared
+library is missing or cannot be loaded, importing a symbol from here raises.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libpairhmm_b200.so")
+
+PHMM_OK = 0
+PHMM_E_ARG, PHMM_E_OFFSETS, PHMM_E_EMPTY, PHMM_E_TOOLONG = -1, -2, -3, -4
+PHMM_E_CUDA, PHMM_E_NOMEM, PHMM_E_UNSUPPORTED = -5, -6, -7
+PHMM_FP32_RESCUE, PHMM_FP64 = 0, 1
+PHMM_FLAG_RESCUED, PHMM_FLAG_LONG = 1, 2
+
+EXPORTS = ["phmm_create", "phmm_destroy", "phmm_forward_batch", "phmm_forward_batch_host", "phmm_get_stats",
+           "phmm_strerror", "phmm_last_cuda_error", "phmm_measure_peak"]
+
+
+class phmm_options(ctypes.Structure):
+    _fields_ = [("size", ctypes.c_uint32), ("rescue_log2_threshold", ctypes.c_int32),
+                ("long_min_hap_len", ctypes.c_int32), ("task_rows", ctypes.c_int32),
+                ("max_table_bytes", ctypes.c_int64)]
+
+
+class phmm_batch(ctypes.Structure):
+    _fields_ = [("n_reads", ctypes.c_int64), ("n_haps", ctypes.c_int64), ("n_pairs", ctypes.c_int64),
+                ("h_read_off", ctypes.c_void_p), ("h_hap_off", ctypes.c_void_p),
+                ("d_read_bases", ctypes.c_void_p), ("d_qual_base", ctypes.c_void_p), ("d_qual_ins", ctypes.c_void_p),
+                ("d_qual_del", ctypes.c_void_p), ("d_qual_gcp", ctypes.c_void_p), ("d_hap_bases", ctypes.c_void_p),
+                ("h_pair_read", ctypes.c_void_p), ("h_pair_hap", ctypes.c_void_p)]
+
+
+class phmm_stats(ctypes.Structure):
+    _fields_ = [("n_pairs", ctypes.c_int64), ("cells", ctypes.c_int64), ("n_short_pairs", ctypes.c_int64),
+                ("n_long_pairs", ctypes.c_int64), ("n_rescued", ctypes.c_int64), ("short_cells", ctypes.c_int64),
+                ("short_padded_cells", ctypes.c_int64), ("n_kernel_launches", ctypes.c_int64),
+                ("table_bytes", ctypes.c_int64), ("host_batch_ms", ctypes.c_double),
+                ("n_short_warps", ctypes.c_int32), ("n_slices", ctypes.c_int32)]
+
+    def as_dict(self):
+        return {k: getattr(self, k) for k, _ in self._fields_}
+
+
+def build(force: bool = False) -> str:
+    """Compile the library in-tree with nvcc for sm_100a (csrc/build.sh)."""
+    src_dir = os.path.join(_HERE, "csrc")
+    srcs = [os.path.join(src_dir, f) for f in os.listdir(src_dir)] + [os.path.join(_HERE, "..", "include", "pairhmm_b200.h")]
+    stale = (not os.path.exists(LIB_PATH)) or any(os.path.getmtime(s) > os.path.getmtime(LIB_PATH) for s in srcs)
+    if force or stale:
+        subprocess.check_call(["sh", os.path.join(src_dir, "build.sh")])
+    return LIB_PATH
+
+
+_lib = None
+
+
+def lib() -> ctypes.CDLL:
+    """The loaded C-ABI library.  Raises (loudly) when it has not been built."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise RuntimeError("libpairhmm_b200.so is missing: run paper_2606_25738_b200.binding.build() "
+                               "(or __graft_entry__.build()); there is no CPU fallback")
+        L = ctypes.CDLL(LIB_PATH)
+        L.phmm_create.argtypes = [ctypes.POINTER(ctypes.c_void_p), ctypes.c_int, ctypes.POINTER(phmm_options)]
+        L.phmm_create.restype = ctypes.c_int
+        L.phmm_destroy.argtypes = [ctypes.c_void_p]
+        L.phmm_destroy.restype = ctypes.c_int
+        L.phmm_forward_batch.argtypes = [ctypes.c_void_p, ctypes.POINTER(phmm_batch), ctypes.c_int, ctypes.c_void_p,
+                                         ctypes.c_void_p, ctypes.c_void_p]
+        L.phmm_forward_batch.restype = ctypes.c_int
+        L.phmm_forward_batch_host.argtypes = [ctypes.c_void_p, ctypes.POINTER(phmm_batch), ctypes.c_int,
+                                              ctypes.c_void_p, ctypes.c_void_p]
+        L.phmm_forward_batch_host.restype = ctypes.c_int
+        L.phmm_get_stats.argtypes = [ctypes.c_void_p, ctypes.POINTER(phmm_stats)]
+        L.phmm_get_stats.restype = ctypes.c_int
+        L.phmm_strerror.argtypes = [ctypes.c_int]
+        L.phmm_strerror.restype = ctypes.c_char_p
+        L.phmm_last_cuda_error.argtypes = [ctypes.c_void_p]
+        L.phmm_last_cuda_error.restype = ctypes.c_int
+        L.phmm_measure_peak.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.POINTER(ctypes.c_double)]
+        L.phmm_measure_peak.restype = ctypes.c_int
+        _lib = L
+    return _lib
+
+
+class PhmmError(RuntimeError):
+    def __init__(self, code: int, cuda: int = 0):
+        self.code = code
+        msg = lib().phmm_strerror(code).decode()
+        super().__init__("phmm error %d: %s%s" % (code, msg, (" (cudaError %d)" % cuda) if cuda else ""))
+
+
+def _hp(a: np.ndarray) -> int:
+    return a.ctypes.data
+
+
+class DeviceBatch:
+    """A workloads.Batch-like object with its payload uploaded to the GPU (torch uint8 tensors) and the
+    offset / pair arrays kept on the host, i.e. exactly the phmm_batch layout."""
+
+    def __init__(self, batch, device="cuda:0"):
+        import torch
+        self.host = batch
+        self.device = torch.device(device)
+        self.read_off = np.ascontiguousarray(batch.read_off, dtype=np.int64)
+        self.hap_off = np.ascontiguousarray(batch.hap_off, dtype=np.int64)
+        self.pair_read = np.ascontiguousarray(batch.pair_read, dtype=np.int32)
+        self.pair_hap = np.ascontiguousarray(batch.pair_hap, dtype=np.int32)
+        up = lambda a: torch.from_numpy(np.ascontiguousarray(a, dtype=np.uint8)).to(self.device)
+        self.t = [up(batch.read_bases), up(batch.qual_base), up(batch.qual_ins), up(batch.qual_del),
+                  up(batch.qual_gcp), up(batch.hap_bases)]
+
+    def with_pairs(self, pair_read, pair_hap) -> "DeviceBatch":
+        o = object.__new__(DeviceBatch)
+        o.__dict__.update(self.__dict__)
+        o.pair_read = np.ascontiguousarray(pair_read, dtype=np.int32)
+        o.pair_hap = np.ascontiguousarray(pair_hap, dtype=np.int32)
+        return o
+
+    @property
+    def n_pairs(self):
+        return len(self.pair_read)
+
+    def c_struct(self) -> phmm_batch:
+        ptr = lambda t: t.data_ptr() if t.numel() else 0
+        return phmm_batch(len(self.read_off) - 1, len(self.hap_off) - 1, len(self.pair_read), _hp(self.read_off),
+                          _hp(self.hap_off), ptr(self.t[0]), ptr(self.t[1]), ptr(self.t[2]), ptr(self.t[3]),
+                          ptr(self.t[4]), ptr(self.t[5]), _hp(self.pair_read), _hp(self.pair_hap))
+
+
+class Context:
+    """phmm_ctx wrapper."""
+
+    def __init__(self, device: int = 0, **opts):
+        self._h = ctypes.c_void_p()
+        o = phmm_options()
+        o.size = ctypes.sizeof(phmm_options)
+        for k, v in opts.items():
+            setattr(o, k, v)
+        rc = lib().phmm_create(ctypes.byref(self._h), device, ctypes.byref(o))
+        if rc != PHMM_OK:
+            raise PhmmError(rc)
+        self.device = device
+
+    def close(self):
+        if self._h:
+            lib().phmm_destroy(self._h)
+            self._h = ctypes.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def forward_batch(self, db: DeviceBatch, precision: int = PHMM_FP32_RESCUE, out=None, flags=None, stream=None,
+                      sync: bool = True):
+        """phmm_forward_batch: returns (log10 likelihoods [float64 cuda tensor], flags [uint8 cuda tensor])."""
+        import torch
+        n = db.n_pairs
+        if out is None:
+            out = torch.empty(n, dtype=torch.float64, device=db.device)
+        if flags is None:
+            flags = torch.zeros(n, dtype=torch.uint8, device=db.device)
+        st = torch.cuda.current_stream(db.device) if stream is None else stream
+        cb = db.c_struct()
+        rc = lib().phmm_forward_batch(self._h, ctypes.byref(cb), precision, out.data_ptr() if n else 0,
+                                      flags.data_ptr() if n else 0, st.cuda_stream)
+        if rc != PHMM_OK:
+            raise PhmmError(rc, lib().phmm_last_cuda_error(self._h))
+        if sync:
+            st.synchronize()
+        return out, flags
+
+    def forward_batch_host(self, batch, precision: int = PHMM_FP32_RESCUE):
+        """phmm_forward_batch_host: everything on the host (numpy); copies are inside the call."""
+        arrs = [np.ascontiguousarray(a, dtype=np.uint8) for a in (batch.read_bases, batch.qual_base, batch.qual_ins,
+                                                                  batch.qual_del, batch.qual_gcp, batch.hap_bases)]
+        ro = np.ascontiguousarray(batch.read_off, dtype=np.int64)
+        ho = np.ascontiguousarray(batch.hap_off, dtype=np.int64)
+        pr = np.ascontiguousarray(batch.pair_read, dtype=np.int32)
+        ph = np.ascontiguousarray(batch.pair_hap, dtype=np.int32)
+        n = len(pr)
+        out = np.empty(n, dtype=np.float64)
+        flags = np.zeros(n, dtype=np.uint8)
+        cb = phmm_batch(len(ro) - 1, len(ho) - 1, n, _hp(ro), _hp(ho), *[_hp(a) for a in arrs], _hp(pr), _hp(ph))
+        rc = lib().phmm_forward_batch_host(self._h, ctypes.byref(cb), precision, _hp(out), _hp(flags))
+        if rc != PHMM_OK:
+            raise PhmmError(rc, lib().phmm_last_cuda_error(self._h))
+        return out, flags
+
+    def stats(self) -> dict:
+        s = phmm_stats()
+        rc = lib().phmm_get_stats(self._h, ctypes.byref(s))
+        if rc != PHMM_OK:
+            raise PhmmError(rc)
+        return s.as_dict()
+
+
+def measure_peak(kind: int, device: int = 0, reps: int = 5) -> float:
+    """TFLOP/s of independent FMA chains: kind 0 FFMA, 1 FFMA2, 2 DFMA."""
+    v = ctypes.c_double()
+    rc = lib().phmm_measure_peak(device, kind, reps, ctypes.byref(v))
+    if rc != PHMM_OK:
+        raise PhmmError(rc)
+    return v.value

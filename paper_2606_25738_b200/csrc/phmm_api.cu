@@ -1,0 +1,373 @@
+// C ABI of libpairhmm_b200.so (include/pairhmm_b200.h): context, workspaces, launch orchestration.
+#include <math.h>
+#include <stdio.h>
+#include <stdlib.h>
+#include <string.h>
+
+#include <chrono>
+#include <new>
+#include <vector>
+
+#include "../../include/pairhmm_b200.h"
+#include "phmm_batcher.h"
+#include "phmm_kernels.h"
+
+using namespace phmm;
+
+namespace {
+
+struct DevBuf {  // grow-only device buffer
+    void* p = nullptr;
+    size_t cap = 0;
+    cudaError_t need(size_t bytes) {
+        if (bytes <= cap) return cudaSuccess;
+        if (p) { cudaError_t e = cudaFree(p); p = nullptr; cap = 0; if (e != cudaSuccess) return e; }
+        size_t want = bytes + bytes / 8 + 256;
+        cudaError_t e = cudaMalloc(&p, want);
+        if (e != cudaSuccess) { e = cudaMalloc(&p, bytes); want = bytes; }
+        if (e == cudaSuccess) cap = want;
+        return e;
+    }
+    void release() { if (p) cudaFree(p); p = nullptr; cap = 0; }
+};
+struct PinBuf {  // grow-only pinned host staging buffer
+    void* p = nullptr;
+    size_t cap = 0;
+    cudaError_t need(size_t bytes) {
+        if (bytes <= cap) return cudaSuccess;
+        if (p) { cudaFreeHost(p); p = nullptr; cap = 0; }
+        size_t want = bytes + bytes / 8 + 256;
+        cudaError_t e = cudaMallocHost(&p, want);
+        if (e == cudaSuccess) cap = want;
+        return e;
+    }
+    void release() { if (p) cudaFreeHost(p); p = nullptr; cap = 0; }
+};
+
+}  // namespace
+
+struct phmm_ctx {
+    int device = 0;
+    int n_sm = 0;
+    phmm_options opt;
+    phmm_stats stats;
+    int last_cuda = 0;
+    cudaEvent_t ev_upload = nullptr;  // staging buffers are free again once this has fired
+    bool upload_pending = false;
+    DevBuf d_lut, d_read_off, d_hap_off, d_pair_read, d_pair_hap, d_table, d_tasks, d_warp_first, d_srt_read, d_srt_out;
+    DevBuf d_counters, d_rescue, d_items, d_boundary, d_progress, d_scratch;
+    DevBuf d_payload, d_out, d_flags;  // phmm_forward_batch_host only
+    PinBuf h_stage;
+    std::vector<uint8_t> is_short;
+    ShortPlan plan;
+    int chain_grid[2] = {0, 0};
+};
+
+#define CK(call)                                                    \
+    do {                                                            \
+        cudaError_t e__ = (call);                                   \
+        if (e__ != cudaSuccess) { ctx->last_cuda = (int)e__; return e__ == cudaErrorMemoryAllocation ? PHMM_E_NOMEM : PHMM_E_CUDA; } \
+    } while (0)
+
+extern "C" const char* phmm_strerror(int code) {
+    switch (code) {
+        case PHMM_OK: return "ok";
+        case PHMM_E_ARG: return "invalid argument";
+        case PHMM_E_OFFSETS: return "offsets not monotone or pair index out of range";
+        case PHMM_E_EMPTY: return "pair references an empty read or haplotype";
+        case PHMM_E_TOOLONG: return "sequence or batch too long";
+        case PHMM_E_CUDA: return "CUDA error";
+        case PHMM_E_NOMEM: return "out of memory";
+        case PHMM_E_UNSUPPORTED: return "unsupported device or option";
+        default: return "unknown error";
+    }
+}
+
+extern "C" int phmm_create(phmm_ctx** out, int device, const phmm_options* opt) {
+    if (!out) return PHMM_E_ARG;
+    *out = nullptr;
+    cudaDeviceProp prop;
+    if (cudaGetDeviceProperties(&prop, device) != cudaSuccess) return PHMM_E_CUDA;
+    if (prop.major != 10) return PHMM_E_UNSUPPORTED;
+    phmm_ctx* ctx = new (std::nothrow) phmm_ctx();
+    if (!ctx) return PHMM_E_NOMEM;
+    ctx->device = device;
+    ctx->n_sm = prop.multiProcessorCount;
+    memset(&ctx->opt, 0, sizeof(ctx->opt));
+    if (opt) memcpy(&ctx->opt, opt, opt->size < sizeof(phmm_options) ? opt->size : sizeof(phmm_options));
+    if (ctx->opt.rescue_log2_threshold == 0) ctx->opt.rescue_log2_threshold = -90;
+    if (ctx->opt.long_min_hap_len <= 0 || ctx->opt.long_min_hap_len > SHORT_MAX_K) ctx->opt.long_min_hap_len = SHORT_MAX_K;
+    if (ctx->opt.task_rows <= 0) ctx->opt.task_rows = 3072;
+    if (ctx->opt.max_table_bytes <= 0) ctx->opt.max_table_bytes = (int64_t)64 << 30;
+    memset(&ctx->stats, 0, sizeof(ctx->stats));
+    if (cudaSetDevice(device) != cudaSuccess) { delete ctx; return PHMM_E_CUDA; }
+    if (cudaEventCreateWithFlags(&ctx->ev_upload, cudaEventDisableTiming) != cudaSuccess) { delete ctx; return PHMM_E_CUDA; }
+    // 10^(-q/10) for q = 0..255, the paper's "q64" table
+    double lut[256];
+    for (int q = 0; q < 256; q++) lut[q] = pow(10.0, -(double)q / 10.0);
+    if (ctx->d_lut.need(sizeof(lut)) != cudaSuccess || cudaMemcpy(ctx->d_lut.p, lut, sizeof(lut), cudaMemcpyHostToDevice) != cudaSuccess) {
+        phmm_destroy(ctx);
+        return PHMM_E_CUDA;
+    }
+    ctx->chain_grid[0] = chain_ctas_per_sm(false) * ctx->n_sm;
+    ctx->chain_grid[1] = chain_ctas_per_sm(true) * ctx->n_sm;
+    *out = ctx;
+    return PHMM_OK;
+}
+
+extern "C" int phmm_destroy(phmm_ctx* ctx) {
+    if (!ctx) return PHMM_E_ARG;
+    cudaSetDevice(ctx->device);
+    cudaDeviceSynchronize();
+    DevBuf* bufs[] = {&ctx->d_lut, &ctx->d_read_off, &ctx->d_hap_off, &ctx->d_pair_read, &ctx->d_pair_hap, &ctx->d_table,
+                      &ctx->d_tasks, &ctx->d_warp_first, &ctx->d_srt_read, &ctx->d_srt_out, &ctx->d_counters, &ctx->d_rescue,
+                      &ctx->d_items, &ctx->d_boundary, &ctx->d_progress, &ctx->d_scratch, &ctx->d_payload, &ctx->d_out, &ctx->d_flags};
+    for (DevBuf* b : bufs) b->release();
+    ctx->h_stage.release();
+    if (ctx->ev_upload) cudaEventDestroy(ctx->ev_upload);
+    delete ctx;
+    return PHMM_OK;
+}
+
+extern "C" int phmm_get_stats(phmm_ctx* ctx, phmm_stats* out) {
+    if (!ctx || !out) return PHMM_E_ARG;
+    if (ctx->d_counters.p && ctx->stats.n_pairs > 0) {  // rescue count lives on the device until the caller has synchronised
+        int n = 0;
+        cudaSetDevice(ctx->device);
+        if (cudaMemcpy(&n, ctx->d_counters.p, sizeof(int), cudaMemcpyDeviceToHost) == cudaSuccess && ctx->stats.n_short_warps > 0)
+            ctx->stats.n_rescued = n;
+    }
+    *out = ctx->stats;
+    return PHMM_OK;
+}
+
+extern "C" int phmm_last_cuda_error(phmm_ctx* ctx) { return ctx ? ctx->last_cuda : 0; }
+
+// ---------------------------------------------------------------- staging helper
+namespace {
+struct Stager {  // packs several host arrays into the pinned buffer and copies them with one memcpy each
+    phmm_ctx* ctx;
+    cudaStream_t st;
+    size_t used = 0;
+    int upload(DevBuf& dst, const void* src, size_t bytes) {
+        if (bytes == 0) return PHMM_OK;
+        CK(dst.need(bytes));
+        const size_t at = (used + 255) & ~(size_t)255;
+        if (at + bytes > ctx->h_stage.cap) return PHMM_E_NOMEM;
+        memcpy((char*)ctx->h_stage.p + at, src, bytes);
+        used = at + bytes;
+        CK(cudaMemcpyAsync(dst.p, (char*)ctx->h_stage.p + at, bytes, cudaMemcpyHostToDevice, st));
+        return PHMM_OK;
+    }
+};
+}  // namespace
+
+#define RC(call) do { int rc__ = (call); if (rc__ != PHMM_OK) return rc__; } while (0)
+
+extern "C" int phmm_forward_batch(phmm_ctx* ctx, const phmm_batch* b, int precision, double* d_out, uint8_t* d_flags,
+                                  void* cuda_stream) {
+    if (!ctx || !b) return PHMM_E_ARG;
+    if (precision != PHMM_FP32_RESCUE && precision != PHMM_FP64) return PHMM_E_ARG;
+    if (b->n_pairs < 0 || b->n_reads < 0 || b->n_haps < 0) return PHMM_E_ARG;
+    memset(&ctx->stats, 0, sizeof(ctx->stats));
+    if (b->n_pairs == 0) return PHMM_OK;
+    if (!d_out || !b->d_read_bases || !b->d_qual_base || !b->d_qual_ins || !b->d_qual_del || !b->d_qual_gcp || !b->d_hap_bases)
+        return PHMM_E_ARG;
+    HostBatchView hv = {b->n_reads, b->n_haps, b->n_pairs, b->h_read_off, b->h_hap_off, b->h_pair_read, b->h_pair_hap};
+    RC(validate_batch(hv));
+    CK(cudaSetDevice(ctx->device));
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const auto t0 = std::chrono::steady_clock::now();
+    const bool fp64 = precision == PHMM_FP64;
+    const int64_t np = b->n_pairs;
+
+    // ---- classify: short (sub-warp systolic fp32 kernel) / chain-sequential (one warp per pair) / chain-strips
+    const int strip_cols = chain_strip_cols(fp64);
+    ctx->is_short.assign((size_t)np, 0);
+    std::vector<int> seq_pairs, strip_pairs;  // chain kernel work lists (caller pair indices)
+    int64_t cells = 0, long_cells = 0;
+    int max_seq_l = 0;
+    for (int64_t p = 0; p < np; p++) {
+        const int r = b->h_pair_read[p], h = b->h_pair_hap[p];
+        const int64_t l = b->h_read_off[r + 1] - b->h_read_off[r], k = b->h_hap_off[h + 1] - b->h_hap_off[h];
+        cells += l * k;
+        const bool is_long = k > ctx->opt.long_min_hap_len || l > 4096;
+        if (is_long) { strip_pairs.push_back((int)p); long_cells += l * k; }
+        else if (fp64) { seq_pairs.push_back((int)p); if (l > max_seq_l) max_seq_l = (int)l; }
+        else { ctx->is_short[(size_t)p] = 1; if (l > max_seq_l) max_seq_l = (int)l; }
+    }
+    ctx->stats.n_pairs = np;
+    ctx->stats.cells = cells;
+    ctx->stats.n_long_pairs = (int64_t)strip_pairs.size();
+    ctx->stats.n_short_pairs = np - (int64_t)strip_pairs.size();
+    if (!fp64) plan_short(hv, ctx->is_short.data(), SHORT_N2, ctx->opt.task_rows, &ctx->plan);
+    else { ctx->plan.tasks.clear(); ctx->plan.warp_first.assign(1, 0); ctx->plan.srt_read.clear(); ctx->plan.srt_out.clear(); ctx->plan.cells = 0; ctx->plan.padded_cells = 0; }
+    const ShortPlan& pl = ctx->plan;
+    const int n_warps = (int)pl.warp_first.size() - 1;
+    ctx->stats.short_cells = pl.cells;
+    ctx->stats.short_padded_cells = pl.padded_cells;
+    ctx->stats.n_short_warps = n_warps;
+
+    // ---- strip items of the long pairs (pair-major, strips ascending: ticket order = dependency order)
+    std::vector<ChainItem> items;
+    int64_t n_bnd_blocks = 0;
+    int n_prog = 0;
+    for (int p : strip_pairs) {
+        const int r = b->h_pair_read[p], h = b->h_pair_hap[p];
+        const int64_t l = b->h_read_off[r + 1] - b->h_read_off[r], k = b->h_hap_off[h + 1] - b->h_hap_off[h];
+        const int ns = (int)((k + strip_cols - 1) / strip_cols);
+        const int64_t nblk = (l + 1 + 31) / 32;
+        for (int s = 0; s < ns; s++) items.push_back(ChainItem{p, s, n_prog, 0, n_bnd_blocks});
+        n_bnd_blocks += (int64_t)(ns > 1 ? ns - 1 : 0) * nblk;
+        n_prog += ns;  // one counter per strip (the last one is unused)
+    }
+    const auto t1 = std::chrono::steady_clock::now();
+    ctx->stats.host_batch_ms = std::chrono::duration<double, std::milli>(t1 - t0).count();
+
+    // ---- uploads (one pinned staging buffer, reused once the previous call's copies have completed)
+    if (ctx->upload_pending) { CK(cudaEventSynchronize(ctx->ev_upload)); ctx->upload_pending = false; }
+    const size_t n_seq = fp64 ? seq_pairs.size() : 0;
+    size_t stage_bytes = 4096 + (size_t)(b->n_reads + 1) * 8 + (size_t)(b->n_haps + 1) * 8 + (size_t)np * 8 +
+                         pl.tasks.size() * sizeof(ShortTask) + pl.warp_first.size() * 4 + pl.srt_read.size() * 8 +
+                         items.size() * sizeof(ChainItem) + n_seq * 4 + 16 * 256;
+    CK(ctx->h_stage.need(stage_bytes));
+    Stager sg{ctx, st};
+    RC(sg.upload(ctx->d_read_off, b->h_read_off, (size_t)(b->n_reads + 1) * 8));
+    RC(sg.upload(ctx->d_hap_off, b->h_hap_off, (size_t)(b->n_haps + 1) * 8));
+    RC(sg.upload(ctx->d_pair_read, b->h_pair_read, (size_t)np * 4));
+    RC(sg.upload(ctx->d_pair_hap, b->h_pair_hap, (size_t)np * 4));
+    RC(sg.upload(ctx->d_tasks, pl.tasks.data(), pl.tasks.size() * sizeof(ShortTask)));
+    RC(sg.upload(ctx->d_warp_first, pl.warp_first.data(), pl.warp_first.size() * 4));
+    RC(sg.upload(ctx->d_srt_read, pl.srt_read.data(), pl.srt_read.size() * 4));
+    RC(sg.upload(ctx->d_srt_out, pl.srt_out.data(), pl.srt_out.size() * 4));
+    RC(sg.upload(ctx->d_items, items.data(), items.size() * sizeof(ChainItem)));
+    // counters: [0] rescue count (= n_items of the rescue launch)  [1] ticket rescue  [2] n strip items  [3] ticket strips
+    //           [4] n sequential fp64 items  [5] ticket sequential
+    int h_counters[8] = {0, 0, (int)items.size(), 0, (int)n_seq, 0, 0, 0};
+    RC(sg.upload(ctx->d_counters, h_counters, sizeof(h_counters)));
+    // rescue list (fp32 mode: filled by the short kernel) / sequential list (fp64 mode: all non-long pairs)
+    CK(ctx->d_rescue.need((size_t)np * 4 + 4));
+    if (n_seq) {
+        const size_t at = (sg.used + 255) & ~(size_t)255;
+        memcpy((char*)ctx->h_stage.p + at, seq_pairs.data(), n_seq * 4);
+        sg.used = at + n_seq * 4;
+        CK(cudaMemcpyAsync(ctx->d_rescue.p, (char*)ctx->h_stage.p + at, n_seq * 4, cudaMemcpyHostToDevice, st));
+    }
+    CK(cudaEventRecord(ctx->ev_upload, st));
+    ctx->upload_pending = true;
+
+    DevBatch db;
+    db.read_bases = b->d_read_bases; db.qual_base = b->d_qual_base; db.qual_ins = b->d_qual_ins;
+    db.qual_del = b->d_qual_del; db.qual_gcp = b->d_qual_gcp; db.hap_bases = b->d_hap_bases;
+    db.read_off = (const int64_t*)ctx->d_read_off.p; db.hap_off = (const int64_t*)ctx->d_hap_off.p;
+    db.n_reads = b->n_reads; db.n_haps = b->n_haps;
+    int* counters = (int*)ctx->d_counters.p;
+    int launches = 0;
+
+    // ---- short path: row-constant table, systolic kernel, then fp64 rescue of what underflowed
+    if (n_warps > 0) {
+        const size_t table_bytes = (size_t)(b->h_read_off[b->n_reads] + b->n_reads + 1) * 32;
+        if ((int64_t)table_bytes > ctx->opt.max_table_bytes) return PHMM_E_NOMEM;
+        CK(ctx->d_table.need(table_bytes));
+        ctx->stats.table_bytes = (int64_t)table_bytes;
+        CK(launch_lut_table(db, (const double*)ctx->d_lut.p, (float*)ctx->d_table.p, st));
+        ShortLaunch sl;
+        sl.table = (const float*)ctx->d_table.p;
+        sl.tasks = (const ShortTask*)ctx->d_tasks.p;
+        sl.warp_first = (const int*)ctx->d_warp_first.p;
+        sl.n_warps = n_warps;
+        sl.srt_read = (const int*)ctx->d_srt_read.p;
+        sl.srt_out = (const int*)ctx->d_srt_out.p;
+        sl.out = d_out;
+        sl.flags = d_flags;
+        sl.rescue_thr = (float)ldexp(1.0, ctx->opt.rescue_log2_threshold);
+        sl.rescue_count = counters + 0;
+        sl.rescue_list = (int*)ctx->d_rescue.p;
+        CK(launch_short_f32(db, sl, st));
+        launches += 2;
+    }
+    // sequential chain launch: fp32 mode = rescue list (device-side count), fp64 mode = all non-long pairs
+    if (n_warps > 0 || n_seq > 0) {
+        const int grid = ctx->chain_grid[1];
+        const int64_t blocks = (max_seq_l + 1 + 31) / 32 + 1;
+        const int max_strips_seq = (ctx->opt.long_min_hap_len + chain_strip_cols(true) - 1) / chain_strip_cols(true);
+        size_t scratch = max_strips_seq > 1 ? (size_t)grid * chain_warps_per_cta() * 2 * blocks * chain_block_bytes(true) : 256;
+        CK(ctx->d_scratch.need(scratch));
+        ChainLaunch cl;
+        memset(&cl, 0, sizeof(cl));
+        cl.items = (const ChainItem*)ctx->d_rescue.p;
+        cl.n_items = counters + (fp64 ? 4 : 0);
+        cl.ticket = counters + (fp64 ? 5 : 1);
+        cl.pair_read = (const int*)ctx->d_pair_read.p;
+        cl.pair_hap = (const int*)ctx->d_pair_hap.p;
+        cl.lut = (const double*)ctx->d_lut.p;
+        cl.boundary = ctx->d_scratch.p;
+        cl.scratch_blocks = blocks;
+        cl.progress = nullptr;
+        cl.out = d_out;
+        cl.flags = d_flags;
+        cl.flag_bits = fp64 ? 0 : PHMM_FLAG_RESCUED;
+        cl.log2C = 0;
+        CK(launch_chain(db, cl, true, true, grid, st));
+        launches++;
+    }
+    // ---- long path: concurrent strips in the requested precision
+    if (!items.empty()) {
+        CK(ctx->d_boundary.need((size_t)(n_bnd_blocks + 1) * chain_block_bytes(fp64)));
+        CK(ctx->d_progress.need((size_t)n_prog * 4 + 4));
+        CK(cudaMemsetAsync(ctx->d_progress.p, 0, (size_t)n_prog * 4 + 4, st));
+        ChainLaunch cl;
+        memset(&cl, 0, sizeof(cl));
+        cl.items = (const ChainItem*)ctx->d_items.p;
+        cl.n_items = counters + 2;
+        cl.ticket = counters + 3;
+        cl.pair_read = (const int*)ctx->d_pair_read.p;
+        cl.pair_hap = (const int*)ctx->d_pair_hap.p;
+        cl.lut = (const double*)ctx->d_lut.p;
+        cl.boundary = ctx->d_boundary.p;
+        cl.scratch_blocks = 0;
+        cl.progress = (int*)ctx->d_progress.p;
+        cl.out = d_out;
+        cl.flags = d_flags;
+        cl.flag_bits = PHMM_FLAG_LONG;
+        cl.log2C = 0;
+        CK(launch_chain(db, cl, fp64, false, ctx->chain_grid[fp64 ? 1 : 0], st));
+        launches++;
+    }
+    ctx->stats.n_kernel_launches = launches;
+    ctx->stats.n_slices = 1;
+    return PHMM_OK;
+}
+
+// ---------------------------------------------------------------- end-to-end entry with host buffers
+extern "C" int phmm_forward_batch_host(phmm_ctx* ctx, const phmm_batch* b, int precision, double* h_out, uint8_t* h_flags) {
+    if (!ctx || !b) return PHMM_E_ARG;
+    if (b->n_pairs < 0 || b->n_reads < 0 || b->n_haps < 0) return PHMM_E_ARG;
+    if (b->n_pairs == 0) { memset(&ctx->stats, 0, sizeof(ctx->stats)); return PHMM_OK; }
+    if (!h_out || !b->h_read_off || !b->h_hap_off) return PHMM_E_ARG;
+    HostBatchView hv = {b->n_reads, b->n_haps, b->n_pairs, b->h_read_off, b->h_hap_off, b->h_pair_read, b->h_pair_hap};
+    RC(validate_batch(hv));
+    CK(cudaSetDevice(ctx->device));
+    const size_t R = (size_t)b->h_read_off[b->n_reads], H = (size_t)b->h_hap_off[b->n_haps];
+    const size_t Ra = (R + 255) & ~(size_t)255, Ha = (H + 255) & ~(size_t)255;
+    CK(ctx->d_payload.need(5 * Ra + Ha + 256));
+    CK(ctx->d_out.need((size_t)b->n_pairs * 8));
+    CK(ctx->d_flags.need((size_t)b->n_pairs));
+    uint8_t* base = (uint8_t*)ctx->d_payload.p;
+    const uint8_t* src[5] = {b->d_read_bases, b->d_qual_base, b->d_qual_ins, b->d_qual_del, b->d_qual_gcp};
+    cudaStream_t st = nullptr;
+    for (int i = 0; i < 5; i++) {
+        if (!src[i]) return PHMM_E_ARG;
+        CK(cudaMemcpyAsync(base + i * Ra, src[i], R, cudaMemcpyHostToDevice, st));
+    }
+    if (!b->d_hap_bases) return PHMM_E_ARG;
+    CK(cudaMemcpyAsync(base + 5 * Ra, b->d_hap_bases, H, cudaMemcpyHostToDevice, st));
+    phmm_batch db = *b;
+    db.d_read_bases = base; db.d_qual_base = base + Ra; db.d_qual_ins = base + 2 * Ra; db.d_qual_del = base + 3 * Ra;
+    db.d_qual_gcp = base + 4 * Ra; db.d_hap_bases = base + 5 * Ra;
+    RC(phmm_forward_batch(ctx, &db, precision, (double*)ctx->d_out.p, (uint8_t*)ctx->d_flags.p, st));
+    CK(cudaMemcpyAsync(h_out, ctx->d_out.p, (size_t)b->n_pairs * 8, cudaMemcpyDeviceToHost, st));
+    if (h_flags) CK(cudaMemcpyAsync(h_flags, ctx->d_flags.p, (size_t)b->n_pairs, cudaMemcpyDeviceToHost, st));
+    CK(cudaStreamSynchronize(st));
+    return PHMM_OK;
+}

@@ -1,0 +1,40 @@
+// Host-side batcher ("pairs are batched according to their
+// lengths and run on dedicated kernels").  Pure host C++; no CUDA types.
+//
+// Short pairs (haplotype fits one warp) are grouped BY HAPLOTYPE: a "task" is a run of reads that
+// are all aligned against the same haplotype by one group of g = ceil(k / columns-per-lane)
+// consecutive lanes, the reads streaming through the lanes back to back, so the systolic
+// fill/drain (2g steps) is paid once per task instead of once per pair.  Tasks are then packed
+// into 32-lane warps: tasks of similar duration share a warp (all groups of a warp run the same
+// number of steps) and the lane counts are bin-packed (largest-fit-first).
+#pragma once
+#include <stdint.h>
+#include <vector>
+
+#include "phmm_kernels.h"
+
+namespace phmm {
+
+struct HostBatchView {
+    int64_t n_reads, n_haps, n_pairs;
+    const int64_t *read_off, *hap_off;
+    const int32_t *pair_read, *pair_hap;
+};
+
+struct ShortPlan {
+    std::vector<ShortTask> tasks;   // ordered by warp
+    std::vector<int> warp_first;    // n_warps + 1
+    std::vector<int> srt_read;      // read index per sorted pair
+    std::vector<int> srt_out;       // caller's pair index per sorted pair
+    int64_t cells = 0;              // real cells of the short pairs
+    int64_t padded_cells = 0;       // lane-cells swept: sum over warps of steps * 32 lanes * columns-per-lane
+    int max_read_len = 0;
+};
+
+// is_short[p] != 0 selects the pairs to plan.  cols_per_lane = 2*NV of the kernel.
+void plan_short(const HostBatchView& b, const uint8_t* is_short, int cols_per_lane, int task_rows, ShortPlan* out);
+
+// Validation of offsets / indices / lengths; returns a PHMM_E_* code or 0.
+int validate_batch(const HostBatchView& b);
+
+}  // namespace phmm

@@ -1,0 +1,75 @@
+// Internal host-side interface between the API / batcher (api.cpp-ish code in phmm_api.cu) and the
+// kernels.  Plain structs of device pointers; nothing here crosses the C ABI.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace phmm {
+
+constexpr int SHORT_NV = 16;              // columns per virtual lane, fp32 short kernel
+constexpr int SHORT_N2 = 2 * SHORT_NV;    // columns per CUDA lane
+constexpr int SHORT_MAX_K = 32 * SHORT_N2;  // 1024: widest haplotype one warp covers
+constexpr int CHAIN_NV_F32 = 16;
+constexpr int CHAIN_NV_F64 = 8;
+constexpr int SHORT_WARPS_PER_CTA = 4;
+
+struct DevBatch {  // device mirrors of the batch
+    const uint8_t *read_bases, *qual_base, *qual_ins, *qual_del, *qual_gcp, *hap_bases;
+    const int64_t *read_off, *hap_off;  // device copies of the host offset arrays
+    int64_t n_reads, n_haps;
+};
+
+struct ShortTask {  // one lane group's work: several reads streamed against one haplotype
+    int hap, pair_first, n_pairs, rows;  // rows = sum of the read lengths (reset rows not counted)
+};
+
+struct ShortLaunch {
+    const float* table;        // 8 floats per entry; read r starts at entry read_off[r] + r
+    const ShortTask* tasks;    // ordered by warp
+    const int* warp_first;     // n_warps+1: first task of each warp
+    int n_warps;
+    const int* srt_read;       // read index of each sorted pair
+    const int* srt_out;        // caller's pair index of each sorted pair
+    double* out;
+    uint8_t* flags;
+    float rescue_thr;          // scaled sums below this (or non-finite) are queued for fp64
+    int* rescue_count;         // device counter
+    int* rescue_list;          // caller pair indices
+};
+
+struct ChainItem {  // one strip (32 lanes x 2NV columns) of one pair, run concurrently with its neighbours
+    int pair;        // caller's pair index
+    int strip;       // strip number, 0 = leftmost
+    int prog0;       // index of the pair's first progress counter (one per strip boundary)
+    int pad;
+    int64_t buf0;    // index (in boundary blocks) of the pair's first boundary buffer
+};
+
+struct ChainLaunch {
+    const ChainItem* items;    // device; or, with items_are_pairs, a plain int array of caller pair indices
+                               // (each such pair is run by one warp, its strips in sequence)
+    const int* n_items;        // device (may be produced by an earlier kernel)
+    int* ticket;               // device, zeroed before the launch
+    const int* pair_read;      // device copies of the caller's pair list
+    const int* pair_hap;
+    const double* lut;         // 256 entries 10^(-q/10)
+    void* boundary;            // concurrent strips: boundary buffers; sequential: 2 x scratch_blocks per warp of the grid
+    int64_t scratch_blocks;
+    int* progress;             // concurrent strips: rows published per boundary
+    double* out;
+    uint8_t* flags;
+    uint8_t flag_bits;         // written to flags[pair]
+    int log2C;                 // scale constant C = 2^log2C of Eq.1 (0 for the rescaled kernels)
+};
+
+cudaError_t launch_lut_table(const DevBatch& b, const double* lut, float* table, cudaStream_t st);
+cudaError_t launch_short_f32(const DevBatch& b, const ShortLaunch& p, cudaStream_t st);
+// rescue_from_list: items are taken from p.items[...] as plain pair indices in `rescue_list` form
+cudaError_t launch_chain(const DevBatch& b, const ChainLaunch& p, bool fp64, bool items_are_pairs, int grid_ctas,
+                         cudaStream_t st);
+int chain_ctas_per_sm(bool fp64);
+int chain_warps_per_cta();
+size_t chain_block_bytes(bool fp64);  // bytes of one 32-row boundary block
+int chain_strip_cols(bool fp64);      // haplotype columns covered by one strip
+
+}  // namespace phmm
