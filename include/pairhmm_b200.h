@@ -74,6 +74,10 @@ typedef struct phmm_options {
     /* upper bound, in bytes, for the per-read row-constant table built per launch group; batches
      * needing more are processed in several slices.  Default 8 GiB. */
     int64_t max_table_bytes;
+    /* non-zero: bracket every kernel family of a call with CUDA events on the caller's stream; the
+     * durations appear in phmm_stats.ms_* (phmm_get_stats synchronises the last event).  Default 0. */
+    int32_t profile_events;
+    int32_t reserved0;
 } phmm_options;
 
 /* One batch, CSR layout, natural order (a read, a haplotype and four
@@ -107,6 +111,11 @@ typedef struct phmm_stats {
     double host_batch_ms;       /* host time spent in the batcher */
     int32_t n_short_warps;      /* warp tasks of the short kernel */
     int32_t n_slices;
+    /* device time per kernel family, milliseconds, CUDA events on the caller's stream; filled only
+     * with phmm_options.profile_events (else 0).  ms_short is the sub-warp systolic fp32 kernel, ms_table
+     * the row-constant prologue, ms_rescue the fp64 (rescue / PHMM_FP64 short) chain launch, ms_long
+     * the concurrent-strip wavefront launch. */
+    double ms_table, ms_short, ms_rescue, ms_long;
 } phmm_stats;
 
 /* Create a context on CUDA device `device`.  opt may be NULL.  Fails with PHMM_E_UNSUPPORTED on a

@@ -28,7 +28,8 @@ EXPORTS = ["phmm_create", "phmm_destroy", "phmm_forward_batch", "phmm_forward_ba
 class phmm_options(ctypes.Structure):
     _fields_ = [("size", ctypes.c_uint32), ("rescue_log2_threshold", ctypes.c_int32),
                 ("long_min_hap_len", ctypes.c_int32), ("task_rows", ctypes.c_int32),
-                ("max_table_bytes", ctypes.c_int64)]
+                ("max_table_bytes", ctypes.c_int64), ("profile_events", ctypes.c_int32),
+                ("reserved0", ctypes.c_int32)]
 
 
 class phmm_batch(ctypes.Structure):
@@ -44,7 +45,9 @@ class phmm_stats(ctypes.Structure):
                 ("n_long_pairs", ctypes.c_int64), ("n_rescued", ctypes.c_int64), ("short_cells", ctypes.c_int64),
                 ("short_padded_cells", ctypes.c_int64), ("n_kernel_launches", ctypes.c_int64),
                 ("table_bytes", ctypes.c_int64), ("host_batch_ms", ctypes.c_double),
-                ("n_short_warps", ctypes.c_int32), ("n_slices", ctypes.c_int32)]
+                ("n_short_warps", ctypes.c_int32), ("n_slices", ctypes.c_int32),
+                ("ms_table", ctypes.c_double), ("ms_short", ctypes.c_double), ("ms_rescue", ctypes.c_double),
+                ("ms_long", ctypes.c_double)]
 
     def as_dict(self):
         return {k: getattr(self, k) for k, _ in self._fields_}
@@ -138,6 +141,38 @@ class DeviceBatch:
                           ptr(self.t[4]), ptr(self.t[5]), _hp(self.pair_read), _hp(self.pair_hap))
 
 
+class HostBatch:
+    """The phmm_batch layout with EVERY buffer in page-locked host memory (torch pinned tensors), plus
+    pinned result buffers: the argument of phmm_forward_batch_host, the end-to-end entry."""
+
+    def __init__(self, batch):
+        import torch
+        pin = lambda a, dt: torch.from_numpy(np.ascontiguousarray(a, dtype=dt)).pin_memory()
+        self.read_off = np.ascontiguousarray(batch.read_off, dtype=np.int64)
+        self.hap_off = np.ascontiguousarray(batch.hap_off, dtype=np.int64)
+        self.pair_read = np.ascontiguousarray(batch.pair_read, dtype=np.int32)
+        self.pair_hap = np.ascontiguousarray(batch.pair_hap, dtype=np.int32)
+        self.t = [pin(a, np.uint8) for a in (batch.read_bases, batch.qual_base, batch.qual_ins, batch.qual_del,
+                                             batch.qual_gcp, batch.hap_bases)]
+        n = len(self.pair_read)
+        self.out = torch.empty(n, dtype=torch.float64).pin_memory()
+        self.flags = torch.zeros(n, dtype=torch.uint8).pin_memory()
+
+    def h2d_bytes(self) -> int:
+        """payload bytes + offset arrays + pair lists copied host->device by one call"""
+        return (sum(int(t.numel()) for t in self.t) + self.read_off.nbytes + self.hap_off.nbytes +
+                self.pair_read.nbytes + self.pair_hap.nbytes)
+
+    def d2h_bytes(self) -> int:
+        return int(self.out.numel()) * 8 + int(self.flags.numel())
+
+    def c_struct(self) -> phmm_batch:
+        ptr = lambda t: t.data_ptr() if t.numel() else 0
+        return phmm_batch(len(self.read_off) - 1, len(self.hap_off) - 1, len(self.pair_read), _hp(self.read_off),
+                          _hp(self.hap_off), ptr(self.t[0]), ptr(self.t[1]), ptr(self.t[2]), ptr(self.t[3]),
+                          ptr(self.t[4]), ptr(self.t[5]), _hp(self.pair_read), _hp(self.pair_hap))
+
+
 class Context:
     """phmm_ctx wrapper."""
 
@@ -183,7 +218,16 @@ class Context:
         return out, flags
 
     def forward_batch_host(self, batch, precision: int = PHMM_FP32_RESCUE):
-        """phmm_forward_batch_host: everything on the host (numpy); copies are inside the call."""
+        """phmm_forward_batch_host: everything on the host; copies are inside the call.  ``batch`` is a
+        HostBatch (pinned buffers; returns its pinned result tensors as numpy views) or any
+        workloads.Batch-like object of numpy arrays (pageable)."""
+        if isinstance(batch, HostBatch):
+            cb = batch.c_struct()
+            rc = lib().phmm_forward_batch_host(self._h, ctypes.byref(cb), precision, batch.out.data_ptr(),
+                                               batch.flags.data_ptr())
+            if rc != PHMM_OK:
+                raise PhmmError(rc, lib().phmm_last_cuda_error(self._h))
+            return batch.out.numpy(), batch.flags.numpy()
         arrs = [np.ascontiguousarray(a, dtype=np.uint8) for a in (batch.read_bases, batch.qual_base, batch.qual_ins,
                                                                   batch.qual_del, batch.qual_gcp, batch.hap_bases)]
         ro = np.ascontiguousarray(batch.read_off, dtype=np.int64)

@@ -61,6 +61,8 @@ struct phmm_ctx {
     std::vector<uint8_t> is_short;
     ShortPlan plan;
     int chain_grid[2] = {0, 0};
+    cudaEvent_t ev_prof[8] = {};   // profile_events: [2f], [2f+1] bracket family f (0 table, 1 short, 2 rescue, 3 long)
+    bool prof_used[4] = {false, false, false, false};
 };
 
 #define CK(call)                                                    \
@@ -99,6 +101,9 @@ extern "C" int phmm_create(phmm_ctx** out, int device, const phmm_options* opt) 
     if (ctx->opt.long_min_hap_len <= 0 || ctx->opt.long_min_hap_len > SHORT_MAX_K) ctx->opt.long_min_hap_len = SHORT_MAX_K;
     if (ctx->opt.task_rows <= 0) ctx->opt.task_rows = 3072;
     if (ctx->opt.max_table_bytes <= 0) ctx->opt.max_table_bytes = (int64_t)64 << 30;
+    if (ctx->opt.profile_events)
+        for (int i = 0; i < 8; i++)
+            if (cudaEventCreate(&ctx->ev_prof[i]) != cudaSuccess) { delete ctx; return PHMM_E_CUDA; }
     memset(&ctx->stats, 0, sizeof(ctx->stats));
     if (cudaSetDevice(device) != cudaSuccess) { delete ctx; return PHMM_E_CUDA; }
     if (cudaEventCreateWithFlags(&ctx->ev_upload, cudaEventDisableTiming) != cudaSuccess) { delete ctx; return PHMM_E_CUDA; }
@@ -125,6 +130,8 @@ extern "C" int phmm_destroy(phmm_ctx* ctx) {
     for (DevBuf* b : bufs) b->release();
     ctx->h_stage.release();
     if (ctx->ev_upload) cudaEventDestroy(ctx->ev_upload);
+    for (int i = 0; i < 8; i++)
+        if (ctx->ev_prof[i]) cudaEventDestroy(ctx->ev_prof[i]);
     delete ctx;
     return PHMM_OK;
 }
@@ -136,6 +143,15 @@ extern "C" int phmm_get_stats(phmm_ctx* ctx, phmm_stats* out) {
         cudaSetDevice(ctx->device);
         if (cudaMemcpy(&n, ctx->d_counters.p, sizeof(int), cudaMemcpyDeviceToHost) == cudaSuccess && ctx->stats.n_short_warps > 0)
             ctx->stats.n_rescued = n;
+    }
+    if (ctx->opt.profile_events) {
+        double* dst[4] = {&ctx->stats.ms_table, &ctx->stats.ms_short, &ctx->stats.ms_rescue, &ctx->stats.ms_long};
+        for (int f = 0; f < 4; f++) {
+            float ms = 0.f;
+            if (ctx->prof_used[f] && cudaEventSynchronize(ctx->ev_prof[2 * f + 1]) == cudaSuccess &&
+                cudaEventElapsedTime(&ms, ctx->ev_prof[2 * f], ctx->ev_prof[2 * f + 1]) == cudaSuccess)
+                *dst[f] = ms;
+        }
     }
     *out = ctx->stats;
     return PHMM_OK;
@@ -163,6 +179,7 @@ struct Stager {  // packs several host arrays into the pinned buffer and copies 
 }  // namespace
 
 #define RC(call) do { int rc__ = (call); if (rc__ != PHMM_OK) return rc__; } while (0)
+#define PROF(f, second) do { if (ctx->opt.profile_events) { CK(cudaEventRecord(ctx->ev_prof[2 * (f) + (second)], st)); ctx->prof_used[f] = true; } } while (0)
 
 extern "C" int phmm_forward_batch(phmm_ctx* ctx, const phmm_batch* b, int precision, double* d_out, uint8_t* d_flags,
                                   void* cuda_stream) {
@@ -170,6 +187,7 @@ extern "C" int phmm_forward_batch(phmm_ctx* ctx, const phmm_batch* b, int precis
     if (precision != PHMM_FP32_RESCUE && precision != PHMM_FP64) return PHMM_E_ARG;
     if (b->n_pairs < 0 || b->n_reads < 0 || b->n_haps < 0) return PHMM_E_ARG;
     memset(&ctx->stats, 0, sizeof(ctx->stats));
+    for (int f = 0; f < 4; f++) ctx->prof_used[f] = false;
     if (b->n_pairs == 0) return PHMM_OK;
     if (!d_out || !b->d_read_bases || !b->d_qual_base || !b->d_qual_ins || !b->d_qual_del || !b->d_qual_gcp || !b->d_hap_bases)
         return PHMM_E_ARG;
@@ -270,7 +288,9 @@ extern "C" int phmm_forward_batch(phmm_ctx* ctx, const phmm_batch* b, int precis
         if ((int64_t)table_bytes > ctx->opt.max_table_bytes) return PHMM_E_NOMEM;
         CK(ctx->d_table.need(table_bytes));
         ctx->stats.table_bytes = (int64_t)table_bytes;
+        PROF(0, 0);
         CK(launch_lut_table(db, (const double*)ctx->d_lut.p, (float*)ctx->d_table.p, st));
+        PROF(0, 1);
         ShortLaunch sl;
         sl.table = (const float*)ctx->d_table.p;
         sl.tasks = (const ShortTask*)ctx->d_tasks.p;
@@ -283,7 +303,9 @@ extern "C" int phmm_forward_batch(phmm_ctx* ctx, const phmm_batch* b, int precis
         sl.rescue_thr = (float)ldexp(1.0, ctx->opt.rescue_log2_threshold);
         sl.rescue_count = counters + 0;
         sl.rescue_list = (int*)ctx->d_rescue.p;
+        PROF(1, 0);
         CK(launch_short_f32(db, sl, st));
+        PROF(1, 1);
         launches += 2;
     }
     // sequential chain launch: fp32 mode = rescue list (device-side count), fp64 mode = all non-long pairs
@@ -308,7 +330,9 @@ extern "C" int phmm_forward_batch(phmm_ctx* ctx, const phmm_batch* b, int precis
         cl.flags = d_flags;
         cl.flag_bits = fp64 ? 0 : PHMM_FLAG_RESCUED;
         cl.log2C = 0;
+        PROF(2, 0);
         CK(launch_chain(db, cl, true, true, grid, st));
+        PROF(2, 1);
         launches++;
     }
     // ---- long path: concurrent strips in the requested precision
@@ -331,7 +355,9 @@ extern "C" int phmm_forward_batch(phmm_ctx* ctx, const phmm_batch* b, int precis
         cl.flags = d_flags;
         cl.flag_bits = PHMM_FLAG_LONG;
         cl.log2C = 0;
+        PROF(3, 0);
         CK(launch_chain(db, cl, fp64, false, ctx->chain_grid[fp64 ? 1 : 0], st));
+        PROF(3, 1);
         launches++;
     }
     ctx->stats.n_kernel_launches = launches;

@@ -1,0 +1,267 @@
+"""Parity of the CUDA path (through the C ABI, include/pairhmm_b200.h) against the CPU oracle.
+
+Element by element on seeded inputs shaped like BASELINE.json configs[0..4] at sizes the oracle
+finishes in seconds, on sampled pairs at the full sizes bench.py times, plus the edge cases.
+Tolerances (BASELINE.json north_star): |dlog10 L| <= 1e-3 for PHMM_FP32_RESCUE (rescued pairs
+included), <= 1e-9 for PHMM_FP64; pair indexing and the rescue flag set exact (reading G16)."""
+import math
+
+import numpy as np
+import pytest
+
+import oracle
+from paper_2606_25738_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+TOL32, TOL64 = 1e-3, 1e-9
+LOG10_2 = math.log10(2.0)
+# G16: the fp32 pass runs with C = 2^120 and a pair is redone in fp64 iff its scaled sum < 2^-90
+RESCUE_LOG10 = (-90 - 120) * LOG10_2
+BORDER = 1e-3
+
+
+@pytest.fixture(scope="module")
+def B():
+    from paper_2606_25738_b200 import binding
+    return binding
+
+
+@pytest.fixture(scope="module")
+def ctx(B):
+    c = B.Context(0)
+    yield c
+    c.close()
+
+
+def run(B, ctx, batch, prec):
+    db = B.DeviceBatch(batch)
+    out, fl = ctx.forward_batch(db, prec)
+    return out.cpu().numpy(), fl.cpu().numpy()
+
+
+def check(B, ctx, batch, prec, ref=None, pairs=None):
+    out, fl = run(B, ctx, batch, prec)
+    assert np.all(np.isfinite(out)), "non-finite outputs at %s" % np.where(~np.isfinite(out))[0][:8]
+    if ref is None:
+        ref = oracle.forward_batch(batch, pairs=pairs)
+    got = out if pairs is None else out[pairs]
+    err = np.abs(got - ref)
+    tol = TOL32 if prec == B.PHMM_FP32_RESCUE else TOL64
+    bad = np.where(~(err <= tol))[0]
+    assert len(bad) == 0, "max err %g at %s (got %s want %s)" % (err.max(), bad[:5], got[bad[:5]], ref[bad[:5]])
+    return out, fl, ref
+
+
+def check_flags(B, batch, fl, ref, pairs=None):
+    """Rescue flags must equal the oracle's prediction except within +-1e-3 of the threshold (G16).
+    Only short-path pairs can be rescued; long-path pairs carry PHMM_FLAG_LONG instead."""
+    f = fl if pairs is None else fl[pairs]
+    is_long = (f & B.PHMM_FLAG_LONG) != 0
+    want = ref < RESCUE_LOG10
+    border = np.abs(ref - RESCUE_LOG10) <= BORDER
+    sel = ~is_long & ~border
+    got = (f & B.PHMM_FLAG_RESCUED) != 0
+    assert np.array_equal(got[sel], want[sel]), "rescue flag mismatch at %s" % np.where(got[sel] != want[sel])[0][:8]
+    assert not np.any(got & is_long)
+    return int(border.sum())
+
+
+# ------------------------------------------------------------------ configs at oracle-sized scale
+def test_config0_tiny_fp32_and_fp64(B, ctx):
+    b = W.generate(0)
+    assert b.n_pairs == 256
+    out, fl, ref = check(B, ctx, b, B.PHMM_FP32_RESCUE)
+    assert check_flags(B, b, fl, ref) == 0
+    # 3 of 4 haplotypes are unrelated to each read: most pairs must have needed the fp64 rescue
+    assert 150 <= int((fl & B.PHMM_FLAG_RESCUED).sum()) <= 200
+    out64, fl64, _ = check(B, ctx, b, B.PHMM_FP64, ref=ref)
+    assert not np.any(fl64 & B.PHMM_FLAG_RESCUED)
+
+
+def test_config1_short_regions(B, ctx):
+    b = W.generate(1, n=12)  # 12 regions x 1024 pairs; spans many warps / tasks and ragged lane groups
+    out, fl, ref = check(B, ctx, b, B.PHMM_FP32_RESCUE)
+    check_flags(B, b, fl, ref)
+    check(B, ctx, b, B.PHMM_FP64, ref=ref)
+
+
+def test_config2_mixed_stream(B, ctx):
+    b = W.generate(2, n=30000)  # unsorted pairs, 5% unrelated reads, haplotypes up to 1200 (short and long path)
+    out, fl, ref = check(B, ctx, b, B.PHMM_FP32_RESCUE)
+    nb = check_flags(B, b, fl, ref)
+    assert nb <= 3
+    n_resc = int((fl & B.PHMM_FLAG_RESCUED).sum())
+    assert 0.02 * b.n_pairs < n_resc < 0.25 * b.n_pairs  # >= the ~5% unrelated reads, plus reads overhanging their haplotype window
+    st = ctx.stats()
+    assert st["n_rescued"] == n_resc
+    b64 = b.select_pairs(np.arange(0, b.n_pairs, 5))
+    check(B, ctx, b64, B.PHMM_FP64, ref=ref[::5])
+
+
+def test_config3_long_reads_scaled(B, ctx):
+    b = W.generate(3, n=6, len_lo=1500, len_hi=2500)
+    out, fl, ref = check(B, ctx, b, B.PHMM_FP32_RESCUE)
+    assert np.all(fl & B.PHMM_FLAG_LONG)
+    check(B, ctx, b, B.PHMM_FP64, ref=ref)
+
+
+def test_config3_long_reads_full_length(B, ctx):
+    b = W.generate(3, n=4)  # 5-15 kbp reads: thousands of bits of dynamic range, rescaling mandatory
+    out, fl, ref = check(B, ctx, b, B.PHMM_FP32_RESCUE)
+    assert ref.min() < -1000
+    check(B, ctx, b, B.PHMM_FP64, ref=ref)
+
+
+def test_config4_very_long_scaled(B, ctx):
+    b = W.generate(4, n=2, len_lo=24000, len_hi=24000)  # same error model, 24 kbp x 25.2 kbp: ~25 strips per pair
+    out, fl, ref = check(B, ctx, b, B.PHMM_FP32_RESCUE)
+    assert np.all(fl & B.PHMM_FLAG_LONG)
+    check(B, ctx, b, B.PHMM_FP64, ref=ref)
+
+
+# ------------------------------------------------------------------ full sizes, sampled
+def test_config1_full_size_sampled(B, ctx):
+    """The batch and launch configuration bench.py times (2.05 M pairs); oracle on 1500 sampled pairs."""
+    b = W.generate(1)
+    assert b.n_pairs == 2000 * 128 * 8
+    rng = np.random.default_rng(5)
+    pairs = np.sort(rng.choice(b.n_pairs, 1500, replace=False))
+    out, fl, ref = check(B, ctx, b, B.PHMM_FP32_RESCUE, pairs=pairs)
+    check_flags(B, b, fl, ref, pairs=pairs)
+    assert np.all(out <= 0.5)  # L stays below a small constant
+
+
+def test_config3_full_size_sampled(B, ctx):
+    b = W.generate(3)
+    rng = np.random.default_rng(6)
+    pairs = np.sort(rng.choice(b.n_pairs, 3, replace=False))
+    check(B, ctx, b, B.PHMM_FP32_RESCUE, pairs=pairs)
+
+
+def test_config4_full_size_properties(B, ctx):
+    """16 pairs of 100 kbp x 105 kbp.  One pair costs the oracle minutes, so: fp32 and fp64 GPU paths
+    (different kernels instantiations, different rescaling ranges) must agree to 1e-3, results are finite,
+    about -0.8 bits per row, and one pair is checked against the oracle."""
+    b = W.generate(4)
+    o32, f32 = run(B, ctx, b, B.PHMM_FP32_RESCUE)
+    o64, f64 = run(B, ctx, b, B.PHMM_FP64)
+    assert np.all(np.isfinite(o32)) and np.all(np.isfinite(o64))
+    assert np.max(np.abs(o32 - o64)) <= TOL32
+    assert np.all((o64 < -15000) & (o64 > -40000))
+    ref = oracle.forward_batch(b, pairs=np.array([7]))
+    assert abs(o64[7] - ref[0]) <= TOL64 * 10  # 1e5 rows of fp64 rounding: allow 1e-8
+    assert abs(o32[7] - ref[0]) <= TOL32
+
+
+# ------------------------------------------------------------------ indexing / batching invariants
+def test_pair_order_and_duplicates_bitwise(B, ctx):
+    b = W.generate(2, n=6000)
+    out, fl = run(B, ctx, b, B.PHMM_FP32_RESCUE)
+    rng = np.random.default_rng(9)
+    perm = rng.permutation(b.n_pairs)
+    out_p, fl_p = run(B, ctx, b.select_pairs(perm), B.PHMM_FP32_RESCUE)
+    assert np.array_equal(out_p, out[perm]) and np.array_equal(fl_p, fl[perm])
+    dup = np.concatenate([np.arange(100), np.arange(100), np.arange(50)])
+    out_d, _ = run(B, ctx, b.select_pairs(dup), B.PHMM_FP32_RESCUE)
+    assert np.array_equal(out_d, out[dup])
+
+
+def test_host_entry_matches_device_entry(B, ctx):
+    b = W.generate(1, n=3)
+    out, fl = run(B, ctx, b, B.PHMM_FP32_RESCUE)
+    oh, fh = ctx.forward_batch_host(b, B.PHMM_FP32_RESCUE)
+    assert np.array_equal(oh, out) and np.array_equal(fh, fl)
+    hb = B.HostBatch(b)
+    oh2, fh2 = ctx.forward_batch_host(hb, B.PHMM_FP32_RESCUE)
+    assert np.array_equal(oh2, out) and np.array_equal(fh2, fl)
+    assert hb.h2d_bytes() > 5 * len(b.read_bases) and hb.d2h_bytes() == 9 * b.n_pairs
+
+
+# ------------------------------------------------------------------ edge cases
+def _rand_seq(rng, n):
+    return "".join(rng.choice(list("ACGT"), n))
+
+
+def test_edge_lengths(B, ctx):
+    """1-base reads / haplotypes, haplotype lengths at and around every tile boundary (32 columns per
+    lane, 1024 per warp = short/long cut, 1024-column strips), reads longer than haplotypes."""
+    rng = np.random.default_rng(21)
+    pairs = []
+    for k in (1, 2, 31, 32, 33, 63, 64, 65, 255, 256, 257, 1023, 1024, 1025, 2047, 2048, 2049, 3100):
+        for l in (1, 2, 17, 130):
+            hap = _rand_seq(rng, k)
+            if l <= k and rng.random() < 0.7:
+                s = int(rng.integers(0, k - l + 1))
+                read = hap[s:s + l]
+            else:
+                read = _rand_seq(rng, l)
+            pairs.append((read, hap, list(rng.integers(5, 41, l)), list(rng.integers(10, 50, l)),
+                          list(rng.integers(10, 50, l)), 10))
+    b = W.from_strings(pairs)
+    check(B, ctx, b, B.PHMM_FP32_RESCUE)
+    check(B, ctx, b, B.PHMM_FP64)
+
+
+def test_read_longer_than_haplotype_and_unrelated(B, ctx):
+    rng = np.random.default_rng(22)
+    pairs = [(_rand_seq(rng, 300), _rand_seq(rng, 40)), (_rand_seq(rng, 250), _rand_seq(rng, 600)),
+             (_rand_seq(rng, 36), _rand_seq(rng, 60)), (_rand_seq(rng, 1), _rand_seq(rng, 1200))]
+    b = W.from_strings(pairs, qb=25, qi=40, qd=40)
+    out, fl, ref = check(B, ctx, b, B.PHMM_FP32_RESCUE)
+    check_flags(B, b, fl, ref)
+    assert fl[0] & B.PHMM_FLAG_RESCUED and fl[1] & B.PHMM_FLAG_RESCUED and not (fl[2] & B.PHMM_FLAG_RESCUED)
+
+
+def test_n_bases_match_nothing_else(B, ctx):
+    """Reading G17: byte equality on A/C/G/T; any other byte matches nothing in the other sequence."""
+    b = W.from_strings([("ACGNTACG", "ACGTTACGGA"), ("ACGTTACG", "ACGNTACGGA"), ("ACGTTACG", "ACGTTACGGA")])
+    out, _ = run(B, ctx, b, B.PHMM_FP64)
+    # oracle with the N replaced by a base that matches nothing at that position pattern is not expressible
+    # with literal byte equality (N==N), so compare to the oracle on inputs where N cannot meet N
+    ref = oracle.forward_batch(b)
+    assert np.max(np.abs(out - ref)) <= TOL64
+    assert out[0] < out[2] and out[1] < out[2]
+
+
+def test_constant_quals_long_read_fp32_error(B, ctx):
+    """SURVEY hard part 4: constant qualities make the fp32 rounding of the row constants systematic;
+    the worst case for the 1e-3 bound.  8 kbp read with constant quals."""
+    rng = np.random.default_rng(23)
+    hap = _rand_seq(rng, 8400)
+    read = list(hap[100:8100])
+    for i in rng.choice(8000, 200, replace=False):
+        read[i] = "ACGT"[("ACGT".index(read[i]) + 1) % 4]
+    b = W.from_strings([("".join(read), hap)], qb=30, qi=40, qd=40)
+    check(B, ctx, b, B.PHMM_FP32_RESCUE)
+    check(B, ctx, b, B.PHMM_FP64)
+
+
+def test_empty_batch_and_errors(B, ctx):
+    import torch
+    b = W.generate(0)
+    e = b.select_pairs(np.zeros(0, dtype=np.int64))
+    out, fl = ctx.forward_batch(B.DeviceBatch(e), B.PHMM_FP32_RESCUE)
+    assert out.numel() == 0
+    assert ctx.stats()["n_pairs"] == 0
+    # pair index out of range -> PHMM_E_OFFSETS, output untouched
+    db = B.DeviceBatch(b)
+    bad = db.with_pairs(np.array([0, b.n_reads], dtype=np.int32), np.array([0, 0], dtype=np.int32))
+    sentinel = torch.full((2,), 7.0, dtype=torch.float64, device="cuda:0")
+    with pytest.raises(B.PhmmError) as ei:
+        ctx.forward_batch(bad, B.PHMM_FP32_RESCUE, out=sentinel)
+    assert ei.value.code == B.PHMM_E_OFFSETS
+    assert torch.all(sentinel == 7.0)
+    # empty read -> PHMM_E_EMPTY
+    z = W.from_strings([("ACGT", "ACGTAA"), ("", "ACGT")])
+    with pytest.raises(B.PhmmError) as ei:
+        ctx.forward_batch(B.DeviceBatch(z), B.PHMM_FP64)
+    assert ei.value.code == B.PHMM_E_EMPTY
+    with pytest.raises(B.PhmmError) as ei:
+        ctx.forward_batch(db, 5)
+    assert ei.value.code == B.PHMM_E_ARG
+
+
+def test_measured_peaks_are_sane(B):
+    f32, f32x2, f64 = B.measure_peak(0), B.measure_peak(1), B.measure_peak(2)
+    assert 40 < f32 < 90 and 40 < f32x2 < 90 and 20 < f64 < 45
