@@ -13,7 +13,7 @@ import subprocess
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "libpairhmm_b200.so")
+LIB_PATH = os.environ.get("PHMM_LIB", os.path.join(_HERE, "libpairhmm_b200.so"))  # PHMM_LIB: try another build of the same ABI
 
 PHMM_OK = 0
 PHMM_E_ARG, PHMM_E_OFFSETS, PHMM_E_EMPTY, PHMM_E_TOOLONG = -1, -2, -3, -4

@@ -246,7 +246,7 @@ extern "C" int phmm_forward_batch(phmm_ctx* ctx, const phmm_batch* b, int precis
     if (ctx->upload_pending) { CK(cudaEventSynchronize(ctx->ev_upload)); ctx->upload_pending = false; }
     const size_t n_seq = fp64 ? seq_pairs.size() : 0;
     size_t stage_bytes = 4096 + (size_t)(b->n_reads + 1) * 8 + (size_t)(b->n_haps + 1) * 8 + (size_t)np * 8 +
-                         pl.tasks.size() * sizeof(ShortTask) + pl.warp_first.size() * 4 + pl.srt_read.size() * 8 +
+                         pl.tasks.size() * sizeof(ShortTask) + pl.warp_first.size() * 4 + pl.srt_read.size() * 16 +
                          items.size() * sizeof(ChainItem) + n_seq * 4 + 16 * 256;
     CK(ctx->h_stage.need(stage_bytes));
     Stager sg{ctx, st};
@@ -256,7 +256,7 @@ extern "C" int phmm_forward_batch(phmm_ctx* ctx, const phmm_batch* b, int precis
     RC(sg.upload(ctx->d_pair_hap, b->h_pair_hap, (size_t)np * 4));
     RC(sg.upload(ctx->d_tasks, pl.tasks.data(), pl.tasks.size() * sizeof(ShortTask)));
     RC(sg.upload(ctx->d_warp_first, pl.warp_first.data(), pl.warp_first.size() * 4));
-    RC(sg.upload(ctx->d_srt_read, pl.srt_read.data(), pl.srt_read.size() * 4));
+    RC(sg.upload(ctx->d_srt_read, pl.srt_ent.data(), pl.srt_ent.size() * 4));
     RC(sg.upload(ctx->d_srt_out, pl.srt_out.data(), pl.srt_out.size() * 4));
     RC(sg.upload(ctx->d_items, items.data(), items.size() * sizeof(ChainItem)));
     // counters: [0] rescue count (= n_items of the rescue launch)  [1] ticket rescue  [2] n strip items  [3] ticket strips
@@ -284,7 +284,9 @@ extern "C" int phmm_forward_batch(phmm_ctx* ctx, const phmm_batch* b, int precis
 
     // ---- short path: row-constant table, systolic kernel, then fp64 rescue of what underflowed
     if (n_warps > 0) {
-        const size_t table_bytes = (size_t)(b->h_read_off[b->n_reads] + b->n_reads + 1) * 32;
+        const int64_t n_entries = TABLE_ZERO_RUN + b->h_read_off[b->n_reads] + (int64_t)TABLE_EXTRA_ROWS * b->n_reads;
+        if (n_entries > INT32_MAX) return PHMM_E_TOOLONG;
+        const size_t table_bytes = (size_t)(n_entries + 64) * 64;
         if ((int64_t)table_bytes > ctx->opt.max_table_bytes) return PHMM_E_NOMEM;
         CK(ctx->d_table.need(table_bytes));
         ctx->stats.table_bytes = (int64_t)table_bytes;
@@ -296,7 +298,7 @@ extern "C" int phmm_forward_batch(phmm_ctx* ctx, const phmm_batch* b, int precis
         sl.tasks = (const ShortTask*)ctx->d_tasks.p;
         sl.warp_first = (const int*)ctx->d_warp_first.p;
         sl.n_warps = n_warps;
-        sl.srt_read = (const int*)ctx->d_srt_read.p;
+        sl.srt_ent = (const int2*)ctx->d_srt_read.p;
         sl.srt_out = (const int*)ctx->d_srt_out.p;
         sl.out = d_out;
         sl.flags = d_flags;

@@ -34,7 +34,7 @@ int validate_batch(const HostBatchView& b) {
 }
 
 void plan_short(const HostBatchView& b, const uint8_t* is_short, int N2, int task_rows, ShortPlan* out) {
-    out->tasks.clear(); out->warp_first.clear(); out->srt_read.clear(); out->srt_out.clear();
+    out->tasks.clear(); out->warp_first.clear(); out->srt_read.clear(); out->srt_out.clear(); out->srt_ent.clear();
     out->cells = 0; out->padded_cells = 0; out->max_read_len = 0;
     const int64_t np = b.n_pairs;
     // ---- 1. stable counting sort of the selected pairs by haplotype
@@ -46,13 +46,17 @@ void plan_short(const HostBatchView& b, const uint8_t* is_short, int N2, int tas
     for (int64_t h = 0; h < b.n_haps; h++) cnt[h + 1] += cnt[h];
     out->srt_read.resize((size_t)n_sel);
     out->srt_out.resize((size_t)n_sel);
+    out->srt_ent.resize((size_t)n_sel * 2);
     {
         std::vector<int> pos(cnt.begin(), cnt.end() - 1);
         for (int64_t p = 0; p < np; p++)
             if (is_short[p]) {
                 const int q = pos[b.pair_hap[p]]++;
-                out->srt_read[q] = b.pair_read[p];
+                const int r = b.pair_read[p];
+                out->srt_read[q] = r;
                 out->srt_out[q] = (int)p;
+                out->srt_ent[2 * (size_t)q] = (int)(TABLE_ZERO_RUN + b.read_off[r] + (int64_t)TABLE_EXTRA_ROWS * r);
+                out->srt_ent[2 * (size_t)q + 1] = (int)(b.read_off[r + 1] - b.read_off[r]) + TABLE_EXTRA_ROWS;
             }
     }
     // ---- 2. cut each haplotype's run of reads into tasks of about task_rows read rows
@@ -80,7 +84,7 @@ void plan_short(const HostBatchView& b, const uint8_t* is_short, int N2, int tas
     // ---- 3. pack tasks into warps: duration classes (longest first), lanes bin-packed largest-fit
     const int NCLS = 8 * 40;  // class = floor(8 * log2(duration)), duration < 2^40
     auto cls_of = [&](const ShortTask& t) {
-        const double d = (double)(t.rows + t.n_pairs);
+        const double d = (double)(t.rows + TABLE_EXTRA_ROWS * t.n_pairs);
         int c = (int)floor(8.0 * log2(d < 1 ? 1 : d));
         return c < 0 ? 0 : (c >= NCLS ? NCLS - 1 : c);
     };
@@ -129,7 +133,7 @@ void plan_short(const HostBatchView& b, const uint8_t* is_short, int N2, int tas
             const ShortTask& t = tasks[ids[avail[c * 33 + g]++]];
             out->tasks.push_back(t);
             cap -= g;
-            bin_steps = std::max(bin_steps, t.rows + t.n_pairs + 2 * g - 1);
+            bin_steps = std::max(bin_steps, t.rows + TABLE_EXTRA_ROWS * t.n_pairs + 2 * g - 1);
             if (cap == 0) close_bin();
         }
     }

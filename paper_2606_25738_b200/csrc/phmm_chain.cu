@@ -10,7 +10,7 @@
 // :319-324, become a skewed wavefront with 32-row handoff blocks), a8 (rescaling), a9, a10 (fp64 rescue).
 // Block-floating arithmetic: every thread keeps one integer exponent for all it holds; values
 // crossing a thread boundary are converted exactly by a power of two.
-#include "phmm_engine.cuh"
+#include "phmm_engine_v0.cuh"
 #include "phmm_kernels.h"
 
 namespace phmm {
@@ -35,7 +35,7 @@ __device__ __forceinline__ void st_release(int* p, int v) {
 template <typename T, int NV>
 __global__ void __launch_bounds__(CHAIN_WARPS * 32, (sizeof(T) == 4 ? 2 : 2))
 k_chain(DevBatch b, ChainLaunch p, int items_are_pairs) {
-    typedef Lane<T, NV, true> L;
+    typedef LaneV0<T, NV, true> L;
     constexpr int N2 = 2 * NV;
     __shared__ T ring[CHAIN_WARPS][8][RING];        // row constants, SoA: [field][slot]
     __shared__ Rec<T> rin[CHAIN_WARPS], rout[CHAIN_WARPS];
@@ -127,7 +127,7 @@ k_chain(DevBatch b, ChainLaunch p, int items_are_pairs) {
                 }
                 // ---- this lane's row constants
                 const int pos = s - 2 * lane;
-                RowConst<T> E;
+                RowConstV0<T> E;
                 E.a = E.pm = E.px = E.c = E.gi = E.gI = E.gm = (T)0;
                 E.meta = 0;
                 if (pos >= 0 && pos <= l) {

@@ -7,9 +7,12 @@
 //     M_{i,j}  = p_{i,j} * ( a_i M_{i-1,j-1} + I'_{i-1,j-1} + c_i S_{i-1,j-2} )
 // with  a_i = 1-iota_i-d_i,  c_i = g_i d_{i-1} (d_0 := 1),  gi_i = g_{i+1} iota_i,  gI_i = gamma_i g_{i+1}/g_i,
 //       g_i = 1-gamma_i,  g_{l+1} := 1  (so that I' = I on the last row, where Eq.4 sums M+I).
-// 6 FP instructions per cell (4 FMA + 2 MUL = 10 flops), one select for p_{i,j} (Eq.3).
-// Row 0 is produced by a "reset row" (pm = px = 0, gamma = 1, incoming S = C/k), which leaves
-// M = I' = 0 and S = C/k in every column: exactly Eq.1 under reading G1 (D_{0,j} = C/k, j = 0..k).
+// The kernels keep U_i := gi_{i+1} M_i instead of M_i (gi_{l+1} := 1), which turns gi_i M_{i-1} into a plain
+// operand: 5 FP instructions per cell (4 FMA + 1 MUL = 9 flops) and one select for p_{i,j} (Eq.3); see
+// phmm_engine.cuh.  Row 0 (Eq.1 under reading G1: D_{0,j} = C/k for j = 0..k, M = I = 0) is realised as
+// S_0 == C/k with gamma_0 := 1 and d_0 := 1: the first lane injects s = C/k on row 1 and the running sum
+// carries it unchanged through every column.  When several reads stream through one lane group, a
+// "reset row" (all constants 0) in front of each read zeroes the U and I' left by the previous read.
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -17,9 +20,9 @@
 namespace phmm {
 
 // ---- row-constant table entry: 8 scalars of type T per (read row), entry 0 of a read = reset row
-// slot: 0 a | 1 pm | 2 px | 3 c | 4 gi | 5 gI | 6 gamma | 7 meta (bit pattern, low 32 bits)
-// reset row: a = g_1 (harmless: multiplies into p = 0), everything else 0 except gamma = 1.
-enum : uint32_t { META_CODE_MASK = 7u, META_RESET = 8u, META_LAST = 16u };
+// slot: 0 a_i/gi_i (row 1: 0) | 1 pm_i gi_{i+1} | 2 px_i gi_{i+1} | 3 c_i/gi_i (row 1: c_1) | 4 gI_i | 5 gamma_{i-1} | 6 - | 7 meta (bits)
+// meta: bits 0-1 read base code (A,C,G,T; other bytes: pm := px, "matches nothing"), RESET, LAST, FIRST.
+enum : uint32_t { META_CODE_MASK = 3u, META_RESET = 8u, META_LAST = 16u, META_FIRST = 32u };
 
 #define PHMM_FULL 0xffffffffu
 

@@ -1,202 +1,150 @@
-// The per-lane engine of the skewed systolic wavefront.
+// The per-lane engine of the skewed systolic wavefront ("T/J form").
 //
-// One CUDA thread = two "virtual lanes" packed in the two halves of 64-bit register pairs (FFMA2 on
-// sm_100a): half .x owns NV consecutive haplotype columns, half .y the next NV columns and runs ONE
-// read row behind .x; the next CUDA lane's .x runs one further row behind, and so on.  With that
-// skew the left neighbour's last-column values (M, I', S) of a row are exact when they are needed,
-// so no scan is required (the paper's lock-step kernels need the weighted warp scan of Alg.1,
-// PAPER.md:221-231, plus a second running sum V, Listing 2 :309).  See phmm_common.cuh for the
-// recurrence; DESIGN.md "Kernel design" for the derivation.
+// One CUDA thread = two "virtual lanes" held in the two halves of float2 values (FFMA2/FMUL2 on
+// sm_100a; two scalars per operation in fp64): half .x owns NV consecutive haplotype columns, half .y
+// the next NV columns and runs ONE stream entry (read row) behind .x; the next CUDA lane's .x runs
+// one further entry behind, and so on.  With that skew everything a virtual lane needs from its left
+// neighbour is already final when it is needed, so no scan is required (the paper's lock-step kernels
+// need the weighted warp scan of Alg.1, plus a second running sum V, Listing 2
+// :309 = 7 FP instructions per cell; this engine needs 5).
+//
+// Recurrence (phmm_common.cuh: M, I' = g_{i+1} I, S = weighted inclusive prefix of M, Eq.6-7 with
+// every constant folded per read row).  State a virtual lane keeps for its columns x between two
+// steps, when the next entry it will process is read row i:
+//     T[x] = a_i M_{i-1,x-1} + I'_{i-1,x-1} + c_i S_{i-1,x-2}     everything of M_{i,x} but the prior
+//     J[x] = I'_{i,x}                                              (already advanced to row i)
+// One step = one row for all NV columns; per column, with U := gi_{i+1} M_{i,x} kept instead of M:
+//     U      = P_{i,x} * T[x]                    P = (pm_i | px_i) * gi_{i+1}, one select (Eq.3)   MUL
+//     W      = A * U + J[x]                      A = a_{i+1} / gi_{i+1}                            FMA
+//     T[x+1] = C * s + W                         C = c_{i+1} / gi_{i+1};  s = gi_{i+1} S_{i,x-1}   FMA
+//     J[x]   = G * J[x] + U                      G = gamma_{i+1} g_{i+2} / g_{i+1}                 FMA
+//     s      = gamma_i * s + U                   the row's running sum, the only serial chain       FMA
+// = 5 FP instructions per cell (4 FMA + 1 MUL, 9 flops); U, W are temporaries, T and J are updated in
+// place.  What crosses a virtual-lane boundary: the T[NV] that drops out on the right (consumed by
+// the neighbour two steps later = when it processes the next row) and the final s (consumed by the
+// neighbour's next step = the same row).  See the row-constant table kernel for the stream of
+// entries (run-in entry, rows 1..l, flush entry) and how Eq.1 and Eq.4 are realised.
 #pragma once
 #include "phmm_common.cuh"
 
 namespace phmm {
 
-template <typename T> struct RowConst {  // one table entry, as loaded for the .x half
-    T a, pm, px, c, gi, gI, gm;
-    uint32_t meta;
+// ---- two-wide arithmetic: float2 -> FFMA2/FMUL2/FADD2 (sm_100a), double2 -> two scalar ops
+template <typename T> struct W2;
+template <> struct W2<float> {
+    typedef float2 V;
+    static __device__ __forceinline__ V mk(float x, float y) { return make_float2(x, y); }
+    static __device__ __forceinline__ V fma(V a, V b, V c) { return __ffma2_rn(a, b, c); }
+    static __device__ __forceinline__ V mul(V a, V b) { return __fmul2_rn(a, b); }
+    static __device__ __forceinline__ V add(V a, V b) { return __fadd2_rn(a, b); }
+};
+template <> struct W2<double> {
+    typedef double2 V;
+    static __device__ __forceinline__ V mk(double x, double y) { return make_double2(x, y); }
+    static __device__ __forceinline__ V fma(V a, V b, V c) { return make_double2(::fma(a.x, b.x, c.x), ::fma(a.y, b.y, c.y)); }
+    static __device__ __forceinline__ V mul(V a, V b) { return make_double2(a.x * b.x, a.y * b.y); }
+    static __device__ __forceinline__ V add(V a, V b) { return make_double2(a.x + b.x, a.y + b.y); }
 };
 
-template <typename T, int NV, bool RESCALE> struct Lane {
-    typedef Pk<T> P;
-    typedef typename P::V V;
-
-    V M[NV], I[NV], S[NV];               // state of the rows last completed by (.x, .y); S[x] = prefix EXCLUSIVE of column x
-    V cA, cPm, cPx, cC, cGi, cGI, cGm;   // row constants (.x: its current row, .y: .x's previous row)
-    V inM, inI, inS;                     // left-boundary values of the rows processed in the last step
-    V sig;                               // running final sums handed to the right
+// One table entry as the kernel sees it: constants of the entry the .x half processes (lo) and of the
+// stream's previous entry, which the .y half processes in the same step (hi).
+template <typename T> struct Entry2 {
+    typename W2<T>::V gam, A, C, G;
+    T pmx, pxx, pmy, pxy;
     uint32_t metaX, metaY;
-    uint32_t mx[5], my[5];               // match bitmasks per base code for the NV columns of .x / .y
-    int nvx, nvy;                        // number of real (j <= k) columns in each half
-    int ex;                              // RESCALE: stored value * 2^ex = true value (one exponent per thread)
+};
+
+template <typename T, int NV> struct Lane2 {
+    typedef W2<T> P;
+    typedef typename P::V V;
+    static constexpr int NW = (NV + 7) / 8;  // 32-bit words of one-hot nibbles per half (8 columns per word)
+
+    V Tt[NV], J[NV];
+    V outT, outS;              // what dropped out on the right in the last step: (.x's, .y's)
+    T sigX, sigY;              // Eq.4 partial sums (columns <= this half's last) of the read finished last
+    uint32_t hx[NW], hy[NW];   // haplotype columns as one-hot nibbles: bit 4*(x%8)+b of word x/8 <=> column x has base b
+    int nvx, nvy;              // number of real (j <= k) columns in each half
 
     __device__ __forceinline__ void init() {
 #pragma unroll
-        for (int x = 0; x < NV; x++) { M[x] = P::zero(); I[x] = P::zero(); S[x] = P::zero(); }
-        cA = cPm = cPx = cC = cGi = cGI = cGm = P::zero();
-        inM = inI = inS = P::zero();
-        sig = P::zero();
-        metaX = metaY = 0;
-        ex = EX_ZERO;
+        for (int x = 0; x < NV; x++) { Tt[x] = P::mk((T)0, (T)0); J[x] = P::mk((T)0, (T)0); }
+        outT = outS = P::mk((T)0, (T)0);
+        sigX = sigY = (T)0;
     }
 
     // hap: pointer to the haplotype bytes, k its length, j0 = 0-based first column of this thread
     __device__ __forceinline__ void load_hap(const uint8_t* __restrict__ hap, int k, int j0) {
 #pragma unroll
-        for (int b = 0; b < 5; b++) { mx[b] = 0; my[b] = 0; }
+        for (int w = 0; w < NW; w++) { hx[w] = 0; hy[w] = 0; }
         nvx = min(max(k - j0, 0), NV);
         nvy = min(max(k - j0 - NV, 0), NV);
 #pragma unroll
         for (int x = 0; x < NV; x++) {
             if (x < nvx) {
-                int c = base_code(hap[j0 + x]);
-#pragma unroll
-                for (int b = 0; b < 5; b++) mx[b] |= (c == b ? 1u : 0u) << x;
+                const int c = base_code(hap[j0 + x]);
+                if (c < 4) hx[x >> 3] |= 1u << (4 * (x & 7) + c);
             }
             if (x < nvy) {
-                int c = base_code(hap[j0 + NV + x]);
-#pragma unroll
-                for (int b = 0; b < 5; b++) my[b] |= (c == b ? 1u : 0u) << x;
+                const int c = base_code(hap[j0 + NV + x]);
+                if (c < 4) hy[x >> 3] |= 1u << (4 * (x & 7) + c);
             }
         }
     }
 
-    static __device__ __forceinline__ uint32_t selmask(const uint32_t* m, uint32_t code) {
-        uint32_t r = (code & 1u) ? m[1] : m[0];
-        uint32_t q = (code & 1u) ? m[3] : m[2];
-        r = (code & 2u) ? q : r;
-        return (code & 4u) ? m[4] : r;
-    }
-
-    // multiply everything this thread holds by 2^-shift, adjust the exponent (exact unless it flushes)
-    __device__ __forceinline__ void rescale(int shift) {
-        int s = max(-Fx<T>::CLAMP, min(Fx<T>::CLAMP, shift));
-        int h = (-s) / 2;
-        T f1 = Fx<T>::exp2i(h), f2 = Fx<T>::exp2i(-s - h);
-        V F1 = P::pack(f1, f1), F2 = P::pack(f2, f2);
+    // One systolic step.  (inS, inT, inSig): the left neighbour thread's (.y) outS, outT, sigY as they stand
+    // after ITS last step, or the column-0 boundary for the first lane of a group (Eq.1 under reading G1:
+    // the run-in entry injects s = C/k and T = g_1 C/k, every other entry 0).
+    __device__ __forceinline__ void step(const Entry2<T>& E, T inS, T inT, T inSig) {
+        V s = P::mk(inS, outS.x);                  // .y continues the row .x finished one step ago
+        const V tgrab = P::mk(inT, outT.x);        // T[0] of the NEXT step
+        uint32_t rx[NW], ry[NW];
+        const uint32_t shx = E.metaX & META_CODE_MASK, shy = E.metaY & META_CODE_MASK;
+#pragma unroll
+        for (int w = 0; w < NW; w++) { rx[w] = hx[w] >> shx; ry[w] = hy[w] >> shy; }
+        auto prior = [&](int x) {                  // Eq.3: one select per half
+            const uint32_t bit = 1u << (4 * (x & 7));
+            return P::mk((rx[x >> 3] & bit) ? E.pmx : E.pxx, (ry[x >> 3] & bit) ? E.pmy : E.pxy);
+        };
+        V U = P::mul(prior(0), Tt[0]);
+        Tt[0] = tgrab;
 #pragma unroll
         for (int x = 0; x < NV; x++) {
-            M[x] = P::mul(P::mul(M[x], F1), F2);
-            I[x] = P::mul(P::mul(I[x], F1), F2);
-            S[x] = P::mul(P::mul(S[x], F1), F2);
+            V Un = U;
+            if (x + 1 < NV) Un = P::mul(prior(x + 1), Tt[x + 1]);
+            const V Wv = P::fma(E.A, U, J[x]);
+            const V Tn = P::fma(E.C, s, Wv);
+            J[x] = P::fma(E.G, J[x], U);
+            s = P::fma(E.gam, s, U);
+            if (x + 1 < NV) Tt[x + 1] = Tn; else outT = Tn;
+            U = Un;
         }
-        inM = P::mul(P::mul(inM, F1), F2);
-        inI = P::mul(P::mul(inI, F1), F2);
-        inS = P::mul(P::mul(inS, F1), F2);
-        sig = P::mul(P::mul(sig, F1), F2);
-        ex += shift;
-    }
-
-    // RESCALE: bring the values (lM, lI, lS, lSig), given at exponent exL, to this thread's exponent;
-    // if they would be too large for it, first move this thread's exponent up (its own state can only
-    // be negligible then, or still representable).
-    __device__ __forceinline__ void absorb(T& lM, T& lI, T& lS, T& lSig, int exL) {
-        T m = Fx<T>::fmax_(Fx<T>::fmax_(lM, lI), Fx<T>::fmax_(lS, lSig));
-        if (m > (T)0) {
-            if (ex == EX_ZERO) ex = exL + Fx<T>::ilogb(m) - Fx<T>::TGT;
-            int d = exL - ex;
-            int e_in = Fx<T>::ilogb(m) + d;
-            if (e_in > Fx<T>::HI) { rescale(e_in - Fx<T>::TGT); d = exL - ex; }
-            d = max(-Fx<T>::CLAMP, min(Fx<T>::CLAMP, d));
-            int h = d / 2;
-            T f1 = Fx<T>::exp2i(h), f2 = Fx<T>::exp2i(d - h);
-            lM = lM * f1 * f2; lI = lI * f1 * f2; lS = lS * f1 * f2; lSig = lSig * f1 * f2;
-        }
-    }
-
-    // RESCALE: every few rows renormalise this thread's state so that its maximum sits near 2^TGT
-    __device__ __forceinline__ void periodic() {
-        V mv = P::zero();
-        T m = (T)0;
+        outS = s;
+        // Eq.4: on the last row G = 1 and gi_{l+1} := 1, so J now holds M_l + I_l; sum this half's real columns
+        if ((E.metaX | E.metaY) & META_LAST) {
+            if (E.metaX & META_LAST) {
+                T a = (T)0;
+                if (nvx == NV) {
 #pragma unroll
-        for (int x = 0; x < NV; x++) {
-            m = Fx<T>::fmax_(m, Fx<T>::fmax_(Fx<T>::fmax_(P::lo(M[x]), P::hi(M[x])), Fx<T>::fmax_(P::lo(I[x]), P::hi(I[x]))));
-            m = Fx<T>::fmax_(m, Fx<T>::fmax_(P::lo(S[x]), P::hi(S[x])));
-        }
-        m = Fx<T>::fmax_(m, Fx<T>::fmax_(Fx<T>::fmax_(P::lo(inM), P::hi(inM)), Fx<T>::fmax_(P::lo(inS), P::hi(inS))));
-        m = Fx<T>::fmax_(m, Fx<T>::fmax_(Fx<T>::fmax_(P::lo(inI), P::hi(inI)), Fx<T>::fmax_(P::lo(sig), P::hi(sig))));
-        (void)mv;
-        if (m > (T)0) {
-            int e = Fx<T>::ilogb(m);
-            if (e > Fx<T>::TGT + Fx<T>::PER_HI || e < Fx<T>::TGT - Fx<T>::PER_LO) rescale(e - Fx<T>::TGT);
-        } else {
-            ex = EX_ZERO;
-        }
-    }
-
-    // One systolic step.  E: constants of the row the .x half processes now; (lM, lI, lS, lSig): the
-    // left neighbour's last-column values of that same row (already at this thread's exponent).
-    __device__ __forceinline__ void step(const RowConst<T>& E, T lM, T lI, T lS, T lSig) {
-        // .y inherits what .x had one step ago
-        cA = P::pack(E.a, P::lo(cA));
-        cPm = P::pack(E.pm, P::lo(cPm));
-        cPx = P::pack(E.px, P::lo(cPx));
-        cC = P::pack(E.c, P::lo(cC));
-        cGi = P::pack(E.gi, P::lo(cGi));
-        cGI = P::pack(E.gI, P::lo(cGI));
-        cGm = P::pack(E.gm, P::lo(cGm));
-        metaY = metaX;
-        metaX = E.meta;
-        // diagonal inputs of column 0 = boundary of the previous row; same-row boundary = new
-        V dM = inM, dI = inI, dS = inS;
-        inM = P::pack(lM, P::lo(M[NV - 1]));
-        inI = P::pack(lI, P::lo(I[NV - 1]));
-        inS = P::pack(lS, P::lo(S[NV - 1]));
-        V sigIn = P::pack(lSig, P::lo(sig));
-        const uint32_t rx = selmask(mx, metaX & META_CODE_MASK), ry = selmask(my, metaY & META_CODE_MASK);
-        const T pmx = P::lo(cPm), pmy = P::hi(cPm), pxx = P::lo(cPx), pxy = P::hi(cPx);
-        // pass 1, columns in DESCENDING order so that every update is in place (column x reads the
-        // old values of column x-1, which are overwritten only afterwards); groups of CG columns are
-        // software-pipelined by hand (stage by stage) because the packed ops are order-pinned asm.
-        constexpr int CG = 4;
-        static_assert(NV % CG == 0, "NV must be a multiple of 4");
+                    for (int x = 0; x < NV; x++) a += J[x].x;
+                } else {
 #pragma unroll
-        for (int xb = NV - CG; xb >= 0; xb -= CG) {
-            V t[CG], u[CG], p[CG];
-#pragma unroll
-            for (int q = CG - 1; q >= 0; q--) {
-                const int x = xb + q;
-                t[q] = P::fma(cA, (x > 0) ? M[x - 1] : dM, (x > 0) ? I[x - 1] : dI);
+                    for (int x = 0; x < NV; x++) a += (x < nvx) ? J[x].x : (T)0;
+                }
+                sigX = inSig + a;
             }
+            if (E.metaY & META_LAST) {
+                T a = (T)0;
+                if (nvy == NV) {
 #pragma unroll
-            for (int q = CG - 1; q >= 0; q--) {
-                const int x = xb + q;
-                t[q] = P::fma(cC, (x > 0) ? S[x - 1] : dS, t[q]);
-                p[q] = P::pack(((rx >> x) & 1u) ? pmx : pxx, ((ry >> x) & 1u) ? pmy : pxy);  // Eq.3
+                    for (int x = 0; x < NV; x++) a += J[x].y;
+                } else {
+#pragma unroll
+                    for (int x = 0; x < NV; x++) a += (x < nvy) ? J[x].y : (T)0;
+                }
+                sigY = sigX + a;
             }
-#pragma unroll
-            for (int q = CG - 1; q >= 0; q--) u[q] = P::mul(cGi, M[xb + q]);
-#pragma unroll
-            for (int q = CG - 1; q >= 0; q--) I[xb + q] = P::fma(cGI, I[xb + q], u[q]);
-#pragma unroll
-            for (int q = CG - 1; q >= 0; q--) M[xb + q] = P::mul(p[q], t[q]);
         }
-        // pass 2, ascending: the weighted prefix sums of the new row (Eq.6), S[x] exclusive of column x
-        S[0] = P::fma(cGm, inS, inM);
-#pragma unroll
-        for (int x = 1; x < NV; x++) S[x] = P::fma(cGm, S[x - 1], M[x - 1]);
-        // Eq.4 on the last row of a read: this thread's share, added to what came from the left
-        T sx = P::lo(sigIn), sy = P::hi(sigIn);
-        if ((metaX | metaY) & META_LAST) {
-            T ax = (T)0, ay = (T)0;
-#pragma unroll
-            for (int x = 0; x < NV; x++) {
-                V t = P::add(M[x], I[x]);
-                ax += (x < nvx) ? P::lo(t) : (T)0;
-                ay += (x < nvy) ? P::hi(t) : (T)0;
-            }
-            sx = (metaX & META_LAST) ? sx + ax : (T)0;
-            sy = (metaY & META_LAST) ? sy + ay : (T)0;
-        } else {
-            sx = (T)0; sy = (T)0;
-        }
-        sig = P::pack(sx, sy);
     }
-
-    __device__ __forceinline__ T outM() const { return P::hi(M[NV - 1]); }
-    __device__ __forceinline__ T outI() const { return P::hi(I[NV - 1]); }
-    __device__ __forceinline__ T outS() const { return P::hi(S[NV - 1]); }
-    __device__ __forceinline__ T outSig() const { return P::hi(sig); }
 };
 
 }  // namespace phmm

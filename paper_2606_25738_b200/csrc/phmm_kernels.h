@@ -12,6 +12,8 @@ constexpr int SHORT_MAX_K = 32 * SHORT_N2;  // 1024: widest haplotype one warp c
 constexpr int CHAIN_NV_F32 = 16;
 constexpr int CHAIN_NV_F64 = 8;
 constexpr int SHORT_WARPS_PER_CTA = 4;
+constexpr int TABLE_ZERO_RUN = 256;       // all-zero entries at the start of the row-constant table (idle lanes read them)
+constexpr int TABLE_EXTRA_ROWS = 2;       // run-in entry in front of and flush entry behind every read's rows (phmm_short.cu)
 
 struct DevBatch {  // device mirrors of the batch
     const uint8_t *read_bases, *qual_base, *qual_ins, *qual_del, *qual_gcp, *hap_bases;
@@ -24,11 +26,11 @@ struct ShortTask {  // one lane group's work: several reads streamed against one
 };
 
 struct ShortLaunch {
-    const float* table;        // 8 floats per entry; read r starts at entry read_off[r] + r
+    const float* table;        // 16 floats (64 bytes) per entry; see k_table_f32 for the layout
     const ShortTask* tasks;    // ordered by warp
     const int* warp_first;     // n_warps+1: first task of each warp
     int n_warps;
-    const int* srt_read;       // read index of each sorted pair
+    const int2* srt_ent;       // (first table entry, number of entries = read length + TABLE_EXTRA_ROWS) of each sorted pair
     const int* srt_out;        // caller's pair index of each sorted pair
     double* out;
     uint8_t* flags;

@@ -5,37 +5,87 @@
 // row), a9 (final reduction, log10), a10 (underflow detection -> rescue queue).
 #include "phmm_engine.cuh"
 #include "phmm_kernels.h"
+#include <type_traits>
+
+#ifndef SHORT_MIN_CTAS
+#define SHORT_MIN_CTAS 4  // resident CTAs per SM the register allocation is held to (4 x 128 threads -> <= 128 registers)
+#endif
 
 namespace phmm {
 
 // ------------------------------------------------------------------ a1: row-constant table
-// One warp per read; entry 0 = reset row, entries 1..l = read rows.  Constants are formed in double
-// from the 10^(-q/10) table and rounded once to float ("q32" table; Listing 2
-// :293-295 for which qualities enter which transition).
+// Stream of entries of one read of length l ("run", l + TABLE_EXTRA_ROWS entries), see phmm_engine.cuh:
+//   e = 0      run-in entry: P = 0 (U = 0), gamma := 1, C := g_1, G := 0, meta FIRST.  The group's first lane
+//              injects s = C/k, which the chain carries unchanged through every column, so the step leaves
+//              T = g_1 C/k (= T_DM_1 D_{0,j-1}, Eq.1-2 under reading G1) and J = 0: the state in front of row 1.
+//   e = 1..l   read row i = e:  P = (pm_i | px_i) gi_{i+1}, gamma_i, A = a_{i+1}/gi_{i+1}, C = g_{i+1} d_i/gi_{i+1},
+//              G = gamma_{i+1} g_{i+2}/g_{i+1};  on the last row gi_{l+1} := 1, A := C := 0, G := 1, meta LAST, so
+//              that the step leaves J = M_l + I_l, the summand of Eq.4.
+//   e = l+1    flush entry, all zero: gives the .y half (one entry behind) its step for row l and zeroes J.
+// Each 64-byte table entry holds the constants of entry e (for the .x half) and of entry e-1 (for .y; zero
+// for e = 0), already paired the way FFMA2 wants them:
+//   float4 0: gamma.x gamma.y A.x A.y | 1: C.x C.y G.x G.y | 2: pm.x px.x pm.y px.y | 3: meta.x meta.y 0 0
+// The table starts with TABLE_ZERO_RUN all-zero entries (what idle lanes fetch); read r's run starts at
+// entry TABLE_ZERO_RUN + read_off[r] + TABLE_EXTRA_ROWS r.  Constants are formed in double from the
+// 10^(-q/10) table and rounded once ("q32" table; Listing 2 :293-295 for which
+// qualities enter which transition).  One warp per read.
+// Memory layout: the entries are permuted inside blocks of 32 so that the lanes of a warp, which read entries
+// two apart (lane L's .x half is 2L entries behind lane 0's), touch consecutive 16-byte slots: block = 2 KB =
+// 4 chunk planes (the four float4 of an entry) x 2 parities x 16 slots.  A lane-strided LDG.128 then costs
+// ~4 L1 wavefronts instead of 32 (ncu: l1tex throughput 90 % -> see profiles/).
+constexpr int TABLE_CHUNK_STRIDE = 32;  // float4 units between the chunk planes of a block
+__host__ __device__ __forceinline__ int64_t table_slot(int64_t pos) {  // float4 index of chunk 0 of entry pos
+    return (pos >> 5) * 128 + (pos & 1) * 16 + ((pos >> 1) & 15);
+}
+
+struct RowC { double gam, A, C, G, pm, px; uint32_t meta; };
+
+__device__ __forceinline__ RowC row_constants(const DevBatch& b, const double* __restrict__ lut, int64_t off, int l, int e) {
+    RowC c = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0u};
+    if (e == 0) {
+        c.gam = 1.0; c.C = 1.0 - lut[b.qual_gcp[off]]; c.meta = META_FIRST;
+    } else if (e >= 1 && e <= l) {
+        const int i = e;  // read row, 1-based
+        const double eps = lut[b.qual_base[off + i - 1]];
+        const int code = base_code(b.read_bases[off + i - 1]);
+        c.meta = (uint32_t)(code & 3) | (i == l ? META_LAST : 0u);
+        c.gam = lut[b.qual_gcp[off + i - 1]];
+        double gin = 1.0;  // gi_{i+1} = g_{i+2} iota_{i+1};  := 1 behind the last row
+        if (i < l) {
+            const double g1 = 1.0 - lut[b.qual_gcp[off + i]];                              // g_{i+1}
+            const double g2 = (i + 1 < l) ? 1.0 - lut[b.qual_gcp[off + i + 1]] : 1.0;      // g_{i+2}, := 1 behind the last row
+            const double io1 = lut[b.qual_ins[off + i]], de1 = lut[b.qual_del[off + i]];   // iota_{i+1}, d_{i+1}
+            gin = g2 * io1;
+            c.A = (1.0 - io1 - de1) / gin;
+            c.C = g1 * lut[b.qual_del[off + i - 1]] / gin;
+            c.G = lut[b.qual_gcp[off + i]] * g2 / g1;
+        } else {
+            c.G = 1.0;
+        }
+        c.pm = (code < 4 ? 1.0 - eps : eps / 3.0) * gin;  // a non-ACGT read base matches nothing (reading G17)
+        c.px = eps / 3.0 * gin;
+    }
+    return c;
+}
+
 __global__ void __launch_bounds__(256) k_table_f32(DevBatch b, const double* __restrict__ lut, float* __restrict__ table) {
     const int64_t r = (int64_t)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
     if (r >= b.n_reads) return;
     const int lane = threadIdx.x & 31;
+    const float4 Z = make_float4(0.f, 0.f, 0.f, 0.f);
+    if (blockIdx.x == 0)
+        for (int i = threadIdx.x; i < 4 * TABLE_ZERO_RUN; i += blockDim.x) reinterpret_cast<float4*>(table)[i] = Z;  // whole blocks
     const int64_t off = b.read_off[r];
     const int l = (int)(b.read_off[r + 1] - off);
-    float4* dst = reinterpret_cast<float4*>(table) + 2 * (off + r);
-    for (int i = lane; i <= l; i += 32) {
-        float4 A, B;
-        if (i == 0) {
-            A = make_float4(0.f, 0.f, 0.f, 0.f);
-            B = make_float4(0.f, 0.f, 1.f, (float)META_RESET);
-        } else {
-            const double eps = lut[b.qual_base[off + i - 1]], io = lut[b.qual_ins[off + i - 1]];
-            const double de = lut[b.qual_del[off + i - 1]], ga = lut[b.qual_gcp[off + i - 1]];
-            const double g = 1.0 - ga;
-            const double gn = (i < l) ? 1.0 - lut[b.qual_gcp[off + i]] : 1.0;
-            const double dp = (i > 1) ? lut[b.qual_del[off + i - 2]] : 1.0;
-            uint32_t meta = (uint32_t)base_code(b.read_bases[off + i - 1]) | (i == l ? META_LAST : 0u);
-            A = make_float4((float)(1.0 - io - de), (float)(1.0 - eps), (float)(eps / 3.0), (float)(g * dp));
-            B = make_float4((float)(gn * io), (float)(ga * gn / g), (float)ga, (float)meta);
-        }
-        dst[2 * i] = A;
-        dst[2 * i + 1] = B;
+    float4* dst = reinterpret_cast<float4*>(table);
+    const int64_t first = TABLE_ZERO_RUN + off + TABLE_EXTRA_ROWS * r;
+    for (int e = lane; e < l + TABLE_EXTRA_ROWS; e += 32) {
+        const RowC x = row_constants(b, lut, off, l, e), y = row_constants(b, lut, off, l, e - 1);
+        float4* d = dst + table_slot(first + e);
+        d[0 * TABLE_CHUNK_STRIDE] = make_float4((float)x.gam, (float)y.gam, (float)x.A, (float)y.A);
+        d[1 * TABLE_CHUNK_STRIDE] = make_float4((float)x.C, (float)y.C, (float)x.G, (float)y.G);
+        d[2 * TABLE_CHUNK_STRIDE] = make_float4((float)x.pm, (float)x.px, (float)y.pm, (float)y.px);
+        d[3 * TABLE_CHUNK_STRIDE] = make_float4(__uint_as_float(x.meta), __uint_as_float(y.meta), 0.f, 0.f);
     }
 }
 
@@ -48,15 +98,21 @@ cudaError_t launch_lut_table(const DevBatch& b, const double* lut, float* table,
 }
 
 // ------------------------------------------------------------------ the short kernel
-template <int NV> struct Cursor {  // where a lane's .x half is in its task's stream of table entries
-    const float4* cur;
-    const float4* nxt;
-    int rem, nxtRem, q, wait;
+// Per lane, the .x half walks its task's stream of table entries (run of read 1, run of read 2, ...) starting
+// 2*lg steps after the group's first lane.  While it waits, and after its stream has ended, a lane walks the
+// zero run at the start of the table (all-zero constants decay T and J to 0), so the fetch needs no special
+// cases.  Entries are loaded one step ahead into two alternating register sets (step loop unrolled by two).
+struct Cursor {
+    int pos, end;        // next entry to fetch, one past the last entry of the current run
+    int npos, nend;      // the run after it: the next read of the task, or the zero run
+    int q;               // reads of the task already handed to (npos, nend)
 };
 
+struct RawEntry { float4 a, b, c; uint2 m; };
+
 template <int NV>
-__global__ void __launch_bounds__(SHORT_WARPS_PER_CTA * 32, 3) k_short_f32(DevBatch b, ShortLaunch p) {
-    typedef Lane<float, NV, false> L;
+__global__ void __launch_bounds__(SHORT_WARPS_PER_CTA * 32, SHORT_MIN_CTAS) k_short_f32(DevBatch b, ShortLaunch p) {
+    typedef Lane2<float, NV> L;
     constexpr int N2 = 2 * NV;
     const int warp = blockIdx.x * SHORT_WARPS_PER_CTA + (threadIdx.x >> 5);
     if (warp >= p.n_warps) return;
@@ -95,7 +151,7 @@ __global__ void __launch_bounds__(SHORT_WARPS_PER_CTA * 32, 3) k_short_f32(DevBa
     const bool is_last = (ti >= 0) && lg == m_g - 1;
 
     // ---- number of steps of this warp: the last lane's .y half finishes the last entry of its stream
-    int steps = (ti < 0) ? 0 : m_rows + m_np + 2 * m_g - 1;
+    int steps = (ti < 0) ? 0 : m_rows + TABLE_EXTRA_ROWS * m_np + 2 * m_g - 1;
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) steps = max(steps, __shfl_xor_sync(PHMM_FULL, steps, o));
 
@@ -104,55 +160,50 @@ __global__ void __launch_bounds__(SHORT_WARPS_PER_CTA * 32, 3) k_short_f32(DevBa
     ln.load_hap(b.hap_bases + (ti < 0 ? 0 : b.hap_off[m_hap]), m_k, lg * N2);
     const float Cok = (float)(ldexp(1.0, 120) / (double)(m_k > 0 ? m_k : 1));  // Eq.1: C/k with C = 2^120
 
-    // ---- stream cursor of the .x half (entry for step s is fetched during step s-1)
     const float4* tab = reinterpret_cast<const float4*>(p.table);
-    Cursor<NV> c;
-    c.cur = tab; c.nxt = tab; c.rem = 0; c.nxtRem = 0; c.q = 0; c.wait = 2 * lg;
+    const int2* ent = p.srt_ent + m_first;
+    Cursor c;
+    c.q = 0;
     auto load_next = [&]() {
+        c.npos = 0; c.nend = TABLE_ZERO_RUN;
         if (c.q < m_np) {
-            const int r = p.srt_read[m_first + c.q];
+            const int2 e = __ldg(ent + c.q);
             c.q++;
-            const int64_t o = b.read_off[r];
-            c.nxt = tab + 2 * (o + r);
-            c.nxtRem = (int)(b.read_off[r + 1] - o) + 1;
-        } else {
-            c.nxtRem = 0;
+            c.npos = e.x; c.nend = e.x + e.y;
         }
     };
+    c.pos = TABLE_ZERO_RUN - 2 * lg; c.end = TABLE_ZERO_RUN;  // 2*lg idle steps before the stream starts
     load_next();
-    float4 eA = make_float4(0.f, 0.f, 0.f, 0.f), eB = make_float4(0.f, 0.f, 0.f, 0.f);
-    auto fetch = [&]() {
-        eA = make_float4(0.f, 0.f, 0.f, 0.f);
-        eB = make_float4(0.f, 0.f, 0.f, 0.f);
-        if (c.wait > 0) {
-            c.wait--;
-        } else {
-            if (c.rem == 0) { c.cur = c.nxt; c.rem = c.nxtRem; load_next(); }
-            if (c.rem > 0) {
-                eA = __ldg(c.cur);
-                eB = __ldg(c.cur + 1);
-                c.cur += 2;
-                c.rem--;
-            }
-        }
+    auto fetch = [&](RawEntry& r) {
+        if (c.pos == c.end) { c.pos = c.npos; c.end = c.nend; load_next(); }
+        const float4* e = tab + table_slot(c.pos);
+        c.pos++;
+        r.a = __ldg(e);
+        r.b = __ldg(e + TABLE_CHUNK_STRIDE);
+        r.c = __ldg(e + 2 * TABLE_CHUNK_STRIDE);
+        r.m = __ldg(reinterpret_cast<const uint2*>(e + 3 * TABLE_CHUNK_STRIDE));
     };
-    fetch();
 
     int nout = 0;
     const double LOG10_2 = 0.30102999566398119521;
-    for (int s = 0; s < steps; s++) {
-        RowConst<float> E;
-        E.a = eA.x; E.pm = eA.y; E.px = eA.z; E.c = eA.w;
-        E.gi = eB.x; E.gI = eB.y; E.gm = eB.z; E.meta = (uint32_t)eB.w;
-        fetch();  // prefetch the next step's entry
-        float lM = __shfl_up_sync(PHMM_FULL, ln.outM(), 1);
-        float lI = __shfl_up_sync(PHMM_FULL, ln.outI(), 1);
-        float lS = __shfl_up_sync(PHMM_FULL, ln.outS(), 1);
-        float lSig = __shfl_up_sync(PHMM_FULL, ln.outSig(), 1);
-        if (is_first) { lM = 0.f; lI = 0.f; lSig = 0.f; lS = (E.meta & META_RESET) ? Cok : 0.f; }
-        ln.step(E, lM, lI, lS, lSig);
-        if (is_last && (ln.metaY & META_LAST)) {
-            const float sg = ln.outSig();
+    auto one_step = [&](const RawEntry& r) {
+        Entry2<float> E;
+        E.gam = make_float2(r.a.x, r.a.y); E.A = make_float2(r.a.z, r.a.w);
+        E.C = make_float2(r.b.x, r.b.y); E.G = make_float2(r.b.z, r.b.w);
+        E.pmx = r.c.x; E.pxx = r.c.y; E.pmy = r.c.z; E.pxy = r.c.w;
+        E.metaX = r.m.x; E.metaY = r.m.y;
+        float inS = __shfl_up_sync(PHMM_FULL, ln.outS.y, 1);
+        float inT = __shfl_up_sync(PHMM_FULL, ln.outT.y, 1);
+        float inSig = __shfl_up_sync(PHMM_FULL, ln.sigY, 1);
+        if (is_first) {  // column-0 boundary, Eq.1
+            const bool f = (E.metaX & META_FIRST) != 0;
+            inS = f ? Cok : 0.f;
+            inT = f ? E.C.x * Cok : 0.f;
+            inSig = 0.f;
+        }
+        ln.step(E, inS, inT, inSig);
+        if (is_last && (E.metaY & META_LAST)) {
+            const float sg = ln.sigY;
             const int pair = p.srt_out[m_first + nout];
             nout++;
             if (isfinite(sg) && sg >= p.rescue_thr) {
@@ -163,6 +214,14 @@ __global__ void __launch_bounds__(SHORT_WARPS_PER_CTA * 32, 3) k_short_f32(DevBa
                 p.rescue_list[idx] = pair;
             }
         }
+    };
+    RawEntry eA, eB;
+    fetch(eA);
+    for (int s = 0; s < steps; s += 2) {  // an odd step count runs one extra all-idle step, which is harmless
+        fetch(eB);
+        one_step(eA);
+        fetch(eA);
+        one_step(eB);
     }
 }
 
