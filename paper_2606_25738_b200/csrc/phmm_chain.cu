@@ -1,27 +1,72 @@
 // Generic rescaled path ("chain" kernel): one warp = one strip of 32 lanes x 2NV haplotype columns of
 // one pair; the strips of a pair are chained left to right through boundary-column buffers in
-// global memory (the last column's M, I', S, running final sum and block exponent for every read
-// row), either concurrently (one strip per warp, progress counters; warps take strips in ticket
-// order so a producer always holds an earlier ticket than its consumer => forward progress) or
-// sequentially inside one warp (rescue of short pairs, fp64 mode).
+// global memory (per stream entry: the running sum s and the T that drop out of the strip's last
+// column, the Eq.4 partial sum, and the strip's block exponent), either concurrently (one strip per
+// warp, progress counters; warps take strips in ticket order so a producer always holds an earlier
+// ticket than its consumer => forward progress) or sequentially inside one warp (fp64 rescue of
+// short pairs, PHMM_FP64 mode).
 //
 // a1 (row constants, computed on the fly into a shared-memory ring), a4,
 // a5, a6/a7 (cross-warp / cross-CTA carry -- the paper's Eq.10/11 lock-step carries, PAPER.md:263-267,
 // :319-324, become a skewed wavefront with 32-row handoff blocks), a8 (rescaling), a9, a10 (fp64 rescue).
-// Block-floating arithmetic: every thread keeps one integer exponent for all it holds; values
-// crossing a thread boundary are converted exactly by a power of two.
-#include "phmm_engine_v0.cuh"
+//
+// Rescaling (reading G15; absent from the paper).  Block floating point per THREAD: true value = stored
+// value * 2^ex with one integer ex for everything a thread holds (the T/J state of its two halves, the
+// values it hands to the right, its Eq.4 partial sums).  The lanes of a warp are 2 read rows apart, so
+// a warp spans 64 rows and, along a row, 32 columns per lane: with unrelated sequence (3.3 bits lost
+// per row or per deleted column) that is more than fp32's exponent range, hence no coarser unit.
+// Every 16 steps a thread takes the maximum of what it holds and, if that left the window around
+// 2^TGT, multiplies everything by the power of two that brings it back (exact, except that values
+// more than the format's range below the thread maximum flush to zero: G15's documented limit).
+// The three values crossing a lane (or strip) boundary per step come with the producer's ex and are
+// converted by one exact multiply; if they would not fit, the consumer first moves its own exponent
+// up.  The recurrence step itself is exactly the short kernel's (phmm_engine.cuh).
+#include "phmm_engine.cuh"
 #include "phmm_kernels.h"
+#include "phmm_rowconst.cuh"
 
 namespace phmm {
 
 constexpr int CHAIN_WARPS = 4;
-constexpr int RING = 128;  // row-constant ring per warp (entries); must cover 62 rows of skew + two 32-row blocks
+constexpr int RING = 128;  // row-constant ring per warp (entries); covers 63 entries of skew + two 32-entry blocks
 
-template <typename T> struct Rec {  // boundary block of 32 entries, SoA
-    T M[32], I[32], S[32], Sig[32];
+template <typename T> struct Rec {  // boundary block of 32 stream entries, SoA
+    T S[32], Tn[32], Sig[32];
     int ex[32];
 };
+
+// ---- ring entry format: NCH chunks of 16 bytes per entry, paired (.x = entry e, .y = entry e-1) like the
+// short path's table; chunk planes of RING slots, the two parities of the slot index in separate halves of
+// a plane so that lanes (which read entries two apart) hit consecutive 16-byte words: conflict-free LDS.128.
+template <typename T> struct RingFmt;
+template <> struct RingFmt<float> {
+    static constexpr int NCH = 4;  // {gam.x gam.y A.x A.y} {C.x C.y G.x G.y} {pm.x px.x pm.y px.y} {meta.x meta.y - -}
+    static constexpr int SPW = 4;  // scalars per 16-byte word
+    static __device__ __forceinline__ int pair_at(int f, int half) { return (f >> 1) * 4 + (f & 1) * 2 + half; }  // f: 0 gam 1 A 2 C 3 G
+    static __device__ __forceinline__ int prior_at(int which, int half) { return 2 * 4 + half * 2 + which; }     // which: 0 pm 1 px
+    static __device__ __forceinline__ int meta_at(int half) { return 3 * 4 + half; }
+    static __device__ __forceinline__ float meta_val(uint32_t m) { return __uint_as_float(m); }
+    static __device__ __forceinline__ uint32_t meta_get(float v) { return __float_as_uint(v); }
+};
+template <> struct RingFmt<double> {
+    static constexpr int NCH = 8;  // {gam} {A} {C} {G} {pm.x px.x} {pm.y px.y} {meta.x meta.y} {-}
+    static constexpr int SPW = 2;
+    static __device__ __forceinline__ int pair_at(int f, int half) { return f * 2 + half; }
+    static __device__ __forceinline__ int prior_at(int which, int half) { return (4 + half) * 2 + which; }
+    static __device__ __forceinline__ int meta_at(int half) { return 6 * 2 + half; }
+    static __device__ __forceinline__ double meta_val(uint32_t m) { return __hiloint2double(0, (int)m); }
+    static __device__ __forceinline__ uint32_t meta_get(double v) { return (uint32_t)__double2loint(v); }
+};
+
+template <typename T> struct Smem {
+    T ring[RingFmt<T>::NCH * RING * RingFmt<T>::SPW];  // [chunk][parity][slot/2][scalars of the 16-byte word]
+    Rec<T> rin, rout;
+};
+
+__device__ __forceinline__ int ring_word(int e) {  // index (in 16-byte words, within a chunk plane) of entry e
+    const int sl = e & (RING - 1);
+    return (sl & 1) * (RING / 2) + (sl >> 1);
+}
 
 __device__ __forceinline__ int ld_acquire(const int* p) {
     int v;
@@ -32,18 +77,70 @@ __device__ __forceinline__ void st_release(int* p, int v) {
     asm volatile("st.release.gpu.global.s32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
 }
 
-template <typename T, int NV>
-__global__ void __launch_bounds__(CHAIN_WARPS * 32, (sizeof(T) == 4 ? 2 : 2))
+// v * 2^d, exact unless it leaves the format (d may exceed one factor's exponent range)
+template <typename T> __device__ __forceinline__ T scale_pow2(T v, int d) {
+    d = max(-Fx<T>::CLAMP, min(Fx<T>::CLAMP, d));
+    const int h = d / 2;
+    return v * Fx<T>::exp2i(h) * Fx<T>::exp2i(d - h);
+}
+
+template <typename T> struct Win;  // keep the thread maximum within 2^(TGT +- WIN); incoming values above 2^(TGT+UP) move ex first
+template <> struct Win<float> { static constexpr int TGT = 60, WIN = 30, UP = 50; };
+template <> struct Win<double> { static constexpr int TGT = 0, WIN = 400, UP = 600; };
+
+template <typename T> __device__ __forceinline__ T warp_max(T m) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) m = Fx<T>::fmax_(m, __shfl_xor_sync(PHMM_FULL, m, o));
+    return m;
+}
+__device__ __forceinline__ int warp_max_i(int m) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) m = max(m, __shfl_xor_sync(PHMM_FULL, m, o));
+    return m;
+}
+
+template <typename T, int NV> __device__ __forceinline__ T lane_max(const Lane2<T, NV>& ln) {
+    T m = Fx<T>::fmax_(Fx<T>::fmax_(ln.outS.x, ln.outS.y), Fx<T>::fmax_(ln.outT.x, ln.outT.y));
+    m = Fx<T>::fmax_(m, Fx<T>::fmax_(ln.sigX, ln.sigY));
+#pragma unroll
+    for (int x = 0; x < NV; x++) {
+        m = Fx<T>::fmax_(m, Fx<T>::fmax_(ln.Tt[x].x, ln.Tt[x].y));
+        m = Fx<T>::fmax_(m, Fx<T>::fmax_(ln.J[x].x, ln.J[x].y));
+    }
+    return m;
+}
+template <typename T, int NV> __device__ __forceinline__ void lane_scale(Lane2<T, NV>& ln, int d) {  // *= 2^d
+    d = max(-Fx<T>::CLAMP, min(Fx<T>::CLAMP, d));
+    const int h = d / 2;
+    const T f1 = Fx<T>::exp2i(h), f2 = Fx<T>::exp2i(d - h);
+    typedef W2<T> P;
+    const typename P::V F1 = P::mk(f1, f1), F2 = P::mk(f2, f2);
+#pragma unroll
+    for (int x = 0; x < NV; x++) {
+        ln.Tt[x] = P::mul(P::mul(ln.Tt[x], F1), F2);
+        ln.J[x] = P::mul(P::mul(ln.J[x], F1), F2);
+    }
+    ln.outS = P::mul(P::mul(ln.outS, F1), F2);
+    ln.outT = P::mul(P::mul(ln.outT, F1), F2);
+    ln.sigX = ln.sigX * f1 * f2;
+    ln.sigY = ln.sigY * f1 * f2;
+}
+
+template <typename T, int NV, int WPC>
+__global__ void __launch_bounds__(WPC * 32, (sizeof(T) == 4 ? 3 : 2))
 k_chain(DevBatch b, ChainLaunch p, int items_are_pairs) {
-    typedef LaneV0<T, NV, true> L;
+    typedef Lane2<T, NV> L;
+    typedef RingFmt<T> RF;
+    typedef typename W2<T>::V V;
     constexpr int N2 = 2 * NV;
-    __shared__ T ring[CHAIN_WARPS][8][RING];        // row constants, SoA: [field][slot]
-    __shared__ Rec<T> rin[CHAIN_WARPS], rout[CHAIN_WARPS];
+    __shared__ __align__(16) Smem<T> sm_all[WPC];
     const int w = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int gwarp = blockIdx.x * CHAIN_WARPS + w;
-    T(*rg)[RING] = ring[w];
-    Rec<T>& RI = rin[w];
-    Rec<T>& RO = rout[w];
+    const int gwarp = blockIdx.x * WPC + w;
+    Smem<T>& sm = sm_all[w];
+    T* rg = sm.ring;
+    const V* rgv = reinterpret_cast<const V*>(sm.ring);  // fp32: 8-byte pairs; fp64: 16-byte pairs
+    Rec<T>& RI = sm.rin;
+    Rec<T>& RO = sm.rout;
     const double LOG10_2 = 0.30102999566398119521;
     const int n_items = *p.n_items;
 
@@ -64,8 +161,9 @@ k_chain(DevBatch b, ChainLaunch p, int items_are_pairs) {
         const int r = p.pair_read[pair], h = p.pair_hap[pair];
         const int64_t ro = b.read_off[r], ho = b.hap_off[h];
         const int l = (int)(b.read_off[r + 1] - ro), k = (int)(b.hap_off[h + 1] - ho);
+        const int n_ent = l + TABLE_EXTRA_ROWS;  // run-in entry, rows 1..l, flush entry
         const int nstrips = (k + 32 * N2 - 1) / (32 * N2);
-        const int nblk = (l + 1 + 31) / 32;  // boundary blocks per buffer
+        const int nblk = (n_ent + 31) / 32;  // boundary blocks per buffer
         const int st_lo = strip < 0 ? 0 : strip, st_hi = strip < 0 ? nstrips : strip + 1;
         const T Cok = (T)(ldexp(1.0, p.log2C) / (double)k);
         Rec<T>* bufbase = reinterpret_cast<Rec<T>*>(p.boundary);
@@ -90,81 +188,133 @@ k_chain(DevBatch b, ChainLaunch p, int items_are_pairs) {
             L ln;
             ln.init();
             ln.load_hap(b.hap_bases + ho, k, (st * 32 + lane) * N2);
-            const int steps = l + 64;
+            int ex = 0;        // true value = stored value * 2^ex, one exponent per thread
+            bool zero = true;  // this thread holds nothing but zeros
+            __syncwarp();
+            for (int i = lane; i < RF::NCH * RING * RF::SPW; i += 32) rg[i] = (T)0;
+            __syncwarp();
+            const int steps = n_ent + 63;
             for (int s = 0; s < steps; s++) {
-                if ((s & 31) == 0) {
-                    __syncwarp();
-                    // ---- a1: constants of entries s..s+31 (entry 0 = reset row), one per lane
-                    const int e = s + lane;
-                    if (e <= l) {
-                        T c0 = 0, c1 = 0, c2 = 0, c3 = 0, c4 = 0, c5 = 0, c6 = 1;
-                        uint32_t meta = META_RESET;
-                        if (e > 0) {
-                            const double eps = p.lut[b.qual_base[ro + e - 1]], io = p.lut[b.qual_ins[ro + e - 1]];
-                            const double de = p.lut[b.qual_del[ro + e - 1]], ga = p.lut[b.qual_gcp[ro + e - 1]];
-                            const double g = 1.0 - ga;
-                            const double gn = (e < l) ? 1.0 - p.lut[b.qual_gcp[ro + e]] : 1.0;
-                            const double dp = (e > 1) ? p.lut[b.qual_del[ro + e - 2]] : 1.0;
-                            meta = (uint32_t)base_code(b.read_bases[ro + e - 1]) | (e == l ? META_LAST : 0u);
-                            c0 = (T)(1.0 - io - de); c1 = (T)(1.0 - eps); c2 = (T)(eps / 3.0); c3 = (T)(g * dp);
-                            c4 = (T)(gn * io); c5 = (T)(ga * gn / g); c6 = (T)ga;
+                if ((s & 15) == 0) {
+                    const bool blk = (s & 31) == 0;
+                    if (blk) {
+                        __syncwarp();
+                        // ---- a1: constants of entries s..s+31, one per lane; .x fields to the entry's own slot,
+                        //      .y fields to the next entry's slot (whose .y half runs one entry behind)
+                        const int e = s + lane;
+                        const RowC c = row_constants(b, p.lut, ro, l, e < n_ent ? e : -1);
+                        T* lo = rg + ring_word(e) * RF::SPW;
+                        T* hi = rg + ring_word(e + 1) * RF::SPW;
+                        constexpr int PL = RING * RF::SPW;  // scalars per chunk plane
+                        const double pr[4] = {c.gam, c.A, c.C, c.G};
+#pragma unroll
+                        for (int f = 0; f < 4; f++) {
+                            const int a0 = RF::pair_at(f, 0), a1 = RF::pair_at(f, 1);
+                            lo[(a0 / RF::SPW) * PL + a0 % RF::SPW] = (T)pr[f];
+                            hi[(a1 / RF::SPW) * PL + a1 % RF::SPW] = (T)pr[f];
                         }
-                        const int sl = e & (RING - 1);
-                        rg[0][sl] = c0; rg[1][sl] = c1; rg[2][sl] = c2; rg[3][sl] = c3;
-                        rg[4][sl] = c4; rg[5][sl] = c5; rg[6][sl] = c6; rg[7][sl] = (T)meta;
+                        const double pq[2] = {c.pm, c.px};
+#pragma unroll
+                        for (int q = 0; q < 2; q++) {
+                            const int a0 = RF::prior_at(q, 0), a1 = RF::prior_at(q, 1);
+                            lo[(a0 / RF::SPW) * PL + a0 % RF::SPW] = (T)pq[q];
+                            hi[(a1 / RF::SPW) * PL + a1 % RF::SPW] = (T)pq[q];
+                        }
+                        {
+                            const int a0 = RF::meta_at(0), a1 = RF::meta_at(1);
+                            lo[(a0 / RF::SPW) * PL + a0 % RF::SPW] = RF::meta_val(c.meta);
+                            hi[(a1 / RF::SPW) * PL + a1 % RF::SPW] = RF::meta_val(c.meta);
+                        }
                     }
                     // ---- incoming boundary block for entries s..s+31 (lane 0 consumes entry s at step s)
-                    if (has_in && s <= l) {
-                        const int need = min(s + 32, l + 1);
+                    if (blk && has_in && s < n_ent) {
+                        const int need = min(s + 32, n_ent);
                         if (inprog) {
                             while (ld_acquire(inprog) < need) __nanosleep(64);
                         }
                         const Rec<T>* src = inb + (s >> 5);
-                        RI.M[lane] = src->M[lane]; RI.I[lane] = src->I[lane]; RI.S[lane] = src->S[lane];
-                        RI.Sig[lane] = src->Sig[lane]; RI.ex[lane] = src->ex[lane];
+                        RI.S[lane] = src->S[lane]; RI.Tn[lane] = src->Tn[lane]; RI.Sig[lane] = src->Sig[lane];
+                        RI.ex[lane] = src->ex[lane];
+                    }
+                    // ---- a8: block-floating event of this thread
+                    const T m = lane_max<T, NV>(ln);
+                    if (m > (T)0) {
+                        const int e = Fx<T>::ilogb(m);
+                        if (e > Win<T>::TGT + Win<T>::WIN || e < Win<T>::TGT - Win<T>::WIN) {
+                            lane_scale<T, NV>(ln, Win<T>::TGT - e);
+                            ex += e - Win<T>::TGT;
+                        }
+                        zero = false;
+                    } else {
+                        zero = true;  // nothing held: the exponent is free, adopt the next incoming one
                     }
                     __syncwarp();
                 }
-                // ---- this lane's row constants
-                const int pos = s - 2 * lane;
-                RowConstV0<T> E;
-                E.a = E.pm = E.px = E.c = E.gi = E.gI = E.gm = (T)0;
-                E.meta = 0;
-                if (pos >= 0 && pos <= l) {
-                    const int sl = pos & (RING - 1);
-                    E.a = rg[0][sl]; E.pm = rg[1][sl]; E.px = rg[2][sl]; E.c = rg[3][sl];
-                    E.gi = rg[4][sl]; E.gI = rg[5][sl]; E.gm = rg[6][sl]; E.meta = (uint32_t)rg[7][sl];
-                }
-                // ---- left boundary: neighbour lane (shuffle), first strip (Eq.1 injection) or buffer
-                T lM = shfl_up1<T>(ln.outM()), lI = shfl_up1<T>(ln.outI()), lS = shfl_up1<T>(ln.outS());
-                T lSig = shfl_up1<T>(ln.outSig());
-                int exL = __shfl_up_sync(PHMM_FULL, ln.ex, 1);
-                if (lane == 0) {
-                    if (has_in && s <= l) {
-                        const int q = s & 31;
-                        lM = RI.M[q]; lI = RI.I[q]; lS = RI.S[q]; lSig = RI.Sig[q]; exL = RI.ex[q];
+                // ---- this lane's entry: .x half at stream position s - 2 lane, .y half one behind (same ring slot)
+                Entry2<T> E;
+                {
+                    const int wd = ring_word(s - 2 * lane);
+                    constexpr int VPW = 16 / sizeof(V);  // pairs per 16-byte word: 2 (fp32) or 1 (fp64)
+                    constexpr int PLV = RING * VPW;       // pairs per chunk plane
+                    const V* q = rgv + wd * VPW;
+                    if (sizeof(T) == 4) {
+                        E.gam = q[0]; E.A = q[1]; E.C = q[PLV]; E.G = q[PLV + 1];
+                        const V pa = q[2 * PLV], pb = q[2 * PLV + 1], mm = q[3 * PLV];
+                        E.pmx = pa.x; E.pxx = pa.y; E.pmy = pb.x; E.pxy = pb.y;
+                        E.metaX = RF::meta_get(mm.x); E.metaY = RF::meta_get(mm.y);
                     } else {
-                        lM = (T)0; lI = (T)0; lSig = (T)0; exL = 0;
-                        lS = (!has_in && s == 0) ? Cok : (T)0;
+                        E.gam = q[0]; E.A = q[PLV]; E.C = q[2 * PLV]; E.G = q[3 * PLV];
+                        const V pa = q[4 * PLV], pb = q[5 * PLV], mm = q[6 * PLV];
+                        E.pmx = pa.x; E.pxx = pa.y; E.pmy = pb.x; E.pxy = pb.y;
+                        E.metaX = RF::meta_get(mm.x); E.metaY = RF::meta_get(mm.y);
                     }
                 }
-                ln.absorb(lM, lI, lS, lSig, exL);
-                ln.step(E, lM, lI, lS, lSig);
-                if ((s & 15) == 15) ln.periodic();
-                // ---- right boundary of the strip: lane 31's .y half finished entry s-63
+                // ---- left boundary: neighbour lane (shuffle), first strip (Eq.1 injection) or boundary block
+                T inS = shfl_up1<T>(ln.outS.y), inT = shfl_up1<T>(ln.outT.y), inSig = shfl_up1<T>(ln.sigY);
+                int exL = __shfl_up_sync(PHMM_FULL, ex, 1);
+                if (lane == 0) {
+                    if (has_in) {
+                        const int q = s & 31;
+                        const bool ok = s < n_ent;
+                        inS = ok ? RI.S[q] : (T)0; inT = ok ? RI.Tn[q] : (T)0; inSig = ok ? RI.Sig[q] : (T)0;
+                        exL = ok ? RI.ex[q] : ex;
+                    } else {
+                        const bool f = (E.metaX & META_FIRST) != 0;  // Eq.1: only the run-in entry injects, at exponent 0
+                        inS = f ? Cok : (T)0;
+                        inT = f ? E.C.x * Cok : (T)0;
+                        inSig = (T)0;
+                        exL = 0;
+                    }
+                }
+                // ---- bring the incoming values to this thread's exponent (exact power-of-two multiply)
+                {
+                    const T mi = Fx<T>::fmax_(Fx<T>::fmax_(inS, inT), inSig);
+                    if (zero) {
+                        if (mi > (T)0) { ex = exL; zero = false; }
+                    } else if (mi > (T)0 && Fx<T>::ilogb(mi) + exL - ex > Win<T>::TGT + Win<T>::UP) {
+                        const int up = Fx<T>::ilogb(mi) + exL - ex - Win<T>::TGT;  // they would not fit: move this thread up first
+                        lane_scale<T, NV>(ln, -up);
+                        ex += up;
+                    }
+                    const int d = max(-Fx<T>::CLAMP, min(Fx<T>::CLAMP, exL - ex));  // two factors: |d| may exceed one exponent range
+                    const int h = d / 2;
+                    const T f1 = Fx<T>::exp2i(h), f2 = Fx<T>::exp2i(d - h);
+                    inS = inS * f1 * f2; inT = inT * f1 * f2; inSig = inSig * f1 * f2;
+                }
+                ln.step(E, inS, inT, inSig);
+                // ---- right boundary of the strip: lane 31's .y half has just finished entry s - 63
                 const int eo = s - 63;
-                if (eo >= 0) {
+                if (eo >= 0 && eo < n_ent) {
                     if (has_out) {
                         if (lane == 31) {
                             const int q = eo & 31;
-                            RO.M[q] = ln.outM(); RO.I[q] = ln.outI(); RO.S[q] = ln.outS(); RO.Sig[q] = ln.outSig();
-                            RO.ex[q] = ln.ex;
+                            RO.S[q] = ln.outS.y; RO.Tn[q] = ln.outT.y; RO.Sig[q] = ln.sigY; RO.ex[q] = ex;
                         }
-                        if ((eo & 31) == 31 || eo == l) {
+                        if ((eo & 31) == 31 || eo == n_ent - 1) {
                             __syncwarp();
                             Rec<T>* dst = outb + (eo >> 5);
-                            dst->M[lane] = RO.M[lane]; dst->I[lane] = RO.I[lane]; dst->S[lane] = RO.S[lane];
-                            dst->Sig[lane] = RO.Sig[lane]; dst->ex[lane] = RO.ex[lane];
+                            dst->S[lane] = RO.S[lane]; dst->Tn[lane] = RO.Tn[lane]; dst->Sig[lane] = RO.Sig[lane];
+                            dst->ex[lane] = RO.ex[lane];
                             __syncwarp();
                             if (outprog && lane == 0) {
                                 __threadfence();
@@ -172,9 +322,8 @@ k_chain(DevBatch b, ChainLaunch p, int items_are_pairs) {
                             }
                             __syncwarp();
                         }
-                    } else if (eo == l && lane == 31) {
-                        const T sg = ln.outSig();
-                        p.out[pair] = log10((double)sg) + ((double)ln.ex - (double)p.log2C) * LOG10_2;
+                    } else if (eo == l && lane == 31) {  // entry l = the read's last row: Eq.4, log10 in double
+                        p.out[pair] = log10((double)ln.sigY) + ((double)ex - (double)p.log2C) * LOG10_2;
                         if (p.flags) p.flags[pair] = p.flag_bits;
                     }
                 }
@@ -184,28 +333,27 @@ k_chain(DevBatch b, ChainLaunch p, int items_are_pairs) {
     }
 }
 
-static int g_chain_grid = 0;
+constexpr int WPC_F32 = 4, WPC_F64 = 2;
 
 cudaError_t launch_chain(const DevBatch& b, const ChainLaunch& p, bool fp64, bool items_are_pairs, int grid_ctas,
                          cudaStream_t st) {
     if (grid_ctas <= 0) return cudaSuccess;
     if (fp64)
-        k_chain<double, CHAIN_NV_F64><<<grid_ctas, CHAIN_WARPS * 32, 0, st>>>(b, p, items_are_pairs ? 1 : 0);
+        k_chain<double, CHAIN_NV_F64, WPC_F64><<<grid_ctas, WPC_F64 * 32, 0, st>>>(b, p, items_are_pairs ? 1 : 0);
     else
-        k_chain<float, CHAIN_NV_F32><<<grid_ctas, CHAIN_WARPS * 32, 0, st>>>(b, p, items_are_pairs ? 1 : 0);
-    (void)g_chain_grid;
+        k_chain<float, CHAIN_NV_F32, WPC_F32><<<grid_ctas, WPC_F32 * 32, 0, st>>>(b, p, items_are_pairs ? 1 : 0);
     return cudaGetLastError();
 }
 
 int chain_ctas_per_sm(bool fp64) {
     int n = 0;
     if (fp64)
-        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, k_chain<double, CHAIN_NV_F64>, CHAIN_WARPS * 32, 0);
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, k_chain<double, CHAIN_NV_F64, WPC_F64>, WPC_F64 * 32, 0);
     else
-        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, k_chain<float, CHAIN_NV_F32>, CHAIN_WARPS * 32, 0);
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, k_chain<float, CHAIN_NV_F32, WPC_F32>, WPC_F32 * 32, 0);
     return n > 0 ? n : 1;
 }
-int chain_warps_per_cta() { return CHAIN_WARPS; }
+int chain_warps_per_cta(bool fp64) { return fp64 ? WPC_F64 : WPC_F32; }
 size_t chain_block_bytes(bool fp64) { return fp64 ? sizeof(Rec<double>) : sizeof(Rec<float>); }
 int chain_strip_cols(bool fp64) { return 32 * 2 * (fp64 ? CHAIN_NV_F64 : CHAIN_NV_F32); }
 

@@ -70,7 +70,7 @@ cudaError_t launch_short_f32(const DevBatch& b, const ShortLaunch& p, cudaStream
 cudaError_t launch_chain(const DevBatch& b, const ChainLaunch& p, bool fp64, bool items_are_pairs, int grid_ctas,
                          cudaStream_t st);
 int chain_ctas_per_sm(bool fp64);
-int chain_warps_per_cta();
+int chain_warps_per_cta(bool fp64);
 size_t chain_block_bytes(bool fp64);  // bytes of one 32-row boundary block
 int chain_strip_cols(bool fp64);      // haplotype columns covered by one strip
 

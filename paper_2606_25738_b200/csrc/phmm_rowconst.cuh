@@ -1,0 +1,50 @@
+// Row constants of the T/J-form engine (phmm_engine.cuh), shared by the table kernel of the short path and
+// the on-the-fly constant ring of the chain kernel.
+//
+// Stream of entries of one read of length l ("run", l + TABLE_EXTRA_ROWS entries), see phmm_engine.cuh:
+//   e = 0      run-in entry: P = 0 (U = 0), gamma := 1, C := g_1, G := 0, meta FIRST.  The group's first lane
+//              injects s = C/k, which the chain carries unchanged through every column, so the step leaves
+//              T = g_1 C/k (= T_DM_1 D_{0,j-1}, Eq.1-2 under reading G1) and J = 0: the state in front of row 1.
+//   e = 1..l   read row i = e:  P = (pm_i | px_i) gi_{i+1}, gamma_i, A = a_{i+1}/gi_{i+1}, C = g_{i+1} d_i/gi_{i+1},
+//              G = gamma_{i+1} g_{i+2}/g_{i+1};  on the last row gi_{l+1} := 1, A := C := 0, G := 1, meta LAST, so
+//              that the step leaves J = M_l + I_l, the summand of Eq.4.
+//   e = l+1    flush entry, all zero: gives the .y half (one entry behind) its step for row l and zeroes J.
+// Constants are formed in double from the 10^(-q/10) table and rounded once to the working type
+// ("q32"/"q64" tables; Listing 2 :293-295 for which qualities enter which transition).
+#pragma once
+#include "phmm_common.cuh"
+#include "phmm_kernels.h"
+
+namespace phmm {
+
+struct RowC { double gam, A, C, G, pm, px; uint32_t meta; };
+
+__device__ __forceinline__ RowC row_constants(const DevBatch& b, const double* __restrict__ lut, int64_t off, int l, int e) {
+    RowC c = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0u};
+    if (e == 0) {
+        c.gam = 1.0; c.C = 1.0 - lut[b.qual_gcp[off]]; c.meta = META_FIRST;
+    } else if (e >= 1 && e <= l) {
+        const int i = e;  // read row, 1-based
+        const double eps = lut[b.qual_base[off + i - 1]];
+        const int code = base_code(b.read_bases[off + i - 1]);
+        c.meta = (uint32_t)(code & 3) | (i == l ? META_LAST : 0u);
+        c.gam = lut[b.qual_gcp[off + i - 1]];
+        double gin = 1.0;  // gi_{i+1} = g_{i+2} iota_{i+1};  := 1 behind the last row
+        if (i < l) {
+            const double g1 = 1.0 - lut[b.qual_gcp[off + i]];                              // g_{i+1}
+            const double g2 = (i + 1 < l) ? 1.0 - lut[b.qual_gcp[off + i + 1]] : 1.0;      // g_{i+2}, := 1 behind the last row
+            const double io1 = lut[b.qual_ins[off + i]], de1 = lut[b.qual_del[off + i]];   // iota_{i+1}, d_{i+1}
+            gin = g2 * io1;
+            c.A = (1.0 - io1 - de1) / gin;
+            c.C = g1 * lut[b.qual_del[off + i - 1]] / gin;
+            c.G = lut[b.qual_gcp[off + i]] * g2 / g1;
+        } else {
+            c.G = 1.0;
+        }
+        c.pm = (code < 4 ? 1.0 - eps : eps / 3.0) * gin;  // a non-ACGT read base matches nothing (reading G17)
+        c.px = eps / 3.0 * gin;
+    }
+    return c;
+}
+
+}  // namespace phmm

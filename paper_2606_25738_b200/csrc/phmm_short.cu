@@ -5,8 +5,12 @@
 // row), a9 (final reduction, log10), a10 (underflow detection -> rescue queue).
 #include "phmm_engine.cuh"
 #include "phmm_kernels.h"
+#include "phmm_rowconst.cuh"
 #include <type_traits>
 
+#ifndef SHORT_PREFETCH
+#define SHORT_PREFETCH 0  // measured: the L1 prefetch costs more issue slots than it saves (2.50 vs 2.70 TCUPS)
+#endif
 #ifndef SHORT_MIN_CTAS
 #define SHORT_MIN_CTAS 4  // resident CTAs per SM the register allocation is held to (4 x 128 threads -> <= 128 registers)
 #endif
@@ -14,14 +18,6 @@
 namespace phmm {
 
 // ------------------------------------------------------------------ a1: row-constant table
-// Stream of entries of one read of length l ("run", l + TABLE_EXTRA_ROWS entries), see phmm_engine.cuh:
-//   e = 0      run-in entry: P = 0 (U = 0), gamma := 1, C := g_1, G := 0, meta FIRST.  The group's first lane
-//              injects s = C/k, which the chain carries unchanged through every column, so the step leaves
-//              T = g_1 C/k (= T_DM_1 D_{0,j-1}, Eq.1-2 under reading G1) and J = 0: the state in front of row 1.
-//   e = 1..l   read row i = e:  P = (pm_i | px_i) gi_{i+1}, gamma_i, A = a_{i+1}/gi_{i+1}, C = g_{i+1} d_i/gi_{i+1},
-//              G = gamma_{i+1} g_{i+2}/g_{i+1};  on the last row gi_{l+1} := 1, A := C := 0, G := 1, meta LAST, so
-//              that the step leaves J = M_l + I_l, the summand of Eq.4.
-//   e = l+1    flush entry, all zero: gives the .y half (one entry behind) its step for row l and zeroes J.
 // Each 64-byte table entry holds the constants of entry e (for the .x half) and of entry e-1 (for .y; zero
 // for e = 0), already paired the way FFMA2 wants them:
 //   float4 0: gamma.x gamma.y A.x A.y | 1: C.x C.y G.x G.y | 2: pm.x px.x pm.y px.y | 3: meta.x meta.y 0 0
@@ -36,36 +32,6 @@ namespace phmm {
 constexpr int TABLE_CHUNK_STRIDE = 32;  // float4 units between the chunk planes of a block
 __host__ __device__ __forceinline__ int64_t table_slot(int64_t pos) {  // float4 index of chunk 0 of entry pos
     return (pos >> 5) * 128 + (pos & 1) * 16 + ((pos >> 1) & 15);
-}
-
-struct RowC { double gam, A, C, G, pm, px; uint32_t meta; };
-
-__device__ __forceinline__ RowC row_constants(const DevBatch& b, const double* __restrict__ lut, int64_t off, int l, int e) {
-    RowC c = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0u};
-    if (e == 0) {
-        c.gam = 1.0; c.C = 1.0 - lut[b.qual_gcp[off]]; c.meta = META_FIRST;
-    } else if (e >= 1 && e <= l) {
-        const int i = e;  // read row, 1-based
-        const double eps = lut[b.qual_base[off + i - 1]];
-        const int code = base_code(b.read_bases[off + i - 1]);
-        c.meta = (uint32_t)(code & 3) | (i == l ? META_LAST : 0u);
-        c.gam = lut[b.qual_gcp[off + i - 1]];
-        double gin = 1.0;  // gi_{i+1} = g_{i+2} iota_{i+1};  := 1 behind the last row
-        if (i < l) {
-            const double g1 = 1.0 - lut[b.qual_gcp[off + i]];                              // g_{i+1}
-            const double g2 = (i + 1 < l) ? 1.0 - lut[b.qual_gcp[off + i + 1]] : 1.0;      // g_{i+2}, := 1 behind the last row
-            const double io1 = lut[b.qual_ins[off + i]], de1 = lut[b.qual_del[off + i]];   // iota_{i+1}, d_{i+1}
-            gin = g2 * io1;
-            c.A = (1.0 - io1 - de1) / gin;
-            c.C = g1 * lut[b.qual_del[off + i - 1]] / gin;
-            c.G = lut[b.qual_gcp[off + i]] * g2 / g1;
-        } else {
-            c.G = 1.0;
-        }
-        c.pm = (code < 4 ? 1.0 - eps : eps / 3.0) * gin;  // a non-ACGT read base matches nothing (reading G17)
-        c.px = eps / 3.0 * gin;
-    }
-    return c;
 }
 
 __global__ void __launch_bounds__(256) k_table_f32(DevBatch b, const double* __restrict__ lut, float* __restrict__ table) {
@@ -107,6 +73,8 @@ struct Cursor {
     int npos, nend;      // the run after it: the next read of the task, or the zero run
     int q;               // reads of the task already handed to (npos, nend)
 };
+
+__device__ __forceinline__ void prefetch_l1(const void* p) { asm volatile("prefetch.global.L1 [%0];" ::"l"(p)); }
 
 struct RawEntry { float4 a, b, c; uint2 m; };
 
@@ -177,6 +145,11 @@ __global__ void __launch_bounds__(SHORT_WARPS_PER_CTA * 32, SHORT_MIN_CTAS) k_sh
     auto fetch = [&](RawEntry& r) {
         if (c.pos == c.end) { c.pos = c.npos; c.end = c.nend; load_next(); }
         const float4* e = tab + table_slot(c.pos);
+#if SHORT_PREFETCH
+        // the group's first lane is the only one that touches new lines: have it pull one line of the NEXT
+        // 2 KB block into L1 per step (16 lines per block, each requested twice in 32 steps)
+        if (is_first) prefetch_l1(tab + ((int64_t)(c.pos >> 5) + 1) * 128 + (c.pos & 15) * 8);
+#endif
         c.pos++;
         r.a = __ldg(e);
         r.b = __ldg(e + TABLE_CHUNK_STRIDE);
