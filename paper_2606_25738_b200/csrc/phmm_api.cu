@@ -56,6 +56,7 @@ struct phmm_ctx {
     bool upload_pending = false;
     DevBuf d_lut, d_read_off, d_hap_off, d_pair_read, d_pair_hap, d_table, d_tasks, d_warp_first, d_srt_read, d_srt_out;
     DevBuf d_counters, d_rescue, d_items, d_boundary, d_progress, d_scratch;
+    DevBuf d_rq, d_rq_queue, d_rq_sorted, d_rq_plan, d_rq_enq;  // fp64 sub-warp recomputation: counters, queue, ordered queue, plan, FP64-mode input list
     DevBuf d_payload, d_out, d_flags;  // phmm_forward_batch_host only
     PinBuf h_stage;
     std::vector<uint8_t> is_short;
@@ -126,7 +127,8 @@ extern "C" int phmm_destroy(phmm_ctx* ctx) {
     cudaDeviceSynchronize();
     DevBuf* bufs[] = {&ctx->d_lut, &ctx->d_read_off, &ctx->d_hap_off, &ctx->d_pair_read, &ctx->d_pair_hap, &ctx->d_table,
                       &ctx->d_tasks, &ctx->d_warp_first, &ctx->d_srt_read, &ctx->d_srt_out, &ctx->d_counters, &ctx->d_rescue,
-                      &ctx->d_items, &ctx->d_boundary, &ctx->d_progress, &ctx->d_scratch, &ctx->d_payload, &ctx->d_out, &ctx->d_flags};
+                      &ctx->d_items, &ctx->d_boundary, &ctx->d_progress, &ctx->d_scratch, &ctx->d_payload, &ctx->d_out, &ctx->d_flags,
+                      &ctx->d_rq, &ctx->d_rq_queue, &ctx->d_rq_sorted, &ctx->d_rq_plan, &ctx->d_rq_enq};
     for (DevBuf* b : bufs) b->release();
     ctx->h_stage.release();
     if (ctx->ev_upload) cudaEventDestroy(ctx->ev_upload);
@@ -141,8 +143,10 @@ extern "C" int phmm_get_stats(phmm_ctx* ctx, phmm_stats* out) {
     if (ctx->d_counters.p && ctx->stats.n_pairs > 0) {  // rescue count lives on the device until the caller has synchronised
         int n = 0;
         cudaSetDevice(ctx->device);
-        if (cudaMemcpy(&n, ctx->d_counters.p, sizeof(int), cudaMemcpyDeviceToHost) == cudaSuccess && ctx->stats.n_short_warps > 0)
-            ctx->stats.n_rescued = n;
+        int rq[48];
+        if (cudaMemcpy(&n, ctx->d_counters.p, sizeof(int), cudaMemcpyDeviceToHost) == cudaSuccess && ctx->d_rq.p &&
+            cudaMemcpy(rq, ctx->d_rq.p, sizeof(rq), cudaMemcpyDeviceToHost) == cudaSuccess && ctx->stats.n_short_warps > 0)
+            ctx->stats.n_rescued = (int64_t)n + rq[34] - rq[40];  // chain-kernel queue + sub-warp queue - passed on from one to the other
     }
     if (ctx->opt.profile_events) {
         double* dst[4] = {&ctx->stats.ms_table, &ctx->stats.ms_short, &ctx->stats.ms_rescue, &ctx->stats.ms_long};
@@ -202,7 +206,7 @@ extern "C" int phmm_forward_batch(phmm_ctx* ctx, const phmm_batch* b, int precis
     // ---- classify: short (sub-warp systolic fp32 kernel) / chain-sequential (one warp per pair) / chain-strips
     const int strip_cols = chain_strip_cols(fp64);
     ctx->is_short.assign((size_t)np, 0);
-    std::vector<int> seq_pairs, strip_pairs;  // chain kernel work lists (caller pair indices)
+    std::vector<int> seq_pairs, strip_pairs, sub_pairs;  // chain kernel work lists, fp64 sub-warp list (caller pair indices)
     int64_t cells = 0, long_cells = 0;
     int max_seq_l = 0;
     for (int64_t p = 0; p < np; p++) {
@@ -211,6 +215,7 @@ extern "C" int phmm_forward_batch(phmm_ctx* ctx, const phmm_batch* b, int precis
         cells += l * k;
         const bool is_long = k > ctx->opt.long_min_hap_len || l > 4096;
         if (is_long) { strip_pairs.push_back((int)p); long_cells += l * k; }
+        else if (fp64 && k <= RESCUE_MAX_K && l <= RESCUE_MAX_L) { sub_pairs.push_back((int)p); if (l > max_seq_l) max_seq_l = (int)l; }
         else if (fp64) { seq_pairs.push_back((int)p); if (l > max_seq_l) max_seq_l = (int)l; }
         else { ctx->is_short[(size_t)p] = 1; if (l > max_seq_l) max_seq_l = (int)l; }
     }
@@ -247,7 +252,7 @@ extern "C" int phmm_forward_batch(phmm_ctx* ctx, const phmm_batch* b, int precis
     const size_t n_seq = fp64 ? seq_pairs.size() : 0;
     size_t stage_bytes = 4096 + (size_t)(b->n_reads + 1) * 8 + (size_t)(b->n_haps + 1) * 8 + (size_t)np * 8 +
                          pl.tasks.size() * sizeof(ShortTask) + pl.warp_first.size() * 4 + pl.srt_read.size() * 16 +
-                         items.size() * sizeof(ChainItem) + n_seq * 4 + 16 * 256;
+                         items.size() * sizeof(ChainItem) + n_seq * 4 + sub_pairs.size() * 4 + 20 * 256;
     CK(ctx->h_stage.need(stage_bytes));
     Stager sg{ctx, st};
     RC(sg.upload(ctx->d_read_off, b->h_read_off, (size_t)(b->n_reads + 1) * 8));
@@ -271,6 +276,12 @@ extern "C" int phmm_forward_batch(phmm_ctx* ctx, const phmm_batch* b, int precis
         sg.used = at + n_seq * 4;
         CK(cudaMemcpyAsync(ctx->d_rescue.p, (char*)ctx->h_stage.p + at, n_seq * 4, cudaMemcpyHostToDevice, st));
     }
+    RC(sg.upload(ctx->d_rq_enq, sub_pairs.data(), sub_pairs.size() * 4));
+    CK(ctx->d_rq.need(48 * 4));
+    CK(ctx->d_rq_plan.need(68 * 4));
+    CK(ctx->d_rq_queue.need((size_t)np * 16 + 16));
+    CK(ctx->d_rq_sorted.need((size_t)np * 4 + 4));
+    CK(cudaMemsetAsync(ctx->d_rq.p, 0, 48 * 4, st));
     CK(cudaEventRecord(ctx->ev_upload, st));
     ctx->upload_pending = true;
 
@@ -303,6 +314,9 @@ extern "C" int phmm_forward_batch(phmm_ctx* ctx, const phmm_batch* b, int precis
         sl.out = d_out;
         sl.flags = d_flags;
         sl.rescue_thr = (float)ldexp(1.0, ctx->opt.rescue_log2_threshold);
+        sl.rescue.queue = (int4*)ctx->d_rq_queue.p;
+        sl.rescue.cnt = (int*)ctx->d_rq.p;
+        sl.rescue.n_queue = (int*)ctx->d_rq.p + 34;
         sl.rescue_count = counters + 0;
         sl.rescue_list = (int*)ctx->d_rescue.p;
         PROF(1, 0);
@@ -310,8 +324,34 @@ extern "C" int phmm_forward_batch(phmm_ctx* ctx, const phmm_batch* b, int precis
         PROF(1, 1);
         launches += 2;
     }
-    // sequential chain launch: fp32 mode = rescue list (device-side count), fp64 mode = all non-long pairs
-    if (n_warps > 0 || n_seq > 0) {
+    // fp64 sub-warp kernel: fp32 mode = what the short kernel queued, fp64 mode = the short pairs it can hold
+    const bool sub = n_warps > 0 || !sub_pairs.empty();
+    if (sub) {
+        RescueLaunch rl;
+        memset(&rl, 0, sizeof(rl));
+        rl.queue.queue = (int4*)ctx->d_rq_queue.p;
+        rl.queue.cnt = (int*)ctx->d_rq.p;
+        rl.queue.n_queue = (int*)ctx->d_rq.p + 34;
+        rl.max_queue = (int)(fp64 ? (int64_t)sub_pairs.size() : ctx->stats.n_short_pairs);
+        rl.enqueue_pairs = fp64 ? (const int*)ctx->d_rq_enq.p : nullptr;
+        rl.n_enqueue = fp64 ? (int)sub_pairs.size() : 0;
+        rl.plan = (int*)ctx->d_rq_plan.p;
+        rl.sorted = (int*)ctx->d_rq_sorted.p;
+        rl.pair_read = (const int*)ctx->d_pair_read.p;
+        rl.pair_hap = (const int*)ctx->d_pair_hap.p;
+        rl.lut = (const double*)ctx->d_lut.p;
+        rl.out = d_out;
+        rl.flags = d_flags;
+        rl.flag_bits = fp64 ? 0 : PHMM_FLAG_RESCUED;
+        rl.fallback_count = counters + (fp64 ? 4 : 0);
+        rl.fallback_list = (int*)ctx->d_rescue.p;
+        PROF(2, 0);
+        CK(launch_rescue_f64(db, rl, st));
+        launches += 3 + (fp64 ? 1 : 0);
+    }
+    // sequential chain launch: fp32 mode = rescue list (device-side count), fp64 mode = the other non-long pairs;
+    // both also receive what the sub-warp kernel passed on
+    if (n_warps > 0 || n_seq > 0 || sub) {
         const int grid = ctx->chain_grid[1];
         const int64_t blocks = (max_seq_l + TABLE_EXTRA_ROWS + 31) / 32 + 1;
         const int max_strips_seq = (ctx->opt.long_min_hap_len + chain_strip_cols(true) - 1) / chain_strip_cols(true);
@@ -332,7 +372,7 @@ extern "C" int phmm_forward_batch(phmm_ctx* ctx, const phmm_batch* b, int precis
         cl.flags = d_flags;
         cl.flag_bits = fp64 ? 0 : PHMM_FLAG_RESCUED;
         cl.log2C = 0;
-        PROF(2, 0);
+        if (!sub) PROF(2, 0);
         CK(launch_chain(db, cl, true, true, grid, st));
         PROF(2, 1);
         launches++;

@@ -57,12 +57,12 @@ template <typename T> struct Entry2 {
 template <typename T, int NV> struct Lane2 {
     typedef W2<T> P;
     typedef typename P::V V;
-    static constexpr int NW = (NV + 7) / 8;  // 32-bit words of one-hot nibbles per half (8 columns per word)
+    static_assert(NV <= 16, "one 32-bit match word per base: 16 columns per half");
 
     V Tt[NV], J[NV];
     V outT, outS;              // what dropped out on the right in the last step: (.x's, .y's)
     T sigX, sigY;              // Eq.4 partial sums (columns <= this half's last) of the read finished last
-    uint32_t hx[NW], hy[NW];   // haplotype columns as one-hot nibbles: bit 4*(x%8)+b of word x/8 <=> column x has base b
+    uint32_t hm[4];            // match words, one per base b: bit x <=> .x column x is b, bit 16+x <=> .y column x is b
     int nvx, nvy;              // number of real (j <= k) columns in each half
 
     __device__ __forceinline__ void init() {
@@ -75,18 +75,20 @@ template <typename T, int NV> struct Lane2 {
     // hap: pointer to the haplotype bytes, k its length, j0 = 0-based first column of this thread
     __device__ __forceinline__ void load_hap(const uint8_t* __restrict__ hap, int k, int j0) {
 #pragma unroll
-        for (int w = 0; w < NW; w++) { hx[w] = 0; hy[w] = 0; }
+        for (int c = 0; c < 4; c++) hm[c] = 0;
         nvx = min(max(k - j0, 0), NV);
         nvy = min(max(k - j0 - NV, 0), NV);
 #pragma unroll
         for (int x = 0; x < NV; x++) {
             if (x < nvx) {
                 const int c = base_code(hap[j0 + x]);
-                if (c < 4) hx[x >> 3] |= 1u << (4 * (x & 7) + c);
+#pragma unroll
+                for (int q = 0; q < 4; q++) hm[q] |= (c == q ? 1u : 0u) << x;
             }
             if (x < nvy) {
                 const int c = base_code(hap[j0 + NV + x]);
-                if (c < 4) hy[x >> 3] |= 1u << (4 * (x & 7) + c);
+#pragma unroll
+                for (int q = 0; q < 4; q++) hm[q] |= (c == q ? 1u : 0u) << (16 + x);
             }
         }
     }
@@ -97,13 +99,14 @@ template <typename T, int NV> struct Lane2 {
     __device__ __forceinline__ void step(const Entry2<T>& E, T inS, T inT, T inSig) {
         V s = P::mk(inS, outS.x);                  // .y continues the row .x finished one step ago
         const V tgrab = P::mk(inT, outT.x);        // T[0] of the NEXT step
-        uint32_t rx[NW], ry[NW];
-        const uint32_t shx = E.metaX & META_CODE_MASK, shy = E.metaY & META_CODE_MASK;
-#pragma unroll
-        for (int w = 0; w < NW; w++) { rx[w] = hx[w] >> shx; ry[w] = hy[w] >> shy; }
+        // match word of this step: the read base of .x's row picks the low half, that of .y's row the high half;
+        // consecutive single-bit tests of one register let ptxas turn 7 of them into one R2P
+        const uint32_t wx01 = (E.metaX & 1u) ? hm[1] : hm[0], wx23 = (E.metaX & 1u) ? hm[3] : hm[2];
+        const uint32_t wy01 = (E.metaY & 1u) ? hm[1] : hm[0], wy23 = (E.metaY & 1u) ? hm[3] : hm[2];
+        const uint32_t wx = (E.metaX & 2u) ? wx23 : wx01, wy = (E.metaY & 2u) ? wy23 : wy01;
+        const uint32_t mw = (wx & 0xffffu) | (wy & 0xffff0000u);
         auto prior = [&](int x) {                  // Eq.3: one select per half
-            const uint32_t bit = 1u << (4 * (x & 7));
-            return P::mk((rx[x >> 3] & bit) ? E.pmx : E.pxx, (ry[x >> 3] & bit) ? E.pmy : E.pxy);
+            return P::mk((mw & (1u << x)) ? E.pmx : E.pxx, (mw & (1u << (16 + x))) ? E.pmy : E.pxy);
         };
         V U = P::mul(prior(0), Tt[0]);
         Tt[0] = tgrab;

@@ -21,6 +21,26 @@ struct DevBatch {  // device mirrors of the batch
     int64_t n_reads, n_haps;
 };
 
+// ---- fp64 recomputation of short pairs (phmm_rescue.cu)
+constexpr int RESCUE_NV = 16;                   // columns per lane
+constexpr int RESCUE_MAX_K = 32 * RESCUE_NV;    // 512: widest haplotype one warp covers in fp64
+constexpr int RESCUE_MAX_L = 512;               // longest read unrescaled fp64 is trusted with (3.3 bits lost per unrelated row)
+
+struct RescueQueue {
+    int4* queue;      // (pair, lane-group size g, ticket within bucket g, -)
+    int* n_queue;     // items in queue
+    int* cnt;         // 48 ints, zeroed per call: [0..32] items per bucket g, [33] warp ticket of k_rescue_f64, [34] = *n_queue,
+                      // [40] pairs passed on to the chain kernel
+};
+#ifdef __CUDACC__
+__device__ __forceinline__ void rescue_push(const RescueQueue& rq, int pair, int k) {
+    const int g = (k + RESCUE_NV - 1) / RESCUE_NV;
+    const int n = atomicAdd(rq.cnt + g, 1);
+    const int i = atomicAdd(rq.n_queue, 1);
+    rq.queue[i] = make_int4(pair, g, n, 0);
+}
+#endif
+
 struct ShortTask {  // one lane group's work: several reads streamed against one haplotype
     int hap, pair_first, n_pairs, rows;  // rows = sum of the read lengths (reset rows not counted)
 };
@@ -35,8 +55,9 @@ struct ShortLaunch {
     double* out;
     uint8_t* flags;
     float rescue_thr;          // scaled sums below this (or non-finite) are queued for fp64
-    int* rescue_count;         // device counter
-    int* rescue_list;          // caller pair indices
+    RescueQueue rescue;        // underflowed pairs with k <= RESCUE_MAX_K and l <= RESCUE_MAX_L: sub-warp fp64 kernel
+    int* rescue_count;         // the others: device counter and
+    int* rescue_list;          // caller pair indices for the rescaled chain kernel
 };
 
 struct ChainItem {  // one strip (32 lanes x 2NV columns) of one pair, run concurrently with its neighbours
@@ -63,6 +84,24 @@ struct ChainLaunch {
     uint8_t flag_bits;         // written to flags[pair]
     int log2C;                 // scale constant C = 2^log2C of Eq.1 (0 for the rescaled kernels)
 };
+
+struct RescueLaunch {
+    RescueQueue queue;
+    int max_queue;             // upper bound of the queue length (grid of the scatter kernel)
+    const int* enqueue_pairs;  // PHMM_FP64 mode: device list of pairs to queue first (else nullptr)
+    int n_enqueue;
+    int* plan;                 // 68 ints of scratch
+    int* sorted;               // max_queue ints of scratch
+    const int* pair_read;
+    const int* pair_hap;
+    const double* lut;
+    double* out;
+    uint8_t* flags;
+    uint8_t flag_bits;
+    int* fallback_count;       // pairs the unrescaled fp64 pass could not represent: queued for the chain kernel
+    int* fallback_list;
+};
+cudaError_t launch_rescue_f64(const DevBatch& b, const RescueLaunch& r, cudaStream_t st);
 
 cudaError_t launch_lut_table(const DevBatch& b, const double* lut, float* table, cudaStream_t st);
 cudaError_t launch_short_f32(const DevBatch& b, const ShortLaunch& p, cudaStream_t st);

@@ -1,0 +1,225 @@
+// fp64 recomputation of short pairs (PHMM_FP64 mode for short pairs):
+// device-side binning of the pairs by lane-group size, then a sub-warp systolic kernel in double.
+//
+// One thread = ONE virtual lane of RESCUE_NV haplotype columns (fp64 has no packed form, so nothing is
+// gained by two halves per thread); lane L of a group runs one stream entry (read row) behind lane L-1.
+// A group works on one pair; a warp holds floor(32/g) groups of the same size g = ceil(k / RESCUE_NV).
+// Which pairs land here is only known on the device (the fp32 kernel's underflow test), so the queue is
+// binned there: the producer takes a ticket in its size bucket, k_rescue_plan turns the 33 bucket counts
+// into warp and list offsets, k_rescue_scatter orders the queue by bucket, and the persistent kernel
+// k_rescue_f64 hands out whole warps by ticket.
+//
+// Arithmetic: the plain (unscaled-I) row-wise form of Eq.6-7 with the row constants formed on the fly
+// from the quality bytes -- no division, no table:
+//     M      = p_{i,x} * T[x]                                 (Eq.3 select)            MUL
+//     s'     = gamma_i * s + M                                S_{i,x}, the serial chain  FMA
+//     T[x+1] = a_{i+1} M + g_{i+1} I[x] + c_{i+1} s           c_{i+1} = g_{i+1} d_i     MUL + 2 FMA
+//     I[x]   = iota_{i+1} M + gamma_{i+1} I[x]                                           MUL + FMA
+// = 7 DP instructions per cell.  Entry 0 is the run-in row (p = 0, gamma_0 := 1, d_0 := 1; the first
+// lane injects s = C/k: Eq.1 under reading G1); behind the last row a' = g' = c' := 0 and iota' =
+// gamma' := 1, which leaves I[x] = M_l + I_l, the summand of Eq.4.  Scale constant C = 2^1000
+// (PAPER.md:61 uses 2^1020; 20 bits of head room because with per-base qualities L is bounded by a
+// small constant, not by 1: SURVEY 8(c) item 3).  A result that is still not a normal finite number
+// goes on to the rescaled chain kernel.
+#include "phmm_common.cuh"
+#include "phmm_kernels.h"
+
+namespace phmm {
+
+constexpr int RESCUE_WARPS = 4;
+constexpr int RESCUE_LOG2C = 1000;
+
+// ---- binning
+// counters layout (ints): [0..32] bucket counts (index g), [33] ticket of k_rescue_f64
+// plan layout (ints): [0..33] first warp of bucket g (exclusive prefix; [33] = total warps), [34..67] first list slot of bucket g
+__global__ void k_rescue_plan(const int* __restrict__ cnt, int* __restrict__ plan) {
+    if (threadIdx.x != 0) return;
+    int w = 0, o = 0;
+    for (int g = 0; g <= 32; g++) {
+        plan[g] = w; plan[34 + g] = o;
+        const int c = cnt[g];
+        if (g >= 1) w += (c + (32 / g) - 1) / (32 / g);
+        o += c;
+    }
+    plan[33] = w; plan[34 + 33] = o;
+}
+
+__global__ void k_rescue_scatter(const int4* __restrict__ queue, const int* __restrict__ n_queue, const int* __restrict__ plan,
+                                 int* __restrict__ sorted) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= *n_queue) return;
+    const int4 q = queue[i];  // pair, g, ticket within the bucket
+    sorted[plan[34 + q.y] + q.z] = q.x;
+}
+
+// PHMM_FP64 mode: every short pair is queued (no fp32 pass ran)
+__global__ void k_rescue_enqueue(DevBatch b, RescueQueue rq, const int* __restrict__ pairs, int n, const int* __restrict__ pair_hap) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const int pair = pairs[i];
+    const int h = pair_hap[pair];
+    const int k = (int)(b.hap_off[h + 1] - b.hap_off[h]);
+    rescue_push(rq, pair, k);
+}
+
+// ---- the kernel
+struct RescueArgs {
+    const int* sorted;       // pairs ordered by bucket
+    const int* cnt;          // [0..32] bucket counts
+    const int* plan;         // see k_rescue_plan
+    int* ticket;
+    const int* pair_read;
+    const int* pair_hap;
+    const double* lut;       // 256 entries 10^(-q/10)
+    double* out;
+    uint8_t* flags;
+    uint8_t flag_bits;
+    int* fallback_count;     // results that are not normal finite numbers: queue for the rescaled chain kernel
+    int* fallback_list;
+    int* fallback_stat;      // number of such pairs (statistics only)
+};
+
+__global__ void __launch_bounds__(RESCUE_WARPS * 32, 3) k_rescue_f64(DevBatch b, RescueArgs p) {
+    constexpr int NV = RESCUE_NV;
+    __shared__ double s_lut[256];
+    __shared__ int s_plan[68];
+    for (int i = threadIdx.x; i < 256; i += blockDim.x) s_lut[i] = p.lut[i];
+    for (int i = threadIdx.x; i < 68; i += blockDim.x) s_plan[i] = p.plan[i];
+    __syncthreads();
+    const int lane = threadIdx.x & 31;
+    const int total_warps = s_plan[33];
+    const double LOG10_2 = 0.30102999566398119521;
+
+    for (;;) {
+        int w = 0;
+        if (lane == 0) w = atomicAdd(p.ticket, 1);
+        w = __shfl_sync(PHMM_FULL, w, 0);
+        if (w >= total_warps) break;
+        int g = 1;
+        while (g < 32 && w >= s_plan[g + 1]) g++;    // bucket of this warp (33 entries, warp-uniform)
+        const int per = 32 / g;                       // pairs per warp
+        const int grp = lane / g, lg = lane - grp * g;
+        const int slot = (w - s_plan[g]) * per + grp;  // index within the bucket
+        const bool active = grp < per && slot < p.cnt[g];
+        int pair = -1, l = 0, k = 1;
+        int64_t ro = 0, ho = 0;
+        if (active) {
+            pair = p.sorted[s_plan[34 + g] + slot];
+            const int r = p.pair_read[pair], h = p.pair_hap[pair];
+            ro = b.read_off[r]; ho = b.hap_off[h];
+            l = (int)(b.read_off[r + 1] - ro); k = (int)(b.hap_off[h + 1] - ho);
+        }
+        int steps = active ? l + g : 0;  // entries 0..l, lane lg one entry behind lane lg-1
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) steps = max(steps, __shfl_xor_sync(PHMM_FULL, steps, o));
+
+        // ---- haplotype columns of this lane: one match word per base (bit x <=> column x carries that base)
+        const int j0 = lg * NV;
+        const int nv = active ? min(max(k - j0, 0), NV) : 0;
+        uint32_t hm[4] = {0u, 0u, 0u, 0u};
+        for (int x = 0; x < nv; x++) {
+            const int c = base_code(b.hap_bases[ho + j0 + x]);
+#pragma unroll
+            for (int q = 0; q < 4; q++) hm[q] |= (c == q ? 1u : 0u) << x;
+        }
+        const double Cok = ldexp(1.0, RESCUE_LOG2C) / (double)k;
+
+        double T[NV], I[NV];
+#pragma unroll
+        for (int x = 0; x < NV; x++) { T[x] = 0.0; I[x] = 0.0; }
+        double outS = 0.0, outT = 0.0, sig = 0.0;
+        double gam_own = 1.0, d_own = 1.0;  // gamma_i and d_i of the entry about to be processed (entry 0: both := 1)
+
+        for (int s = 0; s < steps; s++) {
+            const int e = s - lg;  // stream entry = read row (0 = run-in)
+            const bool on = active && e >= 0 && e <= l;
+            // ---- a1: row constants on the fly
+            double pm = 0.0, px = 0.0, gam = 0.0, an = 0.0, gn = 0.0, cn = 0.0, in_ = 0.0, gan = 0.0;
+            uint32_t mw = 0u;
+            if (on) {
+                gam = gam_own;
+                if (e >= 1) {
+                    const double eps = s_lut[b.qual_base[ro + e - 1]];
+                    const int code = base_code(b.read_bases[ro + e - 1]);
+                    px = eps / 3.0;
+                    pm = code < 4 ? 1.0 - eps : px;  // a non-ACGT read base matches nothing (reading G17)
+                    const uint32_t m01 = (code & 1) ? hm[1] : hm[0], m23 = (code & 1) ? hm[3] : hm[2];
+                    mw = (code & 2) ? m23 : m01;
+                }
+                if (e < l) {
+                    const double io1 = s_lut[b.qual_ins[ro + e]], de1 = s_lut[b.qual_del[ro + e]], ga1 = s_lut[b.qual_gcp[ro + e]];
+                    an = 1.0 - io1 - de1; gn = 1.0 - ga1; cn = gn * d_own; in_ = io1; gan = ga1;
+                    gam_own = ga1; d_own = de1;
+                } else {
+                    in_ = 1.0; gan = 1.0;  // behind the last row: I[x] <- M_l + I_l (Eq.4 summand)
+                }
+            }
+            // ---- left boundary
+            double inS = __shfl_up_sync(PHMM_FULL, outS, 1), inT = __shfl_up_sync(PHMM_FULL, outT, 1);
+            double inSig = __shfl_up_sync(PHMM_FULL, sig, 1);
+            if (lg == 0) {  // column-0 boundary, Eq.1: only the run-in entry injects
+                inS = (on && e == 0) ? Cok : 0.0;
+                inT = cn * inS;
+                inSig = 0.0;
+            }
+            double sr = inS;
+            double M = ((mw & 1u) ? pm : px) * T[0];
+            T[0] = inT;
+#pragma unroll
+            for (int x = 0; x < NV; x++) {
+                double Mn = M;
+                if (x + 1 < NV) Mn = ((mw & (1u << (x + 1))) ? pm : px) * T[x + 1];
+                const double t2 = fma(gn, I[x], an * M);
+                const double Tn = fma(cn, sr, t2);
+                I[x] = fma(gan, I[x], in_ * M);
+                sr = fma(gam, sr, M);
+                if (x + 1 < NV) T[x + 1] = Tn; else outT = Tn;
+                M = Mn;
+            }
+            outS = sr;
+            if (on && e == l) {  // Eq.4
+                double a = 0.0;
+#pragma unroll
+                for (int x = 0; x < NV; x++) a += (x < nv) ? I[x] : 0.0;
+                sig = inSig + a;
+                if (lg == g - 1) {
+                    const double v = log10(sig) - (double)RESCUE_LOG2C * LOG10_2;
+                    if (sig >= 1e-290 && sig < 1e300) {
+                        p.out[pair] = v;
+                        if (p.flags) p.flags[pair] = p.flag_bits;
+                    } else {
+                        const int idx = atomicAdd(p.fallback_count, 1);
+                        p.fallback_list[idx] = pair;
+                        atomicAdd(p.fallback_stat, 1);
+                    }
+                }
+            }
+        }
+        __syncwarp();
+    }
+}
+
+static int g_rescue_grid = 0;
+
+cudaError_t launch_rescue_f64(const DevBatch& b, const RescueLaunch& r, cudaStream_t st) {
+    if (g_rescue_grid == 0) {
+        int n = 0, dev = 0, sms = 0;
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, k_rescue_f64, RESCUE_WARPS * 32, 0);
+        cudaGetDevice(&dev);
+        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+        g_rescue_grid = (n > 0 ? n : 1) * (sms > 0 ? sms : 148);
+    }
+    RescueQueue rq = r.queue;
+    if (r.enqueue_pairs && r.n_enqueue > 0)
+        k_rescue_enqueue<<<(r.n_enqueue + 255) / 256, 256, 0, st>>>(b, rq, r.enqueue_pairs, r.n_enqueue, r.pair_hap);
+    k_rescue_plan<<<1, 32, 0, st>>>(rq.cnt, r.plan);
+    if (r.max_queue > 0) k_rescue_scatter<<<(r.max_queue + 255) / 256, 256, 0, st>>>(rq.queue, rq.n_queue, r.plan, r.sorted);
+    RescueArgs a;
+    a.sorted = r.sorted; a.cnt = rq.cnt; a.plan = r.plan; a.ticket = rq.cnt + 33;
+    a.pair_read = r.pair_read; a.pair_hap = r.pair_hap; a.lut = r.lut; a.out = r.out; a.flags = r.flags; a.flag_bits = r.flag_bits;
+    a.fallback_count = r.fallback_count; a.fallback_list = r.fallback_list; a.fallback_stat = rq.cnt + 40;
+    k_rescue_f64<<<g_rescue_grid, RESCUE_WARPS * 32, 0, st>>>(b, a);
+    return cudaGetLastError();
+}
+
+}  // namespace phmm

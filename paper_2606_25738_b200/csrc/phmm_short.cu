@@ -11,6 +11,9 @@
 #ifndef SHORT_PREFETCH
 #define SHORT_PREFETCH 0  // measured: the L1 prefetch costs more issue slots than it saves (2.50 vs 2.70 TCUPS)
 #endif
+#ifndef SHORT_FETCH_AHEAD
+#define SHORT_FETCH_AHEAD 1
+#endif
 #ifndef SHORT_MIN_CTAS
 #define SHORT_MIN_CTAS 4  // resident CTAs per SM the register allocation is held to (4 x 128 threads -> <= 128 registers)
 #endif
@@ -182,12 +185,27 @@ __global__ void __launch_bounds__(SHORT_WARPS_PER_CTA * 32, SHORT_MIN_CTAS) k_sh
             if (isfinite(sg) && sg >= p.rescue_thr) {
                 p.out[pair] = log10((double)sg) - 120.0 * LOG10_2;
                 if (p.flags) p.flags[pair] = 0;
+            } else if (m_k <= RESCUE_MAX_K && __ldg(ent + nout - 1).y - TABLE_EXTRA_ROWS <= RESCUE_MAX_L) {
+                rescue_push(p.rescue, pair, m_k);  // a10: unrescaled fp64 sub-warp kernel
             } else {
-                const int idx = atomicAdd(p.rescue_count, 1);
+                const int idx = atomicAdd(p.rescue_count, 1);  // rescaled fp64 chain kernel
                 p.rescue_list[idx] = pair;
             }
         }
     };
+#if SHORT_FETCH_AHEAD == 2
+    RawEntry eA, eB, eC;  // entries are loaded two steps ahead into three rotating register sets
+    fetch(eA);
+    fetch(eB);
+    for (int s = 0; s < steps; s += 3) {  // up to two extra all-idle steps at the end, which are harmless
+        fetch(eC);
+        one_step(eA);
+        fetch(eA);
+        one_step(eB);
+        fetch(eB);
+        one_step(eC);
+    }
+#else
     RawEntry eA, eB;
     fetch(eA);
     for (int s = 0; s < steps; s += 2) {  // an odd step count runs one extra all-idle step, which is harmless
@@ -196,6 +214,7 @@ __global__ void __launch_bounds__(SHORT_WARPS_PER_CTA * 32, SHORT_MIN_CTAS) k_sh
         fetch(eA);
         one_step(eB);
     }
+#endif
 }
 
 cudaError_t launch_short_f32(const DevBatch& b, const ShortLaunch& p, cudaStream_t st) {
