@@ -14,8 +14,8 @@ value      GCUPS = cells / time / 1e9 (TCUPS x 1000), payload resi
 e2e        same metric through phmm_forward_batch_host: all buffers in pinned HOST memory, the
            host->device copies of the payload and the device->host copy of the results inside the
            timed region ("with transfers").
-roofline   dominant kernel (short: k_short_f32, long: k_chain) against the FP32 (FP64) non-tensor
-           peak; flops = 10 per cell; duration from the library's CUDA events.
+roofline   dominant kernel (short: k_short_f32, long: k_chain, fp64: k_rescue_f64) against the FP32 (FP64)
+           non-tensor peak; flops = 10 per cell; duration from the library's CUDA events.
 cpu_baseline  the oracle (oracle/, as it stands) on the host cores on a bounded sample of the same batch.
 
 Multi-GPU: the path does not shard (BASELINE.json north_star: one GPU).  --gpus N under torchrun
@@ -45,7 +45,8 @@ WORKLOADS = {  # name -> (BASELINE.json config index, description)
     "long": (3, "configs[3] long-read batch: 2000 pairs, reads 5-15 kbp"),
     "verylong": (4, "configs[4] very-long stress: 16 pairs of 100 kbp x 105 kbp"),
 }
-FLOPS_PER_CELL = 10.0  # 4 FMA + 2 MUL per cell of the implemented recurrence
+FLOPS_PER_CELL = 10.0  # SURVEY 8(d)'s algorithmic count (4 FMA + 2 MUL per cell); DESIGN.md section 7
+FLOPS_PER_CELL_EXECUTED = {"fp32": 9.0, "fp64": 11.0}  # what the engines issue: 4 FMA + 1 MUL (fp32 T/J form), 4 FMA + 3 MUL (fp64 sub-warp kernel)
 
 
 def _measured_peaks():
@@ -56,11 +57,15 @@ def _measured_peaks():
         return {}
 
 
-def _profiled_traffic(name):
-    """DRAM bytes per launch of the dominant kernel from the committed ncu capture, or None."""
+def _profiled_traffic(name, workload, scale):
+    """DRAM bytes per launch of the dominant kernel from the committed ncu capture (profiles/traffic.json),
+    scaled linearly from the captured batch size to this run's; None if there is no capture of this workload."""
     try:
         with open(os.path.join(ROOT, "profiles", "traffic.json")) as f:
-            return json.load(f).get(name)
+            e = json.load(f).get(name)
+        if not e or e.get("workload") != workload:
+            return None
+        return float(e["dram_bytes_per_launch"]) * scale / float(e["scale"])
     except Exception:
         return None
 
@@ -291,16 +296,18 @@ def main():
     if st["n_long_pairs"] * 2 > st["n_pairs"]:
         kname, kms, kcells = "k_chain (concurrent strips)", fam["ms_long"], cells * 1.0
     elif args.precision == "fp64":
-        kname, kms, kcells = "k_chain<double> (one warp per pair)", fam["ms_rescue"], cells * 1.0
+        kname, kms, kcells = "k_rescue_f64 (+ chain fallback)", fam["ms_rescue"], cells * 1.0
     else:
         kname, kms, kcells = "k_short_f32", fam["ms_short"], float(st["short_cells"])
     achieved = FLOPS_PER_CELL * kcells / (kms * 1e-3) / 1e12 if kms > 0 else 0.0
     roofline = {"bound": "alu", "kernel": kname, "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
-                "frac": achieved / peak, "traffic": _profiled_traffic(kname.split(" ")[0]),
+                "frac": achieved / peak, "traffic": _profiled_traffic(kname.split(" ")[0].split("<")[0], args.workload, args.scale),
                 "peak_source": "nominal non-tensor %s peak = %d SMs x %d lanes x 2 x %.0f MHz (DESIGN.md); in-run FMA "
                                "microbenchmark measured %.2f TFLOP/s" % (args.precision.upper(), prop.multi_processor_count,
                                                                         lanes, sm_max, meas),
-                "flops_per_cell": FLOPS_PER_CELL, "kernel_ms_per_launch": kms, "kernel_gcups": kcells / (kms * 1e-3) / 1e9 if kms > 0 else 0.0,
+                "flops_per_cell": FLOPS_PER_CELL, "flops_per_cell_executed": FLOPS_PER_CELL_EXECUTED[args.precision],
+                "frac_at_executed_flops": achieved / peak * FLOPS_PER_CELL_EXECUTED[args.precision] / FLOPS_PER_CELL,
+                "kernel_ms_per_launch": kms, "kernel_gcups": kcells / (kms * 1e-3) / 1e9 if kms > 0 else 0.0,
                 "kernel_share_of_step": kms / ms_step if ms_step > 0 else None,
                 "hbm_gbs_achieved": None, "family_ms": fam, "host_batch_ms": host_ms}
 

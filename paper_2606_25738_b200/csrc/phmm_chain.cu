@@ -27,7 +27,9 @@
 
 namespace phmm {
 
-constexpr int CHAIN_WARPS = 4;
+#ifndef CHAIN_MIN_CTAS_F32
+#define CHAIN_MIN_CTAS_F32 3
+#endif
 constexpr int RING = 128;  // row-constant ring per warp (entries); covers 63 entries of skew + two 32-entry blocks
 
 template <typename T> struct Rec {  // boundary block of 32 stream entries, SoA
@@ -127,7 +129,7 @@ template <typename T, int NV> __device__ __forceinline__ void lane_scale(Lane2<T
 }
 
 template <typename T, int NV, int WPC>
-__global__ void __launch_bounds__(WPC * 32, (sizeof(T) == 4 ? 3 : 2))
+__global__ void __launch_bounds__(WPC * 32, (sizeof(T) == 4 ? CHAIN_MIN_CTAS_F32 : 2))
 k_chain(DevBatch b, ChainLaunch p, int items_are_pairs) {
     typedef Lane2<T, NV> L;
     typedef RingFmt<T> RF;
@@ -296,10 +298,13 @@ k_chain(DevBatch b, ChainLaunch p, int items_are_pairs) {
                         lane_scale<T, NV>(ln, -up);
                         ex += up;
                     }
-                    const int d = max(-Fx<T>::CLAMP, min(Fx<T>::CLAMP, exL - ex));  // two factors: |d| may exceed one exponent range
-                    const int h = d / 2;
-                    const T f1 = Fx<T>::exp2i(h), f2 = Fx<T>::exp2i(d - h);
-                    inS = inS * f1 * f2; inT = inT * f1 * f2; inSig = inSig * f1 * f2;
+                    const int d = exL - ex;
+                    if (d >= -Fx<T>::CLAMP1 && d <= Fx<T>::CLAMP1) {  // the usual case: one exact factor
+                        const T f = Fx<T>::exp2i(d);
+                        inS *= f; inT *= f; inSig *= f;
+                    } else {  // |d| beyond one factor's exponent range
+                        inS = scale_pow2<T>(inS, d); inT = scale_pow2<T>(inT, d); inSig = scale_pow2<T>(inSig, d);
+                    }
                 }
                 ln.step(E, inS, inT, inSig);
                 // ---- right boundary of the strip: lane 31's .y half has just finished entry s - 63

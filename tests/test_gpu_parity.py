@@ -188,7 +188,7 @@ def test_edge_lengths(B, ctx):
     lane, 1024 per warp = short/long cut, 1024-column strips), reads longer than haplotypes."""
     rng = np.random.default_rng(21)
     pairs = []
-    for k in (1, 2, 31, 32, 33, 63, 64, 65, 255, 256, 257, 1023, 1024, 1025, 2047, 2048, 2049, 3100):
+    for k in (1, 2, 15, 16, 17, 31, 32, 33, 63, 64, 65, 255, 256, 257, 511, 512, 513, 1023, 1024, 1025, 2047, 2048, 2049, 3100):
         for l in (1, 2, 17, 130):
             hap = _rand_seq(rng, k)
             if l <= k and rng.random() < 0.7:
@@ -201,6 +201,34 @@ def test_edge_lengths(B, ctx):
     b = W.from_strings(pairs)
     check(B, ctx, b, B.PHMM_FP32_RESCUE)
     check(B, ctx, b, B.PHMM_FP64)
+
+
+def test_nonuniform_gcp_and_streams(B, ctx):
+    """Per-base gap-continuation qualities (reading G7) through every kernel: several reads streamed against
+    one haplotype (short kernel), unrelated reads (fp64 sub-warp kernel), a haplotype > 1024 (chain kernel),
+    reads around the fp64 sub-warp kernel's length limit (512)."""
+    rng = np.random.default_rng(24)
+    reads, haps, pr, ph = [], [], [], []
+    for h, k in enumerate((40, 300, 500, 700, 1500)):
+        haps.append(_rand_seq(rng, k))
+        for l in (3, 60, 200, 511, 512, 513, 600):
+            if l + 5 < k and rng.random() < 0.6:
+                s = int(rng.integers(0, k - l))
+                rd = haps[-1][s:s + l]
+            else:
+                rd = _rand_seq(rng, l)
+            reads.append((rd, list(rng.integers(5, 41, l)), list(rng.integers(12, 50, l)), list(rng.integers(12, 50, l)),
+                          list(rng.integers(5, 30, l))))
+            pr.append(len(reads) - 1); ph.append(h)
+    cat = lambda i: np.concatenate([np.asarray(r[i], dtype=np.uint8) if i else np.frombuffer(r[0].encode(), dtype=np.uint8)
+                                    for r in reads])
+    b = W.Batch(np.concatenate([[0], np.cumsum([len(r[0]) for r in reads])]).astype(np.int64),
+                np.concatenate([[0], np.cumsum([len(h) for h in haps])]).astype(np.int64),
+                cat(0), cat(1), cat(2), cat(3), cat(4), np.frombuffer("".join(haps).encode(), dtype=np.uint8),
+                np.asarray(pr, dtype=np.int32), np.asarray(ph, dtype=np.int32))
+    out, fl, ref = check(B, ctx, b, B.PHMM_FP32_RESCUE)
+    check_flags(B, b, fl, ref)
+    check(B, ctx, b, B.PHMM_FP64, ref=ref)
 
 
 def test_read_longer_than_haplotype_and_unrelated(B, ctx):
