@@ -197,7 +197,7 @@ def main():
 
     import torch
     import torch.distributed as dist
-    from paper_2606_25738_b200 import binding
+    from paper_2606_25738_b200 import binding, replicas
 
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device (there is no CPU fallback)")
@@ -206,7 +206,7 @@ def main():
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device(dev))
 
-    batch, cfg = make_batch(args.workload, args.scale, rank)
+    batch, cfg = make_batch(args.workload, args.scale, replicas.rank_seed(0, rank))
     cells, n_pairs = batch.cells(), batch.n_pairs
     prec = binding.PHMM_FP32_RESCUE if args.precision == "fp32" else binding.PHMM_FP64
     ctx = binding.Context(local, profile_events=1)
@@ -245,17 +245,9 @@ def main():
         fam[k] = s[k]
     host_ms = s["host_batch_ms"]
     clocks = sampler.stop() if sampler else None
-    if world > 1:
-        t = torch.tensor([ms], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
-        c = torch.tensor([float(cells), float(n_pairs)], dtype=torch.float64, device=dev)
-        dist.all_reduce(c, op=dist.ReduceOp.SUM)
-        tot_cells, tot_pairs = float(c[0].item()), float(c[1].item())
-    else:
-        tot_cells, tot_pairs = float(cells), float(n_pairs)
+    ms, tot_cells, tot_pairs = replicas.aggregate(ms, cells, n_pairs, dist if world > 1 else None, dev)
     ms_step = ms / args.steps
-    gcups = tot_cells / (ms_step * 1e-3) / 1e9
+    gcups = replicas.whole_job_gcups(ms, tot_cells, args.steps)
 
     # ---- end to end: host (pinned) buffers in, host results out, copies inside the timed region
     e2e = None

@@ -152,6 +152,18 @@ int phmm_last_cuda_error(phmm_ctx* ctx);
  * independent FMA chains, best of `reps` launches, timed with CUDA events. */
 int phmm_measure_peak(int device, int kind, int reps, double* out_tflops);
 
+/* Host batcher only (no device is touched): the work plan the short path
+ * would use for the pairs of `b` with haplotype length <= long_min_hap_len (0 = default 1024) and read
+ * length <= 4096.  Only the host arrays of `b` are read (offsets, pair list).  Outputs, all host, caller-owned:
+ *   plan_counts[4]   = { n_warps, n_tasks, n_sorted_pairs, columns per lane }
+ *   warp_first       n_warps + 1 ints: first task of each warp              (capacity cap_warps + 1)
+ *   tasks            4 ints per task: haplotype, first sorted pair, number of pairs, read rows (capacity 4 * cap_tasks)
+ *   sorted_pair      caller's pair index of each sorted pair                 (capacity cap_pairs)
+ * Any output pointer may be NULL (then only plan_counts is written).  Returns PHMM_E_NOMEM if a capacity
+ * is too small, validation errors as phmm_forward_batch.  For tests and for sizing workspaces. */
+int phmm_plan_host(const phmm_batch* b, int long_min_hap_len, int task_rows, int64_t* plan_counts, int32_t* warp_first,
+                   int64_t cap_warps, int32_t* tasks, int64_t cap_tasks, int32_t* sorted_pair, int64_t cap_pairs);
+
 #ifdef __cplusplus
 }
 #endif

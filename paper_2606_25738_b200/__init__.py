@@ -5,4 +5,4 @@
 Importing the package does not load the CUDA library; the binding does, and fails loudly
 when it is missing (there is no CPU fallback).
 """
-__all__ = ["binding", "workloads"]
+__all__ = ["binding", "workloads", "replicas"]

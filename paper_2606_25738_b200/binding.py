@@ -22,7 +22,7 @@ PHMM_FP32_RESCUE, PHMM_FP64 = 0, 1
 PHMM_FLAG_RESCUED, PHMM_FLAG_LONG = 1, 2
 
 EXPORTS = ["phmm_create", "phmm_destroy", "phmm_forward_batch", "phmm_forward_batch_host", "phmm_get_stats",
-           "phmm_strerror", "phmm_last_cuda_error", "phmm_measure_peak"]
+           "phmm_strerror", "phmm_last_cuda_error", "phmm_measure_peak", "phmm_plan_host"]
 
 
 class phmm_options(ctypes.Structure):
@@ -91,6 +91,9 @@ def lib() -> ctypes.CDLL:
         L.phmm_last_cuda_error.argtypes = [ctypes.c_void_p]
         L.phmm_last_cuda_error.restype = ctypes.c_int
         L.phmm_measure_peak.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.POINTER(ctypes.c_double)]
+        L.phmm_plan_host.restype = ctypes.c_int
+        L.phmm_plan_host.argtypes = [ctypes.POINTER(phmm_batch), ctypes.c_int, ctypes.c_int, ctypes.c_void_p, ctypes.c_void_p,
+                                     ctypes.c_int64, ctypes.c_void_p, ctypes.c_int64, ctypes.c_void_p, ctypes.c_int64]
         L.phmm_measure_peak.restype = ctypes.c_int
         _lib = L
     return _lib
@@ -139,6 +142,27 @@ class DeviceBatch:
         return phmm_batch(len(self.read_off) - 1, len(self.hap_off) - 1, len(self.pair_read), _hp(self.read_off),
                           _hp(self.hap_off), ptr(self.t[0]), ptr(self.t[1]), ptr(self.t[2]), ptr(self.t[3]),
                           ptr(self.t[4]), ptr(self.t[5]), _hp(self.pair_read), _hp(self.pair_hap))
+
+
+def plan_host(batch, long_min_hap_len: int = 0, task_rows: int = 0):
+    """phmm_plan_host: the host batcher's work plan for a workloads.Batch-like object (no device needed).
+    Returns dict(n_warps, cols_per_lane, warp_first[n_warps+1], tasks[n_tasks,4] = (hap, first sorted pair,
+    n pairs, read rows), sorted_pair[n_sorted])."""
+    ro = np.ascontiguousarray(batch.read_off, dtype=np.int64); ho = np.ascontiguousarray(batch.hap_off, dtype=np.int64)
+    pr = np.ascontiguousarray(batch.pair_read, dtype=np.int32); ph = np.ascontiguousarray(batch.pair_hap, dtype=np.int32)
+    cb = phmm_batch(len(ro) - 1, len(ho) - 1, len(pr), _hp(ro), _hp(ho), 0, 0, 0, 0, 0, 0, _hp(pr), _hp(ph))
+    counts = np.zeros(4, dtype=np.int64)
+    L = lib()
+    rc = L.phmm_plan_host(ctypes.byref(cb), long_min_hap_len, task_rows, counts.ctypes.data, None, 0, None, 0, None, 0)
+    if rc != PHMM_OK:
+        raise PhmmError(rc)
+    nw, nt, ns = int(counts[0]), int(counts[1]), int(counts[2])
+    wf = np.zeros(nw + 1, dtype=np.int32); tk = np.zeros((max(nt, 1), 4), dtype=np.int32); sp = np.zeros(max(ns, 1), dtype=np.int32)
+    rc = L.phmm_plan_host(ctypes.byref(cb), long_min_hap_len, task_rows, counts.ctypes.data, wf.ctypes.data, nw,
+                          tk.ctypes.data, nt, sp.ctypes.data, ns)
+    if rc != PHMM_OK:
+        raise PhmmError(rc)
+    return {"n_warps": nw, "cols_per_lane": int(counts[3]), "warp_first": wf, "tasks": tk[:nt], "sorted_pair": sp[:ns]}
 
 
 class HostBatch:

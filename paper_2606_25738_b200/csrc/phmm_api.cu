@@ -72,6 +72,8 @@ struct phmm_ctx {
         if (e__ != cudaSuccess) { ctx->last_cuda = (int)e__; return e__ == cudaErrorMemoryAllocation ? PHMM_E_NOMEM : PHMM_E_CUDA; } \
     } while (0)
 
+#define RC(call) do { int rc__ = (call); if (rc__ != PHMM_OK) return rc__; } while (0)
+
 extern "C" const char* phmm_strerror(int code) {
     switch (code) {
         case PHMM_OK: return "ok";
@@ -163,6 +165,35 @@ extern "C" int phmm_get_stats(phmm_ctx* ctx, phmm_stats* out) {
 
 extern "C" int phmm_last_cuda_error(phmm_ctx* ctx) { return ctx ? ctx->last_cuda : 0; }
 
+extern "C" int phmm_plan_host(const phmm_batch* b, int long_min_hap_len, int task_rows, int64_t* plan_counts, int32_t* warp_first,
+                              int64_t cap_warps, int32_t* tasks, int64_t cap_tasks, int32_t* sorted_pair, int64_t cap_pairs) {
+    if (!b || !plan_counts || b->n_pairs < 0 || b->n_reads < 0 || b->n_haps < 0) return PHMM_E_ARG;
+    HostBatchView hv = {b->n_reads, b->n_haps, b->n_pairs, b->h_read_off, b->h_hap_off, b->h_pair_read, b->h_pair_hap};
+    if (b->n_pairs > 0) RC(validate_batch(hv));
+    if (long_min_hap_len <= 0 || long_min_hap_len > SHORT_MAX_K) long_min_hap_len = SHORT_MAX_K;
+    if (task_rows <= 0) task_rows = 3072;
+    std::vector<uint8_t> is_short((size_t)b->n_pairs, 0);
+    for (int64_t p = 0; p < b->n_pairs; p++) {
+        const int r = b->h_pair_read[p], h = b->h_pair_hap[p];
+        const int64_t l = b->h_read_off[r + 1] - b->h_read_off[r], k = b->h_hap_off[h + 1] - b->h_hap_off[h];
+        is_short[(size_t)p] = !(k > long_min_hap_len || l > 4096);
+    }
+    ShortPlan pl;
+    plan_short(hv, is_short.data(), SHORT_N2, task_rows, &pl);
+    const int64_t nw = (int64_t)pl.warp_first.size() - 1, nt = (int64_t)pl.tasks.size(), ns = (int64_t)pl.srt_out.size();
+    plan_counts[0] = nw; plan_counts[1] = nt; plan_counts[2] = ns; plan_counts[3] = SHORT_N2;
+    if (warp_first) { if (cap_warps < nw) return PHMM_E_NOMEM; memcpy(warp_first, pl.warp_first.data(), (size_t)(nw + 1) * 4); }
+    if (tasks) {
+        if (cap_tasks < nt) return PHMM_E_NOMEM;
+        for (int64_t i = 0; i < nt; i++) {
+            tasks[4 * i] = pl.tasks[(size_t)i].hap; tasks[4 * i + 1] = pl.tasks[(size_t)i].pair_first;
+            tasks[4 * i + 2] = pl.tasks[(size_t)i].n_pairs; tasks[4 * i + 3] = pl.tasks[(size_t)i].rows;
+        }
+    }
+    if (sorted_pair) { if (cap_pairs < ns) return PHMM_E_NOMEM; memcpy(sorted_pair, pl.srt_out.data(), (size_t)ns * 4); }
+    return PHMM_OK;
+}
+
 // ---------------------------------------------------------------- staging helper
 namespace {
 struct Stager {  // packs several host arrays into the pinned buffer and copies them with one memcpy each
@@ -182,7 +213,6 @@ struct Stager {  // packs several host arrays into the pinned buffer and copies 
 };
 }  // namespace
 
-#define RC(call) do { int rc__ = (call); if (rc__ != PHMM_OK) return rc__; } while (0)
 #define PROF(f, second) do { if (ctx->opt.profile_events) { CK(cudaEventRecord(ctx->ev_prof[2 * (f) + (second)], st)); ctx->prof_used[f] = true; } } while (0)
 
 extern "C" int phmm_forward_batch(phmm_ctx* ctx, const phmm_batch* b, int precision, double* d_out, uint8_t* d_flags,

@@ -1,0 +1,95 @@
+"""Host-side logic without a GPU: the batcher's work plan (phmm_plan_host) and the
+replica aggregation bench.py uses for N > 1 (world_size-2 gloo run on CPU)."""
+import os
+import sys
+
+import numpy as np
+import pytest
+
+from paper_2606_25738_b200 import binding as B
+from paper_2606_25738_b200 import replicas
+from paper_2606_25738_b200 import workloads as W
+
+
+def _check_plan(b, plan, long_min=1024):
+    rl, hl = b.read_len(), b.hap_len()
+    N2 = plan["cols_per_lane"]
+    k = hl[b.pair_hap]; l = rl[b.pair_read]
+    is_short = (k <= long_min) & (l <= 4096)
+    # every short pair exactly once, no long pair
+    assert sorted(plan["sorted_pair"].tolist()) == np.where(is_short)[0].tolist()
+    wf, tk, sp = plan["warp_first"], plan["tasks"], plan["sorted_pair"]
+    assert wf[0] == 0 and wf[-1] == len(tk) and np.all(np.diff(wf) >= 1)
+    # tasks partition the sorted pairs into contiguous, non-overlapping runs of one haplotype each
+    covered = np.zeros(len(sp), dtype=np.int32)
+    for hap, first, n, rows in tk:
+        assert n >= 1
+        idx = sp[first:first + n]
+        covered[first:first + n] += 1
+        assert np.all(b.pair_hap[idx] == hap)
+        assert rows == int(rl[b.pair_read[idx]].sum())
+    assert np.all(covered == 1)
+    # lanes of a warp: sum over its tasks of ceil(k / cols_per_lane) <= 32
+    for w in range(len(wf) - 1):
+        lanes = sum(-(-int(hl[t[0]]) // N2) for t in tk[wf[w]:wf[w + 1]])
+        assert 1 <= lanes <= 32
+
+
+def test_plan_config1_shape():
+    b = W.generate(1, n=6)
+    _check_plan(b, B.plan_host(b))
+
+
+def test_plan_mixed_unsorted_stream_and_long_pairs_left_out():
+    b = W.generate(2, n=4000)
+    p = B.plan_host(b)
+    _check_plan(b, p)
+    assert len(p["sorted_pair"]) < b.n_pairs  # some haplotypes exceed 1024 and go to the chain path
+
+
+def test_plan_custom_cut_and_small_tasks():
+    b = W.generate(1, n=2)
+    p = B.plan_host(b, long_min_hap_len=300, task_rows=500)
+    _check_plan(b, p, long_min=300)
+    assert np.all(p["tasks"][:, 3] < 500 + 260)  # a task closes once it holds >= task_rows read rows
+
+
+def test_plan_empty_and_invalid():
+    b = W.from_strings([("ACGT", "ACGTACGT")])
+    e = b.select_pairs(np.zeros(0, dtype=np.int64))
+    assert B.plan_host(e)["n_warps"] == 0
+    bad = W.Batch(b.read_off, b.hap_off, b.read_bases, b.qual_base, b.qual_ins, b.qual_del, b.qual_gcp, b.hap_bases,
+                  np.array([0], dtype=np.int32), np.array([3], dtype=np.int32))
+    with pytest.raises(B.PhmmError):
+        B.plan_host(bad)
+
+
+def _worker(rank, world, port, q):
+    import torch.distributed as dist
+    os.environ["MASTER_ADDR"] = "127.0.0.1"; os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    ms, cells, pairs = replicas.aggregate(10.0 + 5.0 * rank, 1e9 * (rank + 1), 100 * (rank + 1), dist)
+    q.put((rank, ms, cells, pairs, replicas.rank_seed(7, rank)))
+    dist.destroy_process_group()
+
+
+def test_replica_aggregation_world_size_2_gloo():
+    import torch.multiprocessing as mp
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = 29500 + (os.getpid() % 2000)
+    ps = [ctx.Process(target=_worker, args=(r, 2, port, q)) for r in range(2)]
+    for p in ps:
+        p.start()
+    res = sorted(q.get(timeout=120) for _ in ps)
+    for p in ps:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    for rank, ms, cells, pairs, seed in res:
+        assert ms == 15.0 and cells == 3e9 and pairs == 300  # max over ranks, sums over ranks
+        assert seed == 7 + rank
+    assert replicas.whole_job_gcups(15.0, 3e9, 3) == pytest.approx(3e9 / 5e-3 / 1e9)
+
+
+def test_replica_aggregation_single_process():
+    assert replicas.aggregate(4.0, 8.0, 2.0) == (4.0, 8.0, 2.0)
