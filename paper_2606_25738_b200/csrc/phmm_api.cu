@@ -235,26 +235,46 @@ extern "C" int phmm_forward_batch(phmm_ctx* ctx, const phmm_batch* b, int precis
 
     // ---- classify: short (sub-warp systolic fp32 kernel) / chain-sequential (one warp per pair) / chain-strips
     const int strip_cols = chain_strip_cols(fp64);
-    ctx->is_short.assign((size_t)np, 0);
+    if (ctx->is_short.size() != (size_t)np) ctx->is_short.resize((size_t)np);
     std::vector<int> seq_pairs, strip_pairs, sub_pairs;  // chain kernel work lists, fp64 sub-warp list (caller pair indices)
     int64_t cells = 0, long_cells = 0;
     int max_seq_l = 0;
-    for (int64_t p = 0; p < np; p++) {
-        const int r = b->h_pair_read[p], h = b->h_pair_hap[p];
-        const int64_t l = b->h_read_off[r + 1] - b->h_read_off[r], k = b->h_hap_off[h + 1] - b->h_hap_off[h];
-        cells += l * k;
-        const bool is_long = k > ctx->opt.long_min_hap_len || l > 4096;
-        if (is_long) { strip_pairs.push_back((int)p); long_cells += l * k; }
-        else if (fp64 && k <= RESCUE_MAX_K && l <= RESCUE_MAX_L) { sub_pairs.push_back((int)p); if (l > max_seq_l) max_seq_l = (int)l; }
-        else if (fp64) { seq_pairs.push_back((int)p); if (l > max_seq_l) max_seq_l = (int)l; }
-        else { ctx->is_short[(size_t)p] = 1; if (l > max_seq_l) max_seq_l = (int)l; }
+    {
+        struct Part { std::vector<int> seq, strip, sub; int64_t cells = 0, long_cells = 0; int max_l = 0; };
+        Part part[BATCHER_THREADS];
+        const int long_k = ctx->opt.long_min_hap_len;
+        uint8_t* is_short = ctx->is_short.data();
+        const int T = parallel_chunks(np, 1 << 16, [&](int t, int64_t lo, int64_t hi) {
+            Part& q = part[t];
+            for (int64_t p = lo; p < hi; p++) {
+                const int r = b->h_pair_read[p], h = b->h_pair_hap[p];
+                const int64_t l = b->h_read_off[r + 1] - b->h_read_off[r], k = b->h_hap_off[h + 1] - b->h_hap_off[h];
+                q.cells += l * k;
+                uint8_t sh = 0;
+                if (k > long_k || l > 4096) { q.strip.push_back((int)p); q.long_cells += l * k; }
+                else {
+                    if (fp64 && k <= RESCUE_MAX_K && l <= RESCUE_MAX_L) q.sub.push_back((int)p);
+                    else if (fp64) q.seq.push_back((int)p);
+                    else sh = 1;
+                    if (l > q.max_l) q.max_l = (int)l;
+                }
+                is_short[p] = sh;
+            }
+        });
+        for (int t = 0; t < T; t++) {  // chunks are contiguous and in order: the lists stay sorted by pair index
+            seq_pairs.insert(seq_pairs.end(), part[t].seq.begin(), part[t].seq.end());
+            strip_pairs.insert(strip_pairs.end(), part[t].strip.begin(), part[t].strip.end());
+            sub_pairs.insert(sub_pairs.end(), part[t].sub.begin(), part[t].sub.end());
+            cells += part[t].cells; long_cells += part[t].long_cells;
+            if (part[t].max_l > max_seq_l) max_seq_l = part[t].max_l;
+        }
     }
     ctx->stats.n_pairs = np;
     ctx->stats.cells = cells;
     ctx->stats.n_long_pairs = (int64_t)strip_pairs.size();
     ctx->stats.n_short_pairs = np - (int64_t)strip_pairs.size();
     if (!fp64) plan_short(hv, ctx->is_short.data(), SHORT_N2, ctx->opt.task_rows, &ctx->plan);
-    else { ctx->plan.tasks.clear(); ctx->plan.warp_first.assign(1, 0); ctx->plan.srt_read.clear(); ctx->plan.srt_out.clear(); ctx->plan.cells = 0; ctx->plan.padded_cells = 0; }
+    else { ctx->plan.tasks.clear(); ctx->plan.warp_first.assign(1, 0); ctx->plan.srt_read.clear(); ctx->plan.srt_out.clear(); ctx->plan.srt_ent.clear(); ctx->plan.cells = 0; ctx->plan.padded_cells = 0; }
     const ShortPlan& pl = ctx->plan;
     const int n_warps = (int)pl.warp_first.size() - 1;
     ctx->stats.short_cells = pl.cells;

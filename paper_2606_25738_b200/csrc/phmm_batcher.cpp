@@ -25,31 +25,49 @@ int validate_batch(const HostBatchView& b) {
         if (k > PHMM_MAX_LEN) return PHMM_E_TOOLONG;
     }
     if ((b.n_reads > 0 && b.read_off[0] < 0) || (b.n_haps > 0 && b.hap_off[0] < 0)) return PHMM_E_OFFSETS;
-    for (int64_t p = 0; p < b.n_pairs; p++) {
-        const int64_t r = b.pair_read[p], h = b.pair_hap[p];
-        if (r < 0 || r >= b.n_reads || h < 0 || h >= b.n_haps) return PHMM_E_OFFSETS;
-        if (b.read_off[r + 1] == b.read_off[r] || b.hap_off[h + 1] == b.hap_off[h]) return PHMM_E_EMPTY;
-    }
+    int rc[BATCHER_THREADS] = {0};
+    parallel_chunks(b.n_pairs, 1 << 16, [&](int t, int64_t lo, int64_t hi) {
+        for (int64_t p = lo; p < hi; p++) {
+            const int64_t r = b.pair_read[p], h = b.pair_hap[p];
+            if (r < 0 || r >= b.n_reads || h < 0 || h >= b.n_haps) { rc[t] = PHMM_E_OFFSETS; return; }
+            if (b.read_off[r + 1] == b.read_off[r] || b.hap_off[h + 1] == b.hap_off[h]) { if (!rc[t]) rc[t] = PHMM_E_EMPTY; }
+        }
+    });
+    for (int t = 0; t < BATCHER_THREADS; t++) if (rc[t] == PHMM_E_OFFSETS) return PHMM_E_OFFSETS;
+    for (int t = 0; t < BATCHER_THREADS; t++) if (rc[t]) return rc[t];
     return PHMM_OK;
 }
 
 void plan_short(const HostBatchView& b, const uint8_t* is_short, int N2, int task_rows, ShortPlan* out) {
-    out->tasks.clear(); out->warp_first.clear(); out->srt_read.clear(); out->srt_out.clear(); out->srt_ent.clear();
+    out->tasks.clear(); out->warp_first.clear();  // the sorted arrays keep their size: they are overwritten in full
     out->cells = 0; out->padded_cells = 0; out->max_read_len = 0;
     const int64_t np = b.n_pairs;
-    // ---- 1. stable counting sort of the selected pairs by haplotype
-    std::vector<int> cnt((size_t)b.n_haps + 1, 0);
+    // ---- 1. stable counting sort of the selected pairs by haplotype (chunks of the pair list in parallel:
+    //         per-chunk histograms, then every chunk scatters into its own slice of each haplotype's run)
+    const int64_t nh = b.n_haps;
+    std::vector<int> cnt((size_t)nh + 1, 0);
+    std::vector<std::vector<int>> hist(BATCHER_THREADS);
+    const int T = parallel_chunks(np, 1 << 17, [&](int t, int64_t lo, int64_t hi) {
+        std::vector<int>& hs = hist[t];
+        hs.assign((size_t)nh, 0);
+        for (int64_t p = lo; p < hi; p++)
+            if (is_short[p]) hs[b.pair_hap[p]]++;
+    });
     int64_t n_sel = 0;
-    for (int64_t p = 0; p < np; p++)
-        if (is_short[p]) { cnt[b.pair_hap[p] + 1]++; n_sel++; }
-    if (n_sel == 0) { out->warp_first.push_back(0); return; }
-    for (int64_t h = 0; h < b.n_haps; h++) cnt[h + 1] += cnt[h];
-    out->srt_read.resize((size_t)n_sel);
-    out->srt_out.resize((size_t)n_sel);
-    out->srt_ent.resize((size_t)n_sel * 2);
-    {
-        std::vector<int> pos(cnt.begin(), cnt.end() - 1);
-        for (int64_t p = 0; p < np; p++)
+    for (int64_t h = 0; h < nh; h++) {  // cnt[h] = start of haplotype h's run; hist[t][h] = start of chunk t's slice of it
+        cnt[h] = (int)n_sel;
+        for (int t = 0; t < T; t++) { const int c = hist[t][h]; hist[t][h] = (int)n_sel; n_sel += c; }
+    }
+    cnt[nh] = (int)n_sel;
+    if (n_sel == 0) { out->srt_read.clear(); out->srt_out.clear(); out->srt_ent.clear(); out->warp_first.push_back(0); return; }
+    if (out->srt_read.size() != (size_t)n_sel) {  // steady state: same size as the last call, nothing to (re)initialise
+        out->srt_read.resize((size_t)n_sel);
+        out->srt_out.resize((size_t)n_sel);
+        out->srt_ent.resize((size_t)n_sel * 2);
+    }
+    parallel_chunks(np, 1 << 17, [&](int t, int64_t lo, int64_t hi) {
+        std::vector<int>& pos = hist[t];
+        for (int64_t p = lo; p < hi; p++)
             if (is_short[p]) {
                 const int q = pos[b.pair_hap[p]]++;
                 const int r = b.pair_read[p];
@@ -58,28 +76,45 @@ void plan_short(const HostBatchView& b, const uint8_t* is_short, int N2, int tas
                 out->srt_ent[2 * (size_t)q] = (int)(TABLE_ZERO_RUN + b.read_off[r] + (int64_t)TABLE_EXTRA_ROWS * r);
                 out->srt_ent[2 * (size_t)q + 1] = (int)(b.read_off[r + 1] - b.read_off[r]) + TABLE_EXTRA_ROWS;
             }
-    }
-    // ---- 2. cut each haplotype's run of reads into tasks of about task_rows read rows
+    });
+    // ---- 2. cut each haplotype's run of reads into tasks of about task_rows read rows (haplotype ranges in parallel)
     std::vector<ShortTask> tasks;
-    tasks.reserve((size_t)(n_sel / 4 + 16));
-    for (int64_t h = 0; h < b.n_haps; h++) {
-        const int lo = cnt[h], hi = cnt[h + 1];
-        if (lo == hi) continue;
-        const int64_t k = b.hap_off[h + 1] - b.hap_off[h];
-        ShortTask t = {(int)h, lo, 0, 0};
-        for (int q = lo; q < hi; q++) {
-            const int r = out->srt_read[q];
-            const int l = (int)(b.read_off[r + 1] - b.read_off[r]);
-            out->cells += (int64_t)l * k;
-            if (l > out->max_read_len) out->max_read_len = l;
-            t.n_pairs++;
-            t.rows += l;
-            if (t.rows >= task_rows) {
-                tasks.push_back(t);
-                t.pair_first = q + 1; t.n_pairs = 0; t.rows = 0;
+    {
+        std::vector<ShortTask> part[BATCHER_THREADS];
+        int64_t pcells[BATCHER_THREADS] = {0};
+        int pmax[BATCHER_THREADS] = {0};
+        const int T2 = parallel_chunks(nh, 1 << 12, [&](int t, int64_t hlo, int64_t hhi) {
+            std::vector<ShortTask>& tv = part[t];
+            int64_t cells = 0;
+            int mx = 0;
+            for (int64_t h = hlo; h < hhi; h++) {
+                const int lo = cnt[h], hi = cnt[h + 1];
+                if (lo == hi) continue;
+                const int64_t k = b.hap_off[h + 1] - b.hap_off[h];
+                ShortTask tk = {(int)h, lo, 0, 0};
+                for (int q = lo; q < hi; q++) {
+                    const int l = out->srt_ent[2 * (size_t)q + 1] - TABLE_EXTRA_ROWS;
+                    cells += (int64_t)l * k;
+                    if (l > mx) mx = l;
+                    tk.n_pairs++;
+                    tk.rows += l;
+                    if (tk.rows >= task_rows) {
+                        tv.push_back(tk);
+                        tk.pair_first = q + 1; tk.n_pairs = 0; tk.rows = 0;
+                    }
+                }
+                if (tk.n_pairs > 0) tv.push_back(tk);
             }
+            pcells[t] = cells; pmax[t] = mx;
+        });
+        size_t nt = 0;
+        for (int t = 0; t < T2; t++) nt += part[t].size();
+        tasks.reserve(nt);
+        for (int t = 0; t < T2; t++) {
+            tasks.insert(tasks.end(), part[t].begin(), part[t].end());
+            out->cells += pcells[t];
+            if (pmax[t] > out->max_read_len) out->max_read_len = pmax[t];
         }
-        if (t.n_pairs > 0) tasks.push_back(t);
     }
     // ---- 3. pack tasks into warps: duration classes (longest first), lanes bin-packed largest-fit
     const int NCLS = 8 * 40;  // class = floor(8 * log2(duration)), duration < 2^40

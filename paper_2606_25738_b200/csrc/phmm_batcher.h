@@ -13,7 +13,26 @@
 
 #include "phmm_kernels.h"
 
+#include <algorithm>
+#include <thread>
+
 namespace phmm {
+
+// fn(t, begin, end) over [0, n) in contiguous chunks on up to BATCHER_THREADS threads (the caller's included)
+constexpr int BATCHER_THREADS = 8;
+template <typename F> inline int parallel_chunks(int64_t n, int64_t min_chunk, F fn) {
+    int T = (int)std::min<int64_t>(BATCHER_THREADS, std::max<int64_t>(1, n / min_chunk));
+    const unsigned hw = std::thread::hardware_concurrency();
+    if (hw > 0 && (unsigned)T > hw) T = (int)hw;
+    const int64_t per = (n + T - 1) / T;
+    std::vector<std::thread> th;
+    for (int t = 1; t < T; t++) th.emplace_back([=]() { fn(t, std::min(n, t * per), std::min(n, (t + 1) * per)); });
+    fn(0, 0, std::min(n, per));
+    for (auto& x : th) x.join();
+    return T;
+}
+
+
 
 struct HostBatchView {
     int64_t n_reads, n_haps, n_pairs;
