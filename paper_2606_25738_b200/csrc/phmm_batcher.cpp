@@ -152,25 +152,24 @@ void plan_short(const HostBatchView& b, const uint8_t* is_short, int N2, int tas
         }
         cap = 32; bin_steps = 0;
     };
+    std::vector<uint64_t> nonempty((size_t)NCLS, 0);  // bit g of nonempty[c] <=> bucket (c, g) still has tasks
+    for (int c = 0; c < NCLS; c++)
+        for (int g = 1; g <= 32; g++)
+            if (avail[c * 33 + g] < bstart[c * 33 + g + 1]) nonempty[c] |= 1ull << g;
     for (int c = NCLS - 1; c >= 0; c--) {
-        for (;;) {
-            int g = cap;
-            for (; g >= 1; g--)
-                if (avail[c * 33 + g] < bstart[c * 33 + g + 1]) break;
-            if (g < 1) {
-                // nothing of this class fits the open bin: is anything of this class left at all?
-                bool any = false;
-                for (int gg = cap + 1; gg <= 32 && !any; gg++) any = avail[c * 33 + gg] < bstart[c * 33 + gg + 1];
-                if (!any) break;  // class exhausted: carry the open bin over to the next (shorter) class
-                close_bin();
-                continue;
-            }
-            const ShortTask& t = tasks[ids[avail[c * 33 + g]++]];
+        while (nonempty[c]) {
+            const uint64_t fit = nonempty[c] & ((2ull << cap) - 1);  // lane counts <= cap
+            if (!fit) { close_bin(); continue; }  // nothing of this class fits the open bin
+            const int g = 63 - __builtin_clzll(fit);  // largest fit first
+            const int bk = c * 33 + g;
+            const ShortTask& t = tasks[ids[avail[bk]++]];
+            if (avail[bk] == bstart[bk + 1]) nonempty[c] &= ~(1ull << g);
             out->tasks.push_back(t);
             cap -= g;
             bin_steps = std::max(bin_steps, t.rows + TABLE_EXTRA_ROWS * t.n_pairs + 2 * g - 1);
             if (cap == 0) close_bin();
         }
+        // class exhausted: the open bin carries over to the next (shorter) class
     }
     close_bin();
 }
