@@ -302,6 +302,9 @@ def main():
                 "kernel_ms_per_launch": kms, "kernel_gcups": kcells / (kms * 1e-3) / 1e9 if kms > 0 else 0.0,
                 "kernel_share_of_step": kms / ms_step if ms_step > 0 else None,
                 "hbm_gbs_achieved": None, "family_ms": fam, "host_batch_ms": host_ms}
+    if roofline["traffic"] and kms > 0:  # DRAM bytes of the committed ncu capture (scaled to this batch) / this run's kernel time
+        roofline["hbm_gbs_achieved"] = roofline["traffic"] / (kms * 1e-3) / 1e9
+        roofline["hbm_frac_of_measured_peak"] = roofline["hbm_gbs_achieved"] / float(peaks.get("hbm_gbs") or 6471.1)
 
     cpu = None
     if not args.no_cpu_baseline:

@@ -54,7 +54,9 @@ template <typename T> struct Entry2 {
     uint32_t metaX, metaY;
 };
 
-template <typename T, int NV> struct Lane2 {
+// HS (fp32 only): take the Eq.3 predicates of both halves from one HSETP2 on per-column fp16 base codes instead
+// of two bit tests of the match word: 16 fewer ALU instructions per step, 12 more registers.
+template <typename T, int NV, bool HS = false> struct Lane2 {
     typedef W2<T> P;
     typedef typename P::V V;
     static_assert(NV <= 16, "one 32-bit match word per base: 16 columns per half");
@@ -63,6 +65,7 @@ template <typename T, int NV> struct Lane2 {
     V outT, outS;              // what dropped out on the right in the last step: (.x's, .y's)
     T sigX, sigY;              // Eq.4 partial sums (columns <= this half's last) of the read finished last
     uint32_t hm[4];            // match words, one per base b: bit x <=> .x column x is b, bit 16+x <=> .y column x is b
+    uint32_t h2[HS ? NV : 1];  // HS: per column the base codes of (.x, .y) as two fp16 numbers (1..4, 0 = none)
     int nvx, nvy;              // number of real (j <= k) columns in each half
 
     __device__ __forceinline__ void init() {
@@ -91,6 +94,21 @@ template <typename T, int NV> struct Lane2 {
                 for (int q = 0; q < 4; q++) hm[q] |= (c == q ? 1u : 0u) << (16 + x);
             }
         }
+        if (HS) {
+#pragma unroll
+            for (int x = 0; x < NV; x++) {
+                uint32_t v = 0;
+#pragma unroll
+                for (int q = 0; q < 4; q++) {
+                    if (hm[q] & (1u << x)) v |= half_code(q);
+                    if (hm[q] & (1u << (16 + x))) v |= half_code(q) << 16;
+                }
+                h2[x] = v;
+            }
+        }
+    }
+    static __device__ __forceinline__ uint32_t half_code(int c) {  // fp16 bit pattern of the number c + 1
+        return (uint32_t)((0x4400420040003C00ull >> (16 * c)) & 0xffffull);
     }
 
     // One systolic step.  (inS, inT, inSig): the left neighbour thread's (.y) outS, outT, sigY as they stand
@@ -105,7 +123,14 @@ template <typename T, int NV> struct Lane2 {
         const uint32_t wy01 = (E.metaY & 1u) ? hm[1] : hm[0], wy23 = (E.metaY & 1u) ? hm[3] : hm[2];
         const uint32_t wx = (E.metaX & 2u) ? wx23 : wx01, wy = (E.metaY & 2u) ? wy23 : wy01;
         const uint32_t mw = (wx & 0xffffu) | (wy & 0xffff0000u);
+        const uint32_t r2 = HS ? (half_code(E.metaX & 3u) | (half_code(E.metaY & 3u) << 16)) : 0u;
         auto prior = [&](int x) {                  // Eq.3: one select per half
+            if constexpr (HS && sizeof(T) == 4) {  // one HSETP2 yields both halves' predicates
+                float a, b;
+                asm("{.reg .pred p, q;\n setp.eq.f16x2 p|q, %2, %3;\n selp.f32 %0, %4, %5, p;\n selp.f32 %1, %6, %7, q;}"
+                    : "=f"(a), "=f"(b) : "r"(h2[x]), "r"(r2), "f"((float)E.pmx), "f"((float)E.pxx), "f"((float)E.pmy), "f"((float)E.pxy));
+                return P::mk((T)a, (T)b);
+            }
             return P::mk((mw & (1u << x)) ? E.pmx : E.pxx, (mw & (1u << (16 + x))) ? E.pmy : E.pxy);
         };
         V U = P::mul(prior(0), Tt[0]);

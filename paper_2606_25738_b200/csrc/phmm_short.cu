@@ -11,6 +11,9 @@
 #ifndef SHORT_PREFETCH
 #define SHORT_PREFETCH 0  // measured: the L1 prefetch costs more issue slots than it saves (2.50 vs 2.70 TCUPS)
 #endif
+#ifndef SHORT_HSETP2
+#define SHORT_HSETP2 1  // measured: 2.78 vs 2.60 TCUPS
+#endif
 #ifndef SHORT_FETCH_AHEAD
 #define SHORT_FETCH_AHEAD 1
 #endif
@@ -83,7 +86,7 @@ struct RawEntry { float4 a, b, c; uint2 m; };
 
 template <int NV>
 __global__ void __launch_bounds__(SHORT_WARPS_PER_CTA * 32, SHORT_MIN_CTAS) k_short_f32(DevBatch b, ShortLaunch p) {
-    typedef Lane2<float, NV> L;
+    typedef Lane2<float, NV, SHORT_HSETP2 != 0> L;
     constexpr int N2 = 2 * NV;
     const int warp = blockIdx.x * SHORT_WARPS_PER_CTA + (threadIdx.x >> 5);
     if (warp >= p.n_warps) return;
