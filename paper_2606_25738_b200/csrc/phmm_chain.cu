@@ -27,6 +27,9 @@
 
 namespace phmm {
 
+#ifndef CHAIN_HSETP2
+#define CHAIN_HSETP2 1  // fp32: +1-2 %
+#endif
 #ifndef CHAIN_POLL_ALL
 #define CHAIN_POLL_ALL 1  // measured: all lanes polling (2.02 TCUPS) beats one lane + __syncwarp (1.89)
 #endif
@@ -107,7 +110,7 @@ __device__ __forceinline__ int warp_max_i(int m) {
     return m;
 }
 
-template <typename T, int NV> __device__ __forceinline__ T lane_max(const Lane2<T, NV>& ln) {
+template <typename T, int NV, typename LN> __device__ __forceinline__ T lane_max(const LN& ln) {
     T m = Fx<T>::fmax_(Fx<T>::fmax_(ln.outS.x, ln.outS.y), Fx<T>::fmax_(ln.outT.x, ln.outT.y));
     m = Fx<T>::fmax_(m, Fx<T>::fmax_(ln.sigX, ln.sigY));
 #pragma unroll
@@ -117,7 +120,7 @@ template <typename T, int NV> __device__ __forceinline__ T lane_max(const Lane2<
     }
     return m;
 }
-template <typename T, int NV> __device__ __forceinline__ void lane_scale(Lane2<T, NV>& ln, int d) {  // *= 2^d
+template <typename T, int NV, typename LN> __device__ __forceinline__ void lane_scale(LN& ln, int d) {  // *= 2^d
     d = max(-Fx<T>::CLAMP, min(Fx<T>::CLAMP, d));
     const int h = d / 2;
     const T f1 = Fx<T>::exp2i(h), f2 = Fx<T>::exp2i(d - h);
@@ -134,10 +137,10 @@ template <typename T, int NV> __device__ __forceinline__ void lane_scale(Lane2<T
     ln.sigY = ln.sigY * f1 * f2;
 }
 
-template <typename T, int NV, int WPC>
-__global__ void __launch_bounds__(WPC * 32, (sizeof(T) == 4 ? CHAIN_MIN_CTAS_F32 : 2))
+template <typename T, int NV, int WPC, int MINB>
+__global__ void __launch_bounds__(WPC * 32, MINB)
 k_chain(DevBatch b, ChainLaunch p, int items_are_pairs) {
-    typedef Lane2<T, NV> L;
+    typedef Lane2<T, NV, (CHAIN_HSETP2 != 0) && sizeof(T) == 4> L;
     typedef RingFmt<T> RF;
     typedef typename W2<T>::V V;
     constexpr int N2 = 2 * NV;
@@ -351,23 +354,29 @@ k_chain(DevBatch b, ChainLaunch p, int items_are_pairs) {
 }
 
 constexpr int WPC_F32 = 4, WPC_F64 = 2;
+// fp32 comes in two register budgets: 4 CTAs/SM x 128 registers for throughput (many more strips than warp slots),
+// 3 CTAs/SM x ~166 registers when every strip is resident anyway and the pipeline depth of the wavefront decides
+// (configs[4]: 1.76 vs 1.63 TCUPS; configs[3]: 1.93 vs 2.01)
+constexpr int MINB_F32_MANY = CHAIN_MIN_CTAS_F32, MINB_F32_FEW = 3, MINB_F64 = 2;
 
 cudaError_t launch_chain(const DevBatch& b, const ChainLaunch& p, bool fp64, bool items_are_pairs, int grid_ctas,
-                         cudaStream_t st) {
+                         cudaStream_t st, bool few_items) {
     if (grid_ctas <= 0) return cudaSuccess;
     if (fp64)
-        k_chain<double, CHAIN_NV_F64, WPC_F64><<<grid_ctas, WPC_F64 * 32, 0, st>>>(b, p, items_are_pairs ? 1 : 0);
+        k_chain<double, CHAIN_NV_F64, WPC_F64, MINB_F64><<<grid_ctas, WPC_F64 * 32, 0, st>>>(b, p, items_are_pairs ? 1 : 0);
+    else if (few_items)
+        k_chain<float, CHAIN_NV_F32, WPC_F32, MINB_F32_FEW><<<grid_ctas, WPC_F32 * 32, 0, st>>>(b, p, items_are_pairs ? 1 : 0);
     else
-        k_chain<float, CHAIN_NV_F32, WPC_F32><<<grid_ctas, WPC_F32 * 32, 0, st>>>(b, p, items_are_pairs ? 1 : 0);
+        k_chain<float, CHAIN_NV_F32, WPC_F32, MINB_F32_MANY><<<grid_ctas, WPC_F32 * 32, 0, st>>>(b, p, items_are_pairs ? 1 : 0);
     return cudaGetLastError();
 }
 
 int chain_ctas_per_sm(bool fp64) {
     int n = 0;
     if (fp64)
-        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, k_chain<double, CHAIN_NV_F64, WPC_F64>, WPC_F64 * 32, 0);
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, k_chain<double, CHAIN_NV_F64, WPC_F64, MINB_F64>, WPC_F64 * 32, 0);
     else
-        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, k_chain<float, CHAIN_NV_F32, WPC_F32>, WPC_F32 * 32, 0);
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, k_chain<float, CHAIN_NV_F32, WPC_F32, MINB_F32_MANY>, WPC_F32 * 32, 0);
     return n > 0 ? n : 1;
 }
 int chain_warps_per_cta(bool fp64) { return fp64 ? WPC_F64 : WPC_F32; }

@@ -107,7 +107,7 @@ cudaError_t launch_lut_table(const DevBatch& b, const double* lut, float* table,
 cudaError_t launch_short_f32(const DevBatch& b, const ShortLaunch& p, cudaStream_t st);
 // rescue_from_list: items are taken from p.items[...] as plain pair indices in `rescue_list` form
 cudaError_t launch_chain(const DevBatch& b, const ChainLaunch& p, bool fp64, bool items_are_pairs, int grid_ctas,
-                         cudaStream_t st);
+                         cudaStream_t st, bool few_items = false);
 int chain_ctas_per_sm(bool fp64);
 int chain_warps_per_cta(bool fp64);
 size_t chain_block_bytes(bool fp64);  // bytes of one 32-row boundary block
