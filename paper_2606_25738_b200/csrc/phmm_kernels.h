@@ -22,8 +22,11 @@ struct DevBatch {  // device mirrors of the batch
 };
 
 // ---- fp64 recomputation of short pairs (phmm_rescue.cu)
-constexpr int RESCUE_NV = 16;                   // columns per lane
-constexpr int RESCUE_MAX_K = 32 * RESCUE_NV;    // 512: widest haplotype one warp covers in fp64
+#ifndef RESCUE_NV_
+#define RESCUE_NV_ 32
+#endif
+constexpr int RESCUE_NV = RESCUE_NV_;           // columns per lane
+constexpr int RESCUE_MAX_K = 32 * RESCUE_NV;    // widest haplotype one warp covers in fp64
 constexpr int RESCUE_MAX_L = 512;               // longest read unrescaled fp64 is trusted with (3.3 bits lost per unrelated row)
 
 struct RescueQueue {
