@@ -157,10 +157,29 @@ void plan_short(const HostBatchView& b, const uint8_t* is_short, int N2, int tas
         for (int g = 1; g <= 32; g++)
             if (avail[c * 33 + g] < bstart[c * 33 + g + 1]) nonempty[c] |= 1ull << g;
     for (int c = NCLS - 1; c >= 0; c--) {
+        uint64_t best_mask = 0;  // best[q] = most lanes of a q-lane gap that lane counts of best_mask can fill (unbounded knapsack)
+        int best[33];
         while (nonempty[c]) {
             const uint64_t fit = nonempty[c] & ((2ull << cap) - 1);  // lane counts <= cap
             if (!fit) { close_bin(); continue; }  // nothing of this class fits the open bin
-            const int g = 63 - __builtin_clzll(fit);  // largest fit first
+            if (best_mask != nonempty[c]) {
+                best_mask = nonempty[c];
+                best[0] = 0;
+                for (int q = 1; q <= 32; q++) {
+                    int bq = best[q - 1];
+                    for (uint64_t m = best_mask & ((2ull << q) - 1); m; m &= m - 1) {
+                        const int gg = __builtin_ctzll(m);
+                        bq = std::max(bq, gg + best[q - gg]);
+                    }
+                    best[q] = bq;
+                }
+            }
+            int g = 0, gfill = -1;  // the lane count after which the rest of the gap can be filled best; ties: the larger one
+            for (uint64_t m = fit; m; m &= m - 1) {
+                const int gg = __builtin_ctzll(m);
+                const int f = gg + best[cap - gg];
+                if (f >= gfill) { gfill = f; g = gg; }
+            }
             const int bk = c * 33 + g;
             const ShortTask& t = tasks[ids[avail[bk]++]];
             if (avail[bk] == bstart[bk + 1]) nonempty[c] &= ~(1ull << g);

@@ -11,14 +11,17 @@
 #ifndef SHORT_PREFETCH
 #define SHORT_PREFETCH 0  // measured: the L1 prefetch costs more issue slots than it saves (2.50 vs 2.70 TCUPS)
 #endif
+#ifndef SHORT_L2_PREFETCH
+#define SHORT_L2_PREFETCH 1
+#endif
 #ifndef SHORT_HSETP2
 #define SHORT_HSETP2 1  // measured: 2.78 vs 2.60 TCUPS
 #endif
 #ifndef SHORT_FETCH_AHEAD
-#define SHORT_FETCH_AHEAD 1
+#define SHORT_FETCH_AHEAD 2  // with the HSETP2 engine: 3 CTAs x 168 registers + two steps ahead (2.86) beats 4 x 128 + one (2.78)
 #endif
 #ifndef SHORT_MIN_CTAS
-#define SHORT_MIN_CTAS 4  // resident CTAs per SM the register allocation is held to (4 x 128 threads -> <= 128 registers)
+#define SHORT_MIN_CTAS 3  // resident CTAs per SM the register allocation is held to (3 x 128 threads -> <= 168 registers)
 #endif
 
 namespace phmm {
@@ -81,6 +84,14 @@ struct Cursor {
 };
 
 __device__ __forceinline__ void prefetch_l1(const void* p) { asm volatile("prefetch.global.L1 [%0];" ::"l"(p)); }
+
+// read-only load that asks L2 to fetch the 256-byte pair of lines on a miss: the second line holds the slots this
+// lane group reads 16 steps later
+__device__ __forceinline__ float4 ldg_pf(const float4* p) {
+    float4 v;
+    asm volatile("ld.global.nc.L2::256B.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "l"(p));
+    return v;
+}
 
 struct RawEntry { float4 a, b, c; uint2 m; };
 
@@ -157,10 +168,17 @@ __global__ void __launch_bounds__(SHORT_WARPS_PER_CTA * 32, SHORT_MIN_CTAS) k_sh
         if (is_first) prefetch_l1(tab + ((int64_t)(c.pos >> 5) + 1) * 128 + (c.pos & 15) * 8);
 #endif
         c.pos++;
+#if SHORT_L2_PREFETCH
+        r.a = ldg_pf(e);
+        r.b = ldg_pf(e + TABLE_CHUNK_STRIDE);
+        r.c = ldg_pf(e + 2 * TABLE_CHUNK_STRIDE);
+        { const float4 t = ldg_pf(e + 3 * TABLE_CHUNK_STRIDE); r.m = make_uint2(__float_as_uint(t.x), __float_as_uint(t.y)); }
+#else
         r.a = __ldg(e);
         r.b = __ldg(e + TABLE_CHUNK_STRIDE);
         r.c = __ldg(e + 2 * TABLE_CHUNK_STRIDE);
         r.m = __ldg(reinterpret_cast<const uint2*>(e + 3 * TABLE_CHUNK_STRIDE));
+#endif
     };
 
     int nout = 0;
