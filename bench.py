@@ -44,6 +44,7 @@ WORKLOADS = {  # name -> (BASELINE.json config index, description)
     "mixed": (2, "configs[2] mixed-length stream: 10M unsorted pairs, 5% unrelated reads"),
     "long": (3, "configs[3] long-read batch: 2000 pairs, reads 5-15 kbp"),
     "verylong": (4, "configs[4] very-long stress: 16 pairs of 100 kbp x 105 kbp"),
+    "equal": (5, "paper's scalability-sweep shape (PAPER.md:366): read length = haplotype length = --len, noisy copies"),
 }
 FLOPS_PER_CELL = 10.0  # SURVEY 8(d)'s algorithmic count (4 FMA + 2 MUL per cell); DESIGN.md section 7
 FLOPS_PER_CELL_EXECUTED = {"fp32": 9.0, "fp64": 11.0}  # what the engines issue: 4 FMA + 1 MUL (fp32 T/J form), 4 FMA + 3 MUL (fp64 sub-warp kernel)
@@ -119,9 +120,12 @@ class ClockSampler:
                 "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
 
 
-def make_batch(workload, scale, seed_offset):
+def make_batch(workload, scale, seed_offset, length=512):
     from paper_2606_25738_b200 import workloads
     cfg = WORKLOADS[workload][0]
+    if cfg == 5:  # about 4e10 cells per launch, between 16 and 4M pairs
+        n = int(min(4_000_000, max(16, round(4e10 * min(scale, 1.0) / float(length) ** 2))))
+        return workloads.generate(5, seed=6 + seed_offset, n=n, len_lo=length), cfg
     full = {0: 0, 1: 2000, 2: 10_000_000, 3: 2000, 4: 16}[cfg]
     n = 0 if (scale >= 1.0 or cfg == 0) else max(1, int(round(full * scale)))
     return workloads.generate(cfg, seed=1 + cfg + seed_offset, n=n), cfg
@@ -150,7 +154,7 @@ def run_reference(args, rank, world):
     """--impl reference: the oracle, as it stands, on the host cores (rank 0 only)."""
     if rank != 0:
         return
-    batch, cfg = make_batch(args.workload, args.scale, 0)
+    batch, cfg = make_batch(args.workload, args.scale, 0, args.len)
     budget = 6.0  # seconds of oracle work per step
     res = None
     for _ in range(args.warmup):
@@ -183,6 +187,7 @@ def main():
     ap.add_argument("--workload", default="short", choices=sorted(WORKLOADS))
     ap.add_argument("--precision", default="fp32", choices=["fp32", "fp64"])
     ap.add_argument("--scale", type=float, default=1.0, help="fraction of the workload's full size")
+    ap.add_argument("--len", type=int, default=512, help="--workload equal: read length = haplotype length")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     args = ap.parse_args()
@@ -206,7 +211,7 @@ def main():
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device(dev))
 
-    batch, cfg = make_batch(args.workload, args.scale, replicas.rank_seed(0, rank))
+    batch, cfg = make_batch(args.workload, args.scale, replicas.rank_seed(0, rank), args.len)
     cells, n_pairs = batch.cells(), batch.n_pairs
     prec = binding.PHMM_FP32_RESCUE if args.precision == "fp32" else binding.PHMM_FP64
     ctx = binding.Context(local, profile_events=1)
@@ -316,7 +321,8 @@ def main():
         "metric": "PairHMM forward throughput", "value": gcups, "unit": "GCUPS", "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f32" if args.precision == "fp32" else "f64", "data": "synthetic",
-        "config": {"workload": WORKLOADS[args.workload][1], "precision": "fp32 + fp64 rescue" if args.precision == "fp32" else "fp64",
+        "config": {"workload": WORKLOADS[args.workload][1] + (" (len %d)" % args.len if cfg == 5 else ""),
+                   "precision": "fp32 + fp64 rescue" if args.precision == "fp32" else "fp64",
                    "scale": args.scale, "pairs": int(tot_pairs), "cells": int(tot_cells), "parallelism": "replicas x%d" % world,
                    "l2": "inputs larger than L2 (payload + %.0f MB row-constant table rewritten and re-read every step)" % (st["table_bytes"] / 1e6)},
         "pairs_per_s": tot_pairs / (ms_step * 1e-3),
