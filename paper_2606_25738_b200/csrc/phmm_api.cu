@@ -65,6 +65,8 @@ struct phmm_ctx {
     int chain_grid[2] = {0, 0};
     cudaEvent_t ev_prof[8] = {};   // profile_events: [2f], [2f+1] bracket family f (0 table, 1 short, 2 rescue, 3 long)
     bool prof_used[4] = {false, false, false, false};
+    bool reuse_table = false;    // host entry, chunks after the first: the row-constant table of this payload is already on the device
+    bool stats_final = false;    // host entry: n_rescued was counted from the flags, do not re-read the device counters
 };
 
 #define CK(call)                                                    \
@@ -143,7 +145,7 @@ extern "C" int phmm_destroy(phmm_ctx* ctx) {
 
 extern "C" int phmm_get_stats(phmm_ctx* ctx, phmm_stats* out) {
     if (!ctx || !out) return PHMM_E_ARG;
-    if (ctx->d_counters.p && ctx->stats.n_pairs > 0) {  // rescue count lives on the device until the caller has synchronised
+    if (!ctx->stats_final && ctx->d_counters.p && ctx->stats.n_pairs > 0) {  // rescue count lives on the device until the caller has synchronised
         int n = 0;
         cudaSetDevice(ctx->device);
         int rq[48];
@@ -222,6 +224,7 @@ extern "C" int phmm_forward_batch(phmm_ctx* ctx, const phmm_batch* b, int precis
     if (precision != PHMM_FP32_RESCUE && precision != PHMM_FP64) return PHMM_E_ARG;
     if (b->n_pairs < 0 || b->n_reads < 0 || b->n_haps < 0) return PHMM_E_ARG;
     memset(&ctx->stats, 0, sizeof(ctx->stats));
+    ctx->stats_final = false;
     for (int f = 0; f < 4; f++) ctx->prof_used[f] = false;
     if (b->n_pairs == 0) return PHMM_OK;
     if (!d_out || !b->d_read_bases || !b->d_qual_base || !b->d_qual_ins || !b->d_qual_del || !b->d_qual_gcp || !b->d_hap_bases)
@@ -369,7 +372,7 @@ extern "C" int phmm_forward_batch(phmm_ctx* ctx, const phmm_batch* b, int precis
         CK(ctx->d_table.need(table_bytes));
         ctx->stats.table_bytes = (int64_t)table_bytes;
         PROF(0, 0);
-        CK(launch_lut_table(db, (const double*)ctx->d_lut.p, (float*)ctx->d_table.p, st));
+        if (!ctx->reuse_table) CK(launch_lut_table(db, (const double*)ctx->d_lut.p, (float*)ctx->d_table.p, st));
         PROF(0, 1);
         ShortLaunch sl;
         sl.table = (const float*)ctx->d_table.p;
@@ -505,9 +508,41 @@ extern "C" int phmm_forward_batch_host(phmm_ctx* ctx, const phmm_batch* b, int p
     phmm_batch db = *b;
     db.d_read_bases = base; db.d_qual_base = base + Ra; db.d_qual_ins = base + 2 * Ra; db.d_qual_del = base + 3 * Ra;
     db.d_qual_gcp = base + 4 * Ra; db.d_hap_bases = base + 5 * Ra;
-    RC(phmm_forward_batch(ctx, &db, precision, (double*)ctx->d_out.p, (uint8_t*)ctx->d_flags.p, st));
-    CK(cudaMemcpyAsync(h_out, ctx->d_out.p, (size_t)b->n_pairs * 8, cudaMemcpyDeviceToHost, st));
-    if (h_flags) CK(cudaMemcpyAsync(h_flags, ctx->d_flags.p, (size_t)b->n_pairs, cudaMemcpyDeviceToHost, st));
+    // The pair list is processed in chunks: phmm_forward_batch only enqueues, so the host batcher of chunk c+1 runs
+    // while the GPU works on chunk c, and each chunk's results start their way back as soon as it is done.  The
+    // row-constant table depends on the payload only and is built with the first chunk.
+    const int64_t np = b->n_pairs;
+    const int n_chunks = (int)std::max<int64_t>(1, std::min<int64_t>(8, np / 400000));
+    phmm_stats sum;
+    memset(&sum, 0, sizeof(sum));
+    int rc = PHMM_OK;
+    for (int c = 0; c < n_chunks && rc == PHMM_OK; c++) {
+        const int64_t lo = np * c / n_chunks, hi = np * (c + 1) / n_chunks;
+        phmm_batch cb = db;
+        cb.n_pairs = hi - lo;
+        cb.h_pair_read = b->h_pair_read + lo;
+        cb.h_pair_hap = b->h_pair_hap + lo;
+        ctx->reuse_table = c > 0 && sum.n_short_warps > 0;
+        rc = phmm_forward_batch(ctx, &cb, precision, (double*)ctx->d_out.p + lo, (uint8_t*)ctx->d_flags.p + lo, st);
+        ctx->reuse_table = false;
+        if (rc != PHMM_OK) break;
+        const phmm_stats& t = ctx->stats;
+        sum.n_pairs += t.n_pairs; sum.cells += t.cells; sum.n_short_pairs += t.n_short_pairs; sum.n_long_pairs += t.n_long_pairs;
+        sum.short_cells += t.short_cells; sum.short_padded_cells += t.short_padded_cells; sum.n_short_warps += t.n_short_warps;
+        sum.n_kernel_launches += t.n_kernel_launches; sum.host_batch_ms += t.host_batch_ms;
+        if (t.table_bytes > sum.table_bytes) sum.table_bytes = t.table_bytes;
+        if (cudaMemcpyAsync(h_out + lo, (double*)ctx->d_out.p + lo, (size_t)(hi - lo) * 8, cudaMemcpyDeviceToHost, st) != cudaSuccess) rc = PHMM_E_CUDA;
+    }
+    if (rc != PHMM_OK) { cudaStreamSynchronize(st); return rc; }
+    std::vector<uint8_t> tmp_flags;
+    uint8_t* fl = h_flags;
+    if (!fl) { tmp_flags.resize((size_t)np); fl = tmp_flags.data(); }
+    CK(cudaMemcpyAsync(fl, ctx->d_flags.p, (size_t)np, cudaMemcpyDeviceToHost, st));
     CK(cudaStreamSynchronize(st));
+    sum.n_slices = n_chunks;
+    for (int64_t p = 0; p < np; p++) sum.n_rescued += fl[p] & PHMM_FLAG_RESCUED;
+    ctx->stats = sum;
+    ctx->stats_final = true;
     return PHMM_OK;
 }
+
