@@ -512,7 +512,18 @@ extern "C" int phmm_forward_batch_host(phmm_ctx* ctx, const phmm_batch* b, int p
     // while the GPU works on chunk c, and each chunk's results start their way back as soon as it is done.  The
     // row-constant table depends on the payload only and is built with the first chunk.
     const int64_t np = b->n_pairs;
-    const int n_chunks = (int)std::max<int64_t>(1, std::min<int64_t>(8, np / 400000));
+    int n_chunks = (int)std::max<int64_t>(1, std::min<int64_t>(8, np / 400000));
+    if (n_chunks > 1) {  // only worth it if the chunks use disjoint haplotypes: a shuffled list would split every task
+        int hmin[8], hmax[8];
+        for (int c = 0; c < n_chunks; c++) {
+            const int64_t lo = np * c / n_chunks, hi = np * (c + 1) / n_chunks;
+            int mn = INT32_MAX, mx = -1;
+            for (int64_t p = lo; p < hi; p++) { const int h = b->h_pair_hap[p]; mn = std::min(mn, h); mx = std::max(mx, h); }
+            hmin[c] = mn; hmax[c] = mx;
+        }
+        for (int c = 0; c + 1 < n_chunks; c++)
+            if (hmax[c] >= hmin[c + 1]) { n_chunks = 1; break; }
+    }
     phmm_stats sum;
     memset(&sum, 0, sizeof(sum));
     int rc = PHMM_OK;
