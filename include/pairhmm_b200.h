@@ -137,7 +137,10 @@ int phmm_forward_batch(phmm_ctx* ctx, const phmm_batch* b, int precision, double
 
 /* Same computation with ALL buffers on the host (the d_* members of `b` are host pointers, out
  * pointers are host): the library copies the payload to the device, runs phmm_forward_batch, copies
- * the results back and synchronises.  This is the end-to-end entry ("with transfer"). */
+ * the results back and synchronises.  This is the end-to-end entry ("with transfer").
+ * A large pair list whose consecutive chunks (>= 400 k pairs, at most 8) use disjoint haplotypes is enqueued chunk
+ * by chunk, so that the host batcher of one chunk overlaps the device work of the previous one; results and
+ * flags are the same as for one call.  phmm_get_stats afterwards reports the sums over the chunks. */
 int phmm_forward_batch_host(phmm_ctx* ctx, const phmm_batch* b, int precision, double* h_out_log10,
                             uint8_t* h_out_flags);
 
