@@ -140,7 +140,7 @@ template <typename T, int NV, typename LN> __device__ __forceinline__ void lane_
 template <typename T, int NV, int WPC, int MINB>
 __global__ void __launch_bounds__(WPC * 32, MINB)
 k_chain(DevBatch b, ChainLaunch p, int items_are_pairs) {
-    typedef Lane2<T, NV, (CHAIN_HSETP2 != 0) && sizeof(T) == 4> L;
+    typedef Lane2<T, NV, (CHAIN_HSETP2 != 0) && sizeof(T) == 4 && MINB == 3> L;  // HSETP2 only where the 12 extra registers do not spill
     typedef RingFmt<T> RF;
     typedef typename W2<T>::V V;
     constexpr int N2 = 2 * NV;
