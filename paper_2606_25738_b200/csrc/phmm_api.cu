@@ -53,13 +53,21 @@ struct phmm_ctx {
     phmm_options opt;
     phmm_stats stats;
     int last_cuda = 0;
-    cudaEvent_t ev_upload = nullptr;  // staging buffers are free again once this has fired
-    bool upload_pending = false;
-    DevBuf d_lut, d_read_off, d_hap_off, d_pair_read, d_pair_hap, d_table, d_tasks, d_warp_first, d_srt_read, d_srt_out;
-    DevBuf d_counters, d_rescue, d_items, d_boundary, d_progress, d_scratch;
-    DevBuf d_rq, d_rq_queue, d_rq_sorted, d_rq_plan, d_rq_enq;  // fp64 sub-warp recomputation: counters, queue, ordered queue, plan, FP64-mode input list
+    // The read-only plan arrays of a call live in one of two sets, uploaded on a copy stream of the context: the
+    // uploads of call s+1 overlap the kernels of call s.  A set (and its pinned staging buffer) is reused once the
+    // call that used it two calls ago has completed (ev_free, recorded on the caller's stream at the end of a call).
+    struct PlanSet {
+        DevBuf d_read_off, d_hap_off, d_pair_read, d_pair_hap, d_tasks, d_warp_first, d_srt_read, d_srt_out, d_items, d_rq_enq;
+        PinBuf h_stage;
+        cudaEvent_t ev_free = nullptr, ev_up = nullptr;
+        bool used = false;
+    } set[2];
+    int call_idx = 0;
+    cudaStream_t copy_stream = nullptr;
+    DevBuf d_lut, d_table;
+    DevBuf d_counters, d_rescue, d_boundary, d_progress, d_scratch;
+    DevBuf d_rq, d_rq_queue, d_rq_sorted, d_rq_plan;  // fp64 sub-warp recomputation: counters, queue, ordered queue, plan, FP64-mode input list
     DevBuf d_payload, d_out, d_flags;  // phmm_forward_batch_host only
-    PinBuf h_stage;
     std::vector<uint8_t> is_short;
     ShortPlan plan;
     int chain_grid[2] = {0, 0};
@@ -112,7 +120,10 @@ extern "C" int phmm_create(phmm_ctx** out, int device, const phmm_options* opt) 
             if (cudaEventCreate(&ctx->ev_prof[i]) != cudaSuccess) { delete ctx; return PHMM_E_CUDA; }
     memset(&ctx->stats, 0, sizeof(ctx->stats));
     if (cudaSetDevice(device) != cudaSuccess) { delete ctx; return PHMM_E_CUDA; }
-    if (cudaEventCreateWithFlags(&ctx->ev_upload, cudaEventDisableTiming) != cudaSuccess) { delete ctx; return PHMM_E_CUDA; }
+    for (int i = 0; i < 2; i++)
+        if (cudaEventCreateWithFlags(&ctx->set[i].ev_free, cudaEventDisableTiming) != cudaSuccess ||
+            cudaEventCreateWithFlags(&ctx->set[i].ev_up, cudaEventDisableTiming) != cudaSuccess) { phmm_destroy(ctx); return PHMM_E_CUDA; }
+    if (cudaStreamCreateWithFlags(&ctx->copy_stream, cudaStreamNonBlocking) != cudaSuccess) { phmm_destroy(ctx); return PHMM_E_CUDA; }
     // 10^(-q/10) for q = 0..255, the paper's "q64" table
     double lut[256];
     for (int q = 0; q < 256; q++) lut[q] = pow(10.0, -(double)q / 10.0);
@@ -130,13 +141,19 @@ extern "C" int phmm_destroy(phmm_ctx* ctx) {
     if (!ctx) return PHMM_E_ARG;
     cudaSetDevice(ctx->device);
     cudaDeviceSynchronize();
-    DevBuf* bufs[] = {&ctx->d_lut, &ctx->d_read_off, &ctx->d_hap_off, &ctx->d_pair_read, &ctx->d_pair_hap, &ctx->d_table,
-                      &ctx->d_tasks, &ctx->d_warp_first, &ctx->d_srt_read, &ctx->d_srt_out, &ctx->d_counters, &ctx->d_rescue,
-                      &ctx->d_items, &ctx->d_boundary, &ctx->d_progress, &ctx->d_scratch, &ctx->d_payload, &ctx->d_out, &ctx->d_flags,
-                      &ctx->d_rq, &ctx->d_rq_queue, &ctx->d_rq_sorted, &ctx->d_rq_plan, &ctx->d_rq_enq};
+    DevBuf* bufs[] = {&ctx->d_lut, &ctx->d_table, &ctx->d_counters, &ctx->d_rescue, &ctx->d_boundary, &ctx->d_progress, &ctx->d_scratch,
+                      &ctx->d_payload, &ctx->d_out, &ctx->d_flags, &ctx->d_rq, &ctx->d_rq_queue, &ctx->d_rq_sorted, &ctx->d_rq_plan};
     for (DevBuf* b : bufs) b->release();
-    ctx->h_stage.release();
-    if (ctx->ev_upload) cudaEventDestroy(ctx->ev_upload);
+    for (int i = 0; i < 2; i++) {
+        phmm_ctx::PlanSet& ps = ctx->set[i];
+        DevBuf* sb[] = {&ps.d_read_off, &ps.d_hap_off, &ps.d_pair_read, &ps.d_pair_hap, &ps.d_tasks, &ps.d_warp_first,
+                        &ps.d_srt_read, &ps.d_srt_out, &ps.d_items, &ps.d_rq_enq};
+        for (DevBuf* b : sb) b->release();
+        ps.h_stage.release();
+        if (ps.ev_free) cudaEventDestroy(ps.ev_free);
+        if (ps.ev_up) cudaEventDestroy(ps.ev_up);
+    }
+    if (ctx->copy_stream) cudaStreamDestroy(ctx->copy_stream);
     for (int i = 0; i < 8; i++)
         if (ctx->ev_prof[i]) cudaEventDestroy(ctx->ev_prof[i]);
     delete ctx;
@@ -201,16 +218,17 @@ extern "C" int phmm_plan_host(const phmm_batch* b, int long_min_hap_len, int tas
 namespace {
 struct Stager {  // packs several host arrays into the pinned buffer and copies them with one memcpy each
     phmm_ctx* ctx;
+    PinBuf* stage;
     cudaStream_t st;
     size_t used = 0;
     int upload(DevBuf& dst, const void* src, size_t bytes) {
         if (bytes == 0) return PHMM_OK;
         CK(dst.need(bytes));
         const size_t at = (used + 255) & ~(size_t)255;
-        if (at + bytes > ctx->h_stage.cap) return PHMM_E_NOMEM;
-        memcpy((char*)ctx->h_stage.p + at, src, bytes);
+        if (at + bytes > stage->cap) return PHMM_E_NOMEM;
+        memcpy((char*)stage->p + at, src, bytes);
         used = at + bytes;
-        CK(cudaMemcpyAsync(dst.p, (char*)ctx->h_stage.p + at, bytes, cudaMemcpyHostToDevice, st));
+        CK(cudaMemcpyAsync(dst.p, (char*)stage->p + at, bytes, cudaMemcpyHostToDevice, st));
         return PHMM_OK;
     }
 };
@@ -317,48 +335,53 @@ extern "C" int phmm_forward_batch(phmm_ctx* ctx, const phmm_batch* b, int precis
     const auto t1 = std::chrono::steady_clock::now();
     ctx->stats.host_batch_ms = std::chrono::duration<double, std::milli>(t1 - t0).count();
 
-    // ---- uploads (one pinned staging buffer, reused once the previous call's copies have completed)
-    if (ctx->upload_pending) { CK(cudaEventSynchronize(ctx->ev_upload)); ctx->upload_pending = false; }
+    // ---- uploads.  The plan arrays go to this call's plan set on the context's copy stream (overlapping the kernels
+    // of the previous call, which read the other set); the small per-call counters and lists that kernels also write
+    // stay on the caller's stream.
+    phmm_ctx::PlanSet& ps = ctx->set[ctx->call_idx & 1];
+    ctx->call_idx++;
+    if (ps.used) CK(cudaEventSynchronize(ps.ev_free));  // the call that used this set (two calls ago) has completed
     const size_t n_seq = fp64 ? seq_pairs.size() : 0;
     size_t stage_bytes = 4096 + (size_t)(b->n_reads + 1) * 8 + (size_t)(b->n_haps + 1) * 8 + (size_t)np * 8 +
                          pl.tasks.size() * sizeof(ShortTask) + pl.warp_first.size() * 4 + pl.srt_read.size() * 16 +
                          items.size() * sizeof(ChainItem) + n_seq * 4 + sub_pairs.size() * 4 + 20 * 256;
-    CK(ctx->h_stage.need(stage_bytes));
-    Stager sg{ctx, st};
-    RC(sg.upload(ctx->d_read_off, b->h_read_off, (size_t)(b->n_reads + 1) * 8));
-    RC(sg.upload(ctx->d_hap_off, b->h_hap_off, (size_t)(b->n_haps + 1) * 8));
-    RC(sg.upload(ctx->d_pair_read, b->h_pair_read, (size_t)np * 4));
-    RC(sg.upload(ctx->d_pair_hap, b->h_pair_hap, (size_t)np * 4));
-    RC(sg.upload(ctx->d_tasks, pl.tasks.data(), pl.tasks.size() * sizeof(ShortTask)));
-    RC(sg.upload(ctx->d_warp_first, pl.warp_first.data(), pl.warp_first.size() * 4));
-    RC(sg.upload(ctx->d_srt_read, pl.srt_ent.data(), pl.srt_ent.size() * 4));
-    RC(sg.upload(ctx->d_srt_out, pl.srt_out.data(), pl.srt_out.size() * 4));
-    RC(sg.upload(ctx->d_items, items.data(), items.size() * sizeof(ChainItem)));
+    CK(ps.h_stage.need(stage_bytes));
+    Stager sg{ctx, &ps.h_stage, ctx->copy_stream};
+    RC(sg.upload(ps.d_read_off, b->h_read_off, (size_t)(b->n_reads + 1) * 8));
+    RC(sg.upload(ps.d_hap_off, b->h_hap_off, (size_t)(b->n_haps + 1) * 8));
+    RC(sg.upload(ps.d_pair_read, b->h_pair_read, (size_t)np * 4));
+    RC(sg.upload(ps.d_pair_hap, b->h_pair_hap, (size_t)np * 4));
+    RC(sg.upload(ps.d_tasks, pl.tasks.data(), pl.tasks.size() * sizeof(ShortTask)));
+    RC(sg.upload(ps.d_warp_first, pl.warp_first.data(), pl.warp_first.size() * 4));
+    RC(sg.upload(ps.d_srt_read, pl.srt_ent.data(), pl.srt_ent.size() * 4));
+    RC(sg.upload(ps.d_srt_out, pl.srt_out.data(), pl.srt_out.size() * 4));
+    RC(sg.upload(ps.d_items, items.data(), items.size() * sizeof(ChainItem)));
+    RC(sg.upload(ps.d_rq_enq, sub_pairs.data(), sub_pairs.size() * 4));
+    CK(cudaEventRecord(ps.ev_up, ctx->copy_stream));
+    CK(cudaStreamWaitEvent(st, ps.ev_up, 0));
     // counters: [0] rescue count (= n_items of the rescue launch)  [1] ticket rescue  [2] n strip items  [3] ticket strips
     //           [4] n sequential fp64 items  [5] ticket sequential
+    sg.st = st;  // from here on: buffers that kernels write as well, in stream order with them
     int h_counters[8] = {0, 0, (int)items.size(), 0, (int)n_seq, 0, 0, 0};
     RC(sg.upload(ctx->d_counters, h_counters, sizeof(h_counters)));
     // rescue list (fp32 mode: filled by the short kernel) / sequential list (fp64 mode: all non-long pairs)
     CK(ctx->d_rescue.need((size_t)np * 4 + 4));
-    if (n_seq) {
-        const size_t at = (sg.used + 255) & ~(size_t)255;
-        memcpy((char*)ctx->h_stage.p + at, seq_pairs.data(), n_seq * 4);
-        sg.used = at + n_seq * 4;
-        CK(cudaMemcpyAsync(ctx->d_rescue.p, (char*)ctx->h_stage.p + at, n_seq * 4, cudaMemcpyHostToDevice, st));
-    }
-    RC(sg.upload(ctx->d_rq_enq, sub_pairs.data(), sub_pairs.size() * 4));
+    RC(sg.upload(ctx->d_rescue, seq_pairs.data(), n_seq * 4));
     CK(ctx->d_rq.need(48 * 4));
     CK(ctx->d_rq_plan.need(68 * 4));
     CK(ctx->d_rq_queue.need((size_t)np * 16 + 16));
     CK(ctx->d_rq_sorted.need((size_t)np * 4 + 4));
     CK(cudaMemsetAsync(ctx->d_rq.p, 0, 48 * 4, st));
-    CK(cudaEventRecord(ctx->ev_upload, st));
-    ctx->upload_pending = true;
+    ps.used = true;
+    struct FreeMark {  // whatever path leaves the call: the set is free once everything enqueued so far on st has run
+        cudaEvent_t ev; cudaStream_t st;
+        ~FreeMark() { cudaEventRecord(ev, st); }
+    } free_mark{ps.ev_free, st};
 
     DevBatch db;
     db.read_bases = b->d_read_bases; db.qual_base = b->d_qual_base; db.qual_ins = b->d_qual_ins;
     db.qual_del = b->d_qual_del; db.qual_gcp = b->d_qual_gcp; db.hap_bases = b->d_hap_bases;
-    db.read_off = (const int64_t*)ctx->d_read_off.p; db.hap_off = (const int64_t*)ctx->d_hap_off.p;
+    db.read_off = (const int64_t*)ps.d_read_off.p; db.hap_off = (const int64_t*)ps.d_hap_off.p;
     db.n_reads = b->n_reads; db.n_haps = b->n_haps;
     int* counters = (int*)ctx->d_counters.p;
     int launches = 0;
@@ -376,11 +399,11 @@ extern "C" int phmm_forward_batch(phmm_ctx* ctx, const phmm_batch* b, int precis
         PROF(0, 1);
         ShortLaunch sl;
         sl.table = (const float*)ctx->d_table.p;
-        sl.tasks = (const ShortTask*)ctx->d_tasks.p;
-        sl.warp_first = (const int*)ctx->d_warp_first.p;
+        sl.tasks = (const ShortTask*)ps.d_tasks.p;
+        sl.warp_first = (const int*)ps.d_warp_first.p;
         sl.n_warps = n_warps;
-        sl.srt_ent = (const int2*)ctx->d_srt_read.p;
-        sl.srt_out = (const int*)ctx->d_srt_out.p;
+        sl.srt_ent = (const int2*)ps.d_srt_read.p;
+        sl.srt_out = (const int*)ps.d_srt_out.p;
         sl.out = d_out;
         sl.flags = d_flags;
         sl.rescue_thr = (float)ldexp(1.0, ctx->opt.rescue_log2_threshold);
@@ -403,12 +426,12 @@ extern "C" int phmm_forward_batch(phmm_ctx* ctx, const phmm_batch* b, int precis
         rl.queue.cnt = (int*)ctx->d_rq.p;
         rl.queue.n_queue = (int*)ctx->d_rq.p + 34;
         rl.max_queue = (int)(fp64 ? (int64_t)sub_pairs.size() : ctx->stats.n_short_pairs);
-        rl.enqueue_pairs = fp64 ? (const int*)ctx->d_rq_enq.p : nullptr;
+        rl.enqueue_pairs = fp64 ? (const int*)ps.d_rq_enq.p : nullptr;
         rl.n_enqueue = fp64 ? (int)sub_pairs.size() : 0;
         rl.plan = (int*)ctx->d_rq_plan.p;
         rl.sorted = (int*)ctx->d_rq_sorted.p;
-        rl.pair_read = (const int*)ctx->d_pair_read.p;
-        rl.pair_hap = (const int*)ctx->d_pair_hap.p;
+        rl.pair_read = (const int*)ps.d_pair_read.p;
+        rl.pair_hap = (const int*)ps.d_pair_hap.p;
         rl.lut = (const double*)ctx->d_lut.p;
         rl.out = d_out;
         rl.flags = d_flags;
@@ -432,8 +455,8 @@ extern "C" int phmm_forward_batch(phmm_ctx* ctx, const phmm_batch* b, int precis
         cl.items = (const ChainItem*)ctx->d_rescue.p;
         cl.n_items = counters + (fp64 ? 4 : 0);
         cl.ticket = counters + (fp64 ? 5 : 1);
-        cl.pair_read = (const int*)ctx->d_pair_read.p;
-        cl.pair_hap = (const int*)ctx->d_pair_hap.p;
+        cl.pair_read = (const int*)ps.d_pair_read.p;
+        cl.pair_hap = (const int*)ps.d_pair_hap.p;
         cl.lut = (const double*)ctx->d_lut.p;
         cl.boundary = ctx->d_scratch.p;
         cl.scratch_blocks = blocks;
@@ -454,11 +477,11 @@ extern "C" int phmm_forward_batch(phmm_ctx* ctx, const phmm_batch* b, int precis
         CK(cudaMemsetAsync(ctx->d_progress.p, 0, (size_t)n_prog * 4 + 4, st));
         ChainLaunch cl;
         memset(&cl, 0, sizeof(cl));
-        cl.items = (const ChainItem*)ctx->d_items.p;
+        cl.items = (const ChainItem*)ps.d_items.p;
         cl.n_items = counters + 2;
         cl.ticket = counters + 3;
-        cl.pair_read = (const int*)ctx->d_pair_read.p;
-        cl.pair_hap = (const int*)ctx->d_pair_hap.p;
+        cl.pair_read = (const int*)ps.d_pair_read.p;
+        cl.pair_hap = (const int*)ps.d_pair_hap.p;
         cl.lut = (const double*)ctx->d_lut.p;
         cl.boundary = ctx->d_boundary.p;
         cl.scratch_blocks = 0;

@@ -167,6 +167,27 @@ def test_pair_order_and_duplicates_bitwise(B, ctx):
     assert np.array_equal(out_d, out[dup])
 
 
+def test_async_calls_back_to_back_bitwise(B, ctx):
+    """The call only enqueues: different batches issued back to back on one stream (plan uploads of call s+1 run
+    on the context's copy stream under the kernels of call s, two plan sets alternate) must give exactly what each
+    batch gives alone, in both precisions, also on a side stream."""
+    import torch
+    batches = [W.generate(1, seed=11, n=3), W.generate(2, seed=12, n=6000), W.generate(1, seed=13, n=2),
+               W.generate(3, seed=14, n=3, len_lo=1200, len_hi=2600), W.generate(0, seed=15), W.generate(2, seed=16, n=3000)]
+    dbs = [B.DeviceBatch(b) for b in batches]
+    for prec in (B.PHMM_FP32_RESCUE, B.PHMM_FP64):
+        alone = []
+        for db in dbs:
+            o, f = ctx.forward_batch(db, prec)
+            alone.append((o.cpu().numpy().copy(), f.cpu().numpy().copy()))
+        for stream in (None, torch.cuda.Stream()):
+            res = [ctx.forward_batch(db, prec, stream=stream, sync=False) for db in dbs for _ in range(2)]
+            torch.cuda.synchronize()
+            for i, (o, f) in enumerate(res):
+                a = alone[i // 2]
+                assert np.array_equal(o.cpu().numpy(), a[0]) and np.array_equal(f.cpu().numpy(), a[1]), "call %d differs" % i
+
+
 def test_host_entry_matches_device_entry(B, ctx):
     b = W.generate(1, n=3)
     out, fl = run(B, ctx, b, B.PHMM_FP32_RESCUE)
