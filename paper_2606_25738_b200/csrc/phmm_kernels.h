@@ -27,7 +27,9 @@ struct DevBatch {  // device mirrors of the batch
 #endif
 constexpr int RESCUE_NV = RESCUE_NV_;           // columns per lane
 constexpr int RESCUE_MAX_K = 32 * RESCUE_NV;    // widest haplotype one warp covers in fp64
-constexpr int RESCUE_MAX_L = 512;               // longest read unrescaled fp64 is trusted with (3.3 bits lost per unrelated row)
+constexpr int RESCUE_MAX_L = 4096;              // = the short class.  Unrescaled fp64 holds ~600 unrelated rows (3.3 bits lost per row) but
+                                                // thousands of related ones; a result below 1e-290 is passed on to the rescaled chain kernel,
+                                                // and above it the flushed cells weigh < 2^-36 of the sum
 
 struct RescueQueue {
     int4* queue;      // (pair, lane-group size g, ticket within bucket g, -)

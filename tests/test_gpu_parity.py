@@ -167,6 +167,17 @@ def test_pair_order_and_duplicates_bitwise(B, ctx):
     assert np.array_equal(out_d, out[dup])
 
 
+def test_equal_length_sweep_shape(B, ctx):
+    """the paper's scalability-sweep shape (read length = haplotype length, noisy copies,
+    PAPER.md:366), one length per kernel family: 32 and 512 (short kernel; 512-bp reads partly rescued), 1024 (short
+    kernel + chain fallback of the rescued ones), 3000 (chain kernel, 3 strips)."""
+    for L, n in ((32, 300), (512, 40), (1024, 12), (3000, 4)):
+        b = W.generate(5, seed=40 + L, n=n, len_lo=L)
+        out, fl, ref = check(B, ctx, b, B.PHMM_FP32_RESCUE)
+        check_flags(B, b, fl, ref)
+        check(B, ctx, b, B.PHMM_FP64, ref=ref)
+
+
 def test_async_calls_back_to_back_bitwise(B, ctx):
     """The call only enqueues: different batches issued back to back on one stream (plan uploads of call s+1 run
     on the context's copy stream under the kernels of call s, two plan sets alternate) must give exactly what each
