@@ -30,12 +30,6 @@ namespace phmm {
 #ifndef CHAIN_HSETP2
 #define CHAIN_HSETP2 1  // fp32: +1-2 %
 #endif
-#ifndef CHAIN_POLL_ALL
-#define CHAIN_POLL_ALL 1  // measured: all lanes polling (2.02 TCUPS) beats one lane + __syncwarp (1.89)
-#endif
-#ifndef CHAIN_POLL_NS
-#define CHAIN_POLL_NS 64
-#endif
 #ifndef CHAIN_MIN_CTAS_F32
 #define CHAIN_MIN_CTAS_F32 4  // 128 registers; measured +4.5 % over 3 CTAs x 166 registers
 #endif
@@ -241,13 +235,8 @@ k_chain(DevBatch b, ChainLaunch p, int items_are_pairs) {
                     if (blk && has_in && s < n_ent) {
                         const int need = min(s + 32, n_ent);
                         if (inprog) {  // one lane polls; the others park at the barrier
-#if CHAIN_POLL_ALL
-                            while (ld_acquire(inprog) < need) __nanosleep(CHAIN_POLL_NS);
-#else
-                            if (lane == 0)
-                                while (ld_acquire(inprog) < need) __nanosleep(CHAIN_POLL_NS);
-                            __syncwarp();
-#endif
+                            // every lane polls: measured faster (2.02 vs 1.89 TCUPS) than one polling lane + __syncwarp
+                            while (ld_acquire(inprog) < need) __nanosleep(64);
                         }
                         const Rec<T>* src = inb + (s >> 5);
                         RI.S[lane] = src->S[lane]; RI.Tn[lane] = src->Tn[lane]; RI.Sig[lane] = src->Sig[lane];

@@ -18,8 +18,8 @@
 namespace phmm {
 
 // ---- meta word of a stream entry: bits 0-1 read base code (A,C,G,T; other bytes: pm := px, "matches nothing"),
-// LAST = the read's last row, FIRST = run-in entry (the group's first lane injects C/k); RESET is unused.
-enum : uint32_t { META_CODE_MASK = 3u, META_RESET = 8u, META_LAST = 16u, META_FIRST = 32u };
+// LAST = the read's last row, FIRST = run-in entry (the group's first lane injects C/k).
+enum : uint32_t { META_CODE_MASK = 3u, META_LAST = 16u, META_FIRST = 32u };
 
 #define PHMM_FULL 0xffffffffu
 
@@ -31,19 +31,18 @@ __host__ __device__ inline int base_code(uint8_t b) {
 // ---- exponent helpers for the block-floating (rescaled) variants
 template <typename T> struct Fx;
 template <> struct Fx<float> {
-    static constexpr int TGT = 16, HI = 56, PER_LO = 24, PER_HI = 24, CLAMP = 280, CLAMP1 = 126;
+    static constexpr int CLAMP = 280, CLAMP1 = 126;  // largest shift applied with two factors / with one
     static __device__ __forceinline__ int ilogb(float v) { return (int)((__float_as_uint(v) >> 23) & 0xffu) - 127; }
     // 2^e for e in [-126,127]; below -> 0, above -> 2^127
     static __device__ __forceinline__ float exp2i(int e) { return e < -126 ? 0.f : __uint_as_float((unsigned)(min(e, 127) + 127) << 23); }
     static __device__ __forceinline__ float fmax_(float a, float b) { return fmaxf(a, b); }
 };
 template <> struct Fx<double> {
-    static constexpr int TGT = 0, HI = 600, PER_LO = 300, PER_HI = 300, CLAMP = 2200, CLAMP1 = 1022;
+    static constexpr int CLAMP = 2200, CLAMP1 = 1022;
     static __device__ __forceinline__ int ilogb(double v) { return (int)((__double2hiint(v) >> 20) & 0x7ff) - 1023; }
     static __device__ __forceinline__ double exp2i(int e) { return e < -1022 ? 0.0 : __hiloint2double((min(e, 1023) + 1023) << 20, 0); }
     static __device__ __forceinline__ double fmax_(double a, double b) { return fmax(a, b); }
 };
-constexpr int EX_ZERO = -(1 << 28);  // exponent of a lane whose state is identically zero
 
 template <typename T> __device__ __forceinline__ T shfl_up1(T v);
 template <> __device__ __forceinline__ float shfl_up1<float>(float v) { return __shfl_up_sync(PHMM_FULL, v, 1); }

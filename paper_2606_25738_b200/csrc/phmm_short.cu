@@ -1,18 +1,16 @@
 // Short-pair path: row-constant table prologue + the sub-warp systolic fp32 kernel.
 //
 // Hot path rows of SURVEY.md section 8(a): a1 (quality -> row constants: table kernel), a2 (haplotype
-// staging: match bitmasks in registers), a3/a4 (row updates), a5 (lane-to-lane carry: 4 shuffles per
-// row), a9 (final reduction, log10), a10 (underflow detection -> rescue queue).
+// staging: match words / fp16 base codes in registers), a3/a4 (row updates), a5 (lane-to-lane carry: 3 shuffles
+// per row), a9 (final reduction, log10), a10 (underflow detection -> rescue queue).
 #include "phmm_engine.cuh"
 #include "phmm_kernels.h"
 #include "phmm_rowconst.cuh"
 #include <type_traits>
 
-#ifndef SHORT_PREFETCH
-#define SHORT_PREFETCH 0  // measured: the L1 prefetch costs more issue slots than it saves (2.50 vs 2.70 TCUPS)
-#endif
+// Tunables, each with the measurement that chose it (configs[1], in-kernel TCUPS)
 #ifndef SHORT_L2_PREFETCH
-#define SHORT_L2_PREFETCH 1
+#define SHORT_L2_PREFETCH 1  // table loads carry the L2 256-byte prefetch hint: +0.6 %
 #endif
 #ifndef SHORT_HSETP2
 #define SHORT_HSETP2 1  // measured: 2.78 vs 2.60 TCUPS
@@ -76,14 +74,13 @@ cudaError_t launch_lut_table(const DevBatch& b, const double* lut, float* table,
 // Per lane, the .x half walks its task's stream of table entries (run of read 1, run of read 2, ...) starting
 // 2*lg steps after the group's first lane.  While it waits, and after its stream has ended, a lane walks the
 // zero run at the start of the table (all-zero constants decay T and J to 0), so the fetch needs no special
-// cases.  Entries are loaded one step ahead into two alternating register sets (step loop unrolled by two).
+// cases.  Entries are loaded SHORT_FETCH_AHEAD steps ahead into rotating register sets (the step loop is unrolled
+// by the number of sets, so no register is ever copied).
 struct Cursor {
     int pos, end;        // next entry to fetch, one past the last entry of the current run
     int npos, nend;      // the run after it: the next read of the task, or the zero run
     int q;               // reads of the task already handed to (npos, nend)
 };
-
-__device__ __forceinline__ void prefetch_l1(const void* p) { asm volatile("prefetch.global.L1 [%0];" ::"l"(p)); }
 
 // read-only load that asks L2 to fetch the 256-byte pair of lines on a miss: the second line holds the slots this
 // lane group reads 16 steps later
@@ -162,11 +159,6 @@ __global__ void __launch_bounds__(SHORT_WARPS_PER_CTA * 32, SHORT_MIN_CTAS) k_sh
     auto fetch = [&](RawEntry& r) {
         if (c.pos == c.end) { c.pos = c.npos; c.end = c.nend; load_next(); }
         const float4* e = tab + table_slot(c.pos);
-#if SHORT_PREFETCH
-        // the group's first lane is the only one that touches new lines: have it pull one line of the NEXT
-        // 2 KB block into L1 per step (16 lines per block, each requested twice in 32 steps)
-        if (is_first) prefetch_l1(tab + ((int64_t)(c.pos >> 5) + 1) * 128 + (c.pos & 15) * 8);
-#endif
         c.pos++;
 #if SHORT_L2_PREFETCH
         r.a = ldg_pf(e);
