@@ -130,10 +130,10 @@ void plan_short(const HostBatchView& b, const uint8_t* is_short, int N2, int tas
     // bucket index = cls * 33 + g ; counting sort of task ids
     std::vector<int> bstart((size_t)NCLS * 33 + 1, 0);
     std::vector<int> tb(tasks.size());
-    for (size_t i = 0; i < tasks.size(); i++) {
-        tb[i] = cls_of(tasks[i]) * 33 + lanes_of(tasks[i]);
-        bstart[tb[i] + 1]++;
-    }
+    parallel_chunks((int64_t)tasks.size(), 1 << 14, [&](int, int64_t lo, int64_t hi) {
+        for (int64_t i = lo; i < hi; i++) tb[(size_t)i] = cls_of(tasks[(size_t)i]) * 33 + lanes_of(tasks[(size_t)i]);
+    });
+    for (size_t i = 0; i < tasks.size(); i++) bstart[tb[i] + 1]++;
     for (size_t i = 0; i + 1 < bstart.size(); i++) bstart[i + 1] += bstart[i];
     std::vector<int> ids(tasks.size());
     {
@@ -141,56 +141,86 @@ void plan_short(const HostBatchView& b, const uint8_t* is_short, int N2, int tas
         for (size_t i = 0; i < tasks.size(); i++) ids[pos[tb[i]]++] = (int)i;
     }
     std::vector<int> avail(bstart.begin(), bstart.end() - 1);  // next unused id per bucket
-    out->tasks.reserve(tasks.size());
-    out->warp_first.reserve(tasks.size() / 2 + 2);
-    out->warp_first.push_back(0);
-    int cap = 32, bin_steps = 0;
-    auto close_bin = [&]() {
-        if (cap < 32) {
-            out->warp_first.push_back((int)out->tasks.size());
-            out->padded_cells += (int64_t)bin_steps * 32 * N2;
-        }
-        cap = 32; bin_steps = 0;
-    };
     std::vector<uint64_t> nonempty((size_t)NCLS, 0);  // bit g of nonempty[c] <=> bucket (c, g) still has tasks
     for (int c = 0; c < NCLS; c++)
         for (int g = 1; g <= 32; g++)
             if (avail[c * 33 + g] < bstart[c * 33 + g + 1]) nonempty[c] |= 1ull << g;
-    for (int c = NCLS - 1; c >= 0; c--) {
-        uint64_t best_mask = 0;  // best[q] = most lanes of a q-lane gap that lane counts of best_mask can fill (unbounded knapsack)
-        int best[33];
-        while (nonempty[c]) {
-            const uint64_t fit = nonempty[c] & ((2ull << cap) - 1);  // lane counts <= cap
-            if (!fit) { close_bin(); continue; }  // nothing of this class fits the open bin
-            if (best_mask != nonempty[c]) {
-                best_mask = nonempty[c];
-                best[0] = 0;
-                for (int q = 1; q <= 32; q++) {
-                    int bq = best[q - 1];
-                    for (uint64_t m = best_mask & ((2ull << q) - 1); m; m &= m - 1) {
-                        const int gg = __builtin_ctzll(m);
-                        bq = std::max(bq, gg + best[q - gg]);
-                    }
-                    best[q] = bq;
-                }
-            }
-            int g = 0, gfill = -1;  // the lane count after which the rest of the gap can be filled best; ties: the larger one
-            for (uint64_t m = fit; m; m &= m - 1) {
-                const int gg = __builtin_ctzll(m);
-                const int f = gg + best[cap - gg];
-                if (f >= gfill) { gfill = f; g = gg; }
-            }
-            const int bk = c * 33 + g;
-            const ShortTask& t = tasks[ids[avail[bk]++]];
-            if (avail[bk] == bstart[bk + 1]) nonempty[c] &= ~(1ull << g);
-            out->tasks.push_back(t);
-            cap -= g;
-            bin_steps = std::max(bin_steps, t.rows + TABLE_EXTRA_ROWS * t.n_pairs + 2 * g - 1);
-            if (cap == 0) close_bin();
+    // the classes are packed in parallel: contiguous class ranges of about equal task counts, longest classes first;
+    // inside a range the open bin carries over from a class to the next shorter one, at the end of a range it is closed
+    struct Part { std::vector<ShortTask> tasks; std::vector<int> warp_end; int64_t padded = 0; };
+    Part part[BATCHER_THREADS];
+    int range_hi[BATCHER_THREADS + 1];
+    const int TP = (int)std::min<int64_t>(BATCHER_THREADS, std::max<int64_t>(1, (int64_t)tasks.size() / (1 << 14)));
+    {
+        const int64_t per = ((int64_t)tasks.size() + TP - 1) / TP;
+        int t = 0;
+        range_hi[0] = NCLS - 1;
+        int64_t acc = 0;
+        for (int c = NCLS - 1; c >= 0 && t + 1 < TP; c--) {
+            acc += bstart[(size_t)(c + 1) * 33] - bstart[(size_t)c * 33];
+            if (acc >= per * (t + 1)) range_hi[++t] = c - 1;
         }
-        // class exhausted: the open bin carries over to the next (shorter) class
+        while (t < TP) range_hi[++t] = -1;
     }
-    close_bin();
+    auto pack_range = [&](int t) {
+        Part& P = part[t];
+        int cap = 32, bin_steps = 0;
+        auto close_bin = [&]() {
+            if (cap < 32) {
+                P.warp_end.push_back((int)P.tasks.size());
+                P.padded += (int64_t)bin_steps * 32 * N2;
+            }
+            cap = 32; bin_steps = 0;
+        };
+        for (int c = range_hi[t]; c > range_hi[t + 1]; c--) {
+            uint64_t best_mask = 0;  // best[q] = most lanes of a q-lane gap that lane counts of best_mask can fill (unbounded knapsack)
+            int best[33];
+            while (nonempty[c]) {
+                const uint64_t fit = nonempty[c] & ((2ull << cap) - 1);  // lane counts <= cap
+                if (!fit) { close_bin(); continue; }  // nothing of this class fits the open bin
+                if (best_mask != nonempty[c]) {
+                    best_mask = nonempty[c];
+                    best[0] = 0;
+                    for (int q = 1; q <= 32; q++) {
+                        int bq = best[q - 1];
+                        for (uint64_t m = best_mask & ((2ull << q) - 1); m; m &= m - 1) {
+                            const int gg = __builtin_ctzll(m);
+                            bq = std::max(bq, gg + best[q - gg]);
+                        }
+                        best[q] = bq;
+                    }
+                }
+                int g = 0, gfill = -1;  // the lane count after which the rest of the gap can be filled best; ties: the larger one
+                for (uint64_t m = fit; m; m &= m - 1) {
+                    const int gg = __builtin_ctzll(m);
+                    const int f = gg + best[cap - gg];
+                    if (f >= gfill) { gfill = f; g = gg; }
+                }
+                const int bk = c * 33 + g;
+                const ShortTask& tk = tasks[ids[avail[bk]++]];
+                if (avail[bk] == bstart[bk + 1]) nonempty[c] &= ~(1ull << g);
+                P.tasks.push_back(tk);
+                cap -= g;
+                bin_steps = std::max(bin_steps, tk.rows + TABLE_EXTRA_ROWS * tk.n_pairs + 2 * g - 1);
+                if (cap == 0) close_bin();
+            }
+        }
+        close_bin();
+    };
+    {
+        std::vector<std::thread> th;
+        for (int t = 1; t < TP; t++) th.emplace_back(pack_range, t);
+        pack_range(0);
+        for (auto& x : th) x.join();
+    }
+    out->tasks.reserve(tasks.size());
+    out->warp_first.push_back(0);
+    for (int t = 0; t < TP; t++) {
+        const int base = (int)out->tasks.size();
+        out->tasks.insert(out->tasks.end(), part[t].tasks.begin(), part[t].tasks.end());
+        for (int e : part[t].warp_end) out->warp_first.push_back(base + e);
+        out->padded_cells += part[t].padded;
+    }
 }
 
 }  // namespace phmm
