@@ -57,7 +57,7 @@ struct phmm_ctx {
     // uploads of call s+1 overlap the kernels of call s.  A set (and its pinned staging buffer) is reused once the
     // call that used it two calls ago has completed (ev_free, recorded on the caller's stream at the end of a call).
     struct PlanSet {
-        DevBuf d_read_off, d_hap_off, d_pair_read, d_pair_hap, d_tasks, d_warp_first, d_srt_read, d_srt_out, d_items, d_rq_enq;
+        DevBuf d_read_off, d_hap_off, d_pair_read, d_pair_hap, d_tasks, d_warp_first, d_srt_ent, d_srt_out, d_items, d_rq_enq;
         PinBuf h_stage;
         cudaEvent_t ev_free = nullptr, ev_up = nullptr;
         bool used = false;
@@ -147,7 +147,7 @@ extern "C" int phmm_destroy(phmm_ctx* ctx) {
     for (int i = 0; i < 2; i++) {
         phmm_ctx::PlanSet& ps = ctx->set[i];
         DevBuf* sb[] = {&ps.d_read_off, &ps.d_hap_off, &ps.d_pair_read, &ps.d_pair_hap, &ps.d_tasks, &ps.d_warp_first,
-                        &ps.d_srt_read, &ps.d_srt_out, &ps.d_items, &ps.d_rq_enq};
+                        &ps.d_srt_ent, &ps.d_srt_out, &ps.d_items, &ps.d_rq_enq};
         for (DevBuf* b : sb) b->release();
         ps.h_stage.release();
         if (ps.ev_free) cudaEventDestroy(ps.ev_free);
@@ -296,7 +296,7 @@ extern "C" int phmm_forward_batch(phmm_ctx* ctx, const phmm_batch* b, int precis
     ctx->stats.n_long_pairs = (int64_t)strip_pairs.size();
     ctx->stats.n_short_pairs = np - (int64_t)strip_pairs.size();
     if (!fp64) plan_short(hv, ctx->is_short.data(), SHORT_N2, ctx->opt.task_rows, &ctx->plan);
-    else { ctx->plan.tasks.clear(); ctx->plan.warp_first.assign(1, 0); ctx->plan.srt_read.clear(); ctx->plan.srt_out.clear(); ctx->plan.srt_ent.clear(); ctx->plan.cells = 0; ctx->plan.padded_cells = 0; }
+    else { ctx->plan.tasks.clear(); ctx->plan.warp_first.assign(1, 0); ctx->plan.srt_out.clear(); ctx->plan.srt_ent.clear(); ctx->plan.cells = 0; ctx->plan.padded_cells = 0; }
     const ShortPlan& pl = ctx->plan;
     const int n_warps = (int)pl.warp_first.size() - 1;
     ctx->stats.short_cells = pl.cells;
@@ -343,7 +343,7 @@ extern "C" int phmm_forward_batch(phmm_ctx* ctx, const phmm_batch* b, int precis
     if (ps.used) CK(cudaEventSynchronize(ps.ev_free));  // the call that used this set (two calls ago) has completed
     const size_t n_seq = fp64 ? seq_pairs.size() : 0;
     size_t stage_bytes = 4096 + (size_t)(b->n_reads + 1) * 8 + (size_t)(b->n_haps + 1) * 8 + (size_t)np * 8 +
-                         pl.tasks.size() * sizeof(ShortTask) + pl.warp_first.size() * 4 + pl.srt_read.size() * 16 +
+                         pl.tasks.size() * sizeof(ShortTask) + pl.warp_first.size() * 4 + pl.srt_out.size() * 16 +
                          items.size() * sizeof(ChainItem) + n_seq * 4 + sub_pairs.size() * 4 + 20 * 256;
     CK(ps.h_stage.need(stage_bytes));
     Stager sg{ctx, &ps.h_stage, ctx->copy_stream};
@@ -353,7 +353,7 @@ extern "C" int phmm_forward_batch(phmm_ctx* ctx, const phmm_batch* b, int precis
     RC(sg.upload(ps.d_pair_hap, b->h_pair_hap, (size_t)np * 4));
     RC(sg.upload(ps.d_tasks, pl.tasks.data(), pl.tasks.size() * sizeof(ShortTask)));
     RC(sg.upload(ps.d_warp_first, pl.warp_first.data(), pl.warp_first.size() * 4));
-    RC(sg.upload(ps.d_srt_read, pl.srt_ent.data(), pl.srt_ent.size() * 4));
+    RC(sg.upload(ps.d_srt_ent, pl.srt_ent.data(), pl.srt_ent.size() * 4));
     RC(sg.upload(ps.d_srt_out, pl.srt_out.data(), pl.srt_out.size() * 4));
     RC(sg.upload(ps.d_items, items.data(), items.size() * sizeof(ChainItem)));
     RC(sg.upload(ps.d_rq_enq, sub_pairs.data(), sub_pairs.size() * 4));
@@ -402,7 +402,7 @@ extern "C" int phmm_forward_batch(phmm_ctx* ctx, const phmm_batch* b, int precis
         sl.tasks = (const ShortTask*)ps.d_tasks.p;
         sl.warp_first = (const int*)ps.d_warp_first.p;
         sl.n_warps = n_warps;
-        sl.srt_ent = (const int2*)ps.d_srt_read.p;
+        sl.srt_ent = (const int2*)ps.d_srt_ent.p;
         sl.srt_out = (const int*)ps.d_srt_out.p;
         sl.out = d_out;
         sl.flags = d_flags;

@@ -59,9 +59,8 @@ void plan_short(const HostBatchView& b, const uint8_t* is_short, int N2, int tas
         for (int t = 0; t < T; t++) { const int c = hist[t][h]; hist[t][h] = (int)n_sel; n_sel += c; }
     }
     cnt[nh] = (int)n_sel;
-    if (n_sel == 0) { out->srt_read.clear(); out->srt_out.clear(); out->srt_ent.clear(); out->warp_first.push_back(0); return; }
-    if (out->srt_read.size() != (size_t)n_sel) {  // steady state: same size as the last call, nothing to (re)initialise
-        out->srt_read.resize((size_t)n_sel);
+    if (n_sel == 0) { out->srt_out.clear(); out->srt_ent.clear(); out->warp_first.push_back(0); return; }
+    if (out->srt_out.size() != (size_t)n_sel) {  // steady state: same size as the last call, nothing to (re)initialise
         out->srt_out.resize((size_t)n_sel);
         out->srt_ent.resize((size_t)n_sel * 2);
     }
@@ -71,7 +70,6 @@ void plan_short(const HostBatchView& b, const uint8_t* is_short, int N2, int tas
             if (is_short[p]) {
                 const int q = pos[b.pair_hap[p]]++;
                 const int r = b.pair_read[p];
-                out->srt_read[q] = r;
                 out->srt_out[q] = (int)p;
                 out->srt_ent[2 * (size_t)q] = (int)(TABLE_ZERO_RUN + b.read_off[r] + (int64_t)TABLE_EXTRA_ROWS * r);
                 out->srt_ent[2 * (size_t)q + 1] = (int)(b.read_off[r + 1] - b.read_off[r]) + TABLE_EXTRA_ROWS;
