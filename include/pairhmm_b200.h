@@ -66,13 +66,15 @@ typedef struct phmm_options {
      * C = 2^120; a pair is redone in fp64 iff its scaled sum is not finite or is
      * < 2^rescue_log2_threshold.  Default -90  (<=> L < 2^-210 ~ 10^-63.2). */
     int32_t rescue_log2_threshold;
-    /* haplotypes longer than this many bases use the long (CTA-chain) path; default 1280 */
+    /* haplotypes longer than this many bases (or reads longer than 4096) use the long, rescaled multi-strip path;
+     * default and maximum 1024 (= 32 lanes x 32 columns, what one warp of the short kernel covers) */
     int32_t long_min_hap_len;
     /* target number of read rows per short-path task (a task streams several reads of one
-     * haplotype through one lane group); default 3072 */
+     * haplotype through one lane group); 0 = chosen per batch between 1024 and 8192 so that the
+     * GPU still gets several waves of warps */
     int32_t task_rows;
-    /* upper bound, in bytes, for the per-read row-constant table built per launch group; batches
-     * needing more are processed in several slices.  Default 8 GiB. */
+    /* upper bound, in bytes, for the row-constant table of the short path (64 bytes per read base + 128 per
+     * read); a batch needing more fails with PHMM_E_NOMEM (split it).  Default 64 GiB. */
     int64_t max_table_bytes;
     /* non-zero: bracket every kernel family of a call with CUDA events on the caller's stream; the
      * durations appear in phmm_stats.ms_* (phmm_get_stats synchronises the last event).  Default 0. */

@@ -113,7 +113,6 @@ extern "C" int phmm_create(phmm_ctx** out, int device, const phmm_options* opt) 
     if (opt) memcpy(&ctx->opt, opt, opt->size < sizeof(phmm_options) ? opt->size : sizeof(phmm_options));
     if (ctx->opt.rescue_log2_threshold == 0) ctx->opt.rescue_log2_threshold = -90;
     if (ctx->opt.long_min_hap_len <= 0 || ctx->opt.long_min_hap_len > SHORT_MAX_K) ctx->opt.long_min_hap_len = SHORT_MAX_K;
-    if (ctx->opt.task_rows <= 0) ctx->opt.task_rows = 3072;
     if (ctx->opt.max_table_bytes <= 0) ctx->opt.max_table_bytes = (int64_t)64 << 30;
     if (ctx->opt.profile_events)
         for (int i = 0; i < 8; i++)
@@ -259,10 +258,10 @@ extern "C" int phmm_forward_batch(phmm_ctx* ctx, const phmm_batch* b, int precis
     const int strip_cols = chain_strip_cols(fp64);
     if (ctx->is_short.size() != (size_t)np) ctx->is_short.resize((size_t)np);
     std::vector<int> seq_pairs, strip_pairs, sub_pairs;  // chain kernel work lists, fp64 sub-warp list (caller pair indices)
-    int64_t cells = 0, long_cells = 0;
+    int64_t cells = 0, long_cells = 0, lane_rows = 0;  // lane_rows: sum over short pairs of read rows x lanes of the group
     int max_seq_l = 0;
     {
-        struct Part { std::vector<int> seq, strip, sub; int64_t cells = 0, long_cells = 0; int max_l = 0; };
+        struct Part { std::vector<int> seq, strip, sub; int64_t cells = 0, long_cells = 0, lane_rows = 0; int max_l = 0; };
         Part part[BATCHER_THREADS];
         const int long_k = ctx->opt.long_min_hap_len;
         uint8_t* is_short = ctx->is_short.data();
@@ -277,7 +276,7 @@ extern "C" int phmm_forward_batch(phmm_ctx* ctx, const phmm_batch* b, int precis
                 else {
                     if (fp64 && k <= RESCUE_MAX_K && l <= RESCUE_MAX_L) q.sub.push_back((int)p);
                     else if (fp64) q.seq.push_back((int)p);
-                    else sh = 1;
+                    else { sh = 1; q.lane_rows += l * ((k + SHORT_N2 - 1) / SHORT_N2); }
                     if (l > q.max_l) q.max_l = (int)l;
                 }
                 is_short[p] = sh;
@@ -287,7 +286,7 @@ extern "C" int phmm_forward_batch(phmm_ctx* ctx, const phmm_batch* b, int precis
             seq_pairs.insert(seq_pairs.end(), part[t].seq.begin(), part[t].seq.end());
             strip_pairs.insert(strip_pairs.end(), part[t].strip.begin(), part[t].strip.end());
             sub_pairs.insert(sub_pairs.end(), part[t].sub.begin(), part[t].sub.end());
-            cells += part[t].cells; long_cells += part[t].long_cells;
+            cells += part[t].cells; long_cells += part[t].long_cells; lane_rows += part[t].lane_rows;
             if (part[t].max_l > max_seq_l) max_seq_l = part[t].max_l;
         }
     }
@@ -295,7 +294,14 @@ extern "C" int phmm_forward_batch(phmm_ctx* ctx, const phmm_batch* b, int precis
     ctx->stats.cells = cells;
     ctx->stats.n_long_pairs = (int64_t)strip_pairs.size();
     ctx->stats.n_short_pairs = np - (int64_t)strip_pairs.size();
-    if (!fp64) plan_short(hv, ctx->is_short.data(), SHORT_N2, ctx->opt.task_rows, &ctx->plan);
+    // task size: as large as possible (fewer run-ins, pipeline fills and host work; 8192 rows measured best on
+    // configs[1]) while leaving at least ~6 warps of work per resident warp slot
+    int task_rows = ctx->opt.task_rows;
+    if (task_rows <= 0) {
+        const int64_t slots = (int64_t)ctx->n_sm * 12;
+        task_rows = (int)std::max<int64_t>(1024, std::min<int64_t>(8192, lane_rows / 32 / (6 * slots)));
+    }
+    if (!fp64) plan_short(hv, ctx->is_short.data(), SHORT_N2, task_rows, &ctx->plan);
     else { ctx->plan.tasks.clear(); ctx->plan.warp_first.assign(1, 0); ctx->plan.srt_out.clear(); ctx->plan.srt_ent.clear(); ctx->plan.cells = 0; ctx->plan.padded_cells = 0; }
     const ShortPlan& pl = ctx->plan;
     const int n_warps = (int)pl.warp_first.size() - 1;
