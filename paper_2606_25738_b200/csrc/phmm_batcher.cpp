@@ -162,6 +162,11 @@ void plan_short(const HostBatchView& b, const uint8_t* is_short, int N2, int tas
     }
     auto pack_range = [&](int t) {
         Part& P = part[t];
+        if (range_hi[t] > range_hi[t + 1]) {
+            const size_t n_range = (size_t)(bstart[(size_t)(range_hi[t] + 1) * 33] - bstart[(size_t)(range_hi[t + 1] + 1) * 33]);
+            P.tasks.reserve(n_range);
+            P.warp_end.reserve(n_range / 2 + 1);
+        }
         int cap = 32, bin_steps = 0;
         auto close_bin = [&]() {
             if (cap < 32) {
