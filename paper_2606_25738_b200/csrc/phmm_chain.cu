@@ -166,7 +166,7 @@ k_chain(DevBatch b, ChainLaunch p, int items_are_pairs) {
         const int r = p.pair_read[pair], h = p.pair_hap[pair];
         const int64_t ro = b.read_off[r], ho = b.hap_off[h];
         const int l = (int)(b.read_off[r + 1] - ro), k = (int)(b.hap_off[h + 1] - ho);
-        const int n_ent = l + TABLE_EXTRA_ROWS;  // run-in entry, rows 1..l, flush entry
+        const int n_ent = l + CHAIN_EXTRA_ROWS;  // run-in entry, rows 1..l, flush entry
         const int nstrips = (k + 32 * N2 - 1) / (32 * N2);
         const int nblk = (n_ent + 31) / 32;  // boundary blocks per buffer
         const int st_lo = strip < 0 ? 0 : strip, st_hi = strip < 0 ? nstrips : strip + 1;

@@ -52,14 +52,22 @@ template <typename T> struct Entry2 {
     typename W2<T>::V gam, A, C, G;
     T pmx, pxx, pmy, pxy;
     uint32_t metaX, metaY;
+    uint32_t r2;  // SC only: the fp16 base codes of (.x's row, .y's row), as the table stores them
 };
 
 // HS (fp32 only): take the Eq.3 predicates of both halves from one HSETP2 on per-column fp16 base codes instead
 // of two bit tests of the match word: 16 fewer ALU instructions per step, 12 more registers.
-template <typename T, int NV, bool HS = false> struct Lane2 {
+// SC (with HS): Eq.4 comes out of the running sum s instead of a per-lane summation of J.  The stream then carries a
+// "sum entry" behind the last row (phmm_rowconst.cuh): the last row leaves T[x+1] = M_{l,x} + I_{l,x} (A := 1, C := 0),
+// and the sum entry has gamma := 1, pm := 0, px := 1 and base code 0, so that U = T on every column whose code is not
+// 0 and the chain s = s + U adds them up across the whole lane group.  Columns behind the haplotype carry code 0
+// (U = 0) except the first one, which holds T = (M+I) of the last real column and carries code 5; a haplotype 'N'
+// carries code 6 (both match no read base).  No divergent per-lane summation, no third value handed from lane to lane.
+template <typename T, int NV, bool HS = false, bool SC = false> struct Lane2 {
     typedef W2<T> P;
     typedef typename P::V V;
     static_assert(NV <= 16, "one 32-bit match word per base: 16 columns per half");
+    static_assert(!SC || HS, "the sum entry selects by base code");
 
     V Tt[NV], J[NV];
     V outT, outS;              // what dropped out on the right in the last step: (.x's, .y's)
@@ -77,6 +85,16 @@ template <typename T, int NV, bool HS = false> struct Lane2 {
 
     // hap: pointer to the haplotype bytes, k its length, j0 = 0-based first column of this thread
     __device__ __forceinline__ void load_hap(const uint8_t* __restrict__ hap, int k, int j0) {
+        if constexpr (SC) {
+#pragma unroll
+            for (int x = 0; x < NV; x++) {
+                const int jx = j0 + x, jy = j0 + NV + x;
+                const uint32_t cx = jx < k ? col_code(hap[jx]) : (jx == k ? 0x4500u : 0u);
+                const uint32_t cy = jy < k ? col_code(hap[jy]) : (jy == k ? 0x4500u : 0u);
+                h2[x] = cx | (cy << 16);
+            }
+            return;
+        }
 #pragma unroll
         for (int c = 0; c < 4; c++) hm[c] = 0;
         nvx = min(max(k - j0, 0), NV);
@@ -110,6 +128,10 @@ template <typename T, int NV, bool HS = false> struct Lane2 {
     static __device__ __forceinline__ uint32_t half_code(int c) {  // fp16 bit pattern of the number c + 1
         return (uint32_t)((0x4400420040003C00ull >> (16 * c)) & 0xffffull);
     }
+    static __device__ __forceinline__ uint32_t col_code(uint8_t b) {  // SC: fp16 1..4 for A,C,G,T; 6 for anything else
+        const int c = base_code(b);
+        return c < 4 ? half_code(c) : 0x4600u;
+    }
 
     // One systolic step.  (inS, inT, inSig): the left neighbour thread's (.y) outS, outT, sigY as they stand
     // after ITS last step, or the column-0 boundary for the first lane of a group (Eq.1 under reading G1:
@@ -119,11 +141,14 @@ template <typename T, int NV, bool HS = false> struct Lane2 {
         const V tgrab = P::mk(inT, outT.x);        // T[0] of the NEXT step
         // match word of this step: the read base of .x's row picks the low half, that of .y's row the high half;
         // consecutive single-bit tests of one register let ptxas turn 7 of them into one R2P
-        const uint32_t wx01 = (E.metaX & 1u) ? hm[1] : hm[0], wx23 = (E.metaX & 1u) ? hm[3] : hm[2];
-        const uint32_t wy01 = (E.metaY & 1u) ? hm[1] : hm[0], wy23 = (E.metaY & 1u) ? hm[3] : hm[2];
-        const uint32_t wx = (E.metaX & 2u) ? wx23 : wx01, wy = (E.metaY & 2u) ? wy23 : wy01;
-        const uint32_t mw = (wx & 0xffffu) | (wy & 0xffff0000u);
-        const uint32_t r2 = HS ? (half_code(E.metaX & 3u) | (half_code(E.metaY & 3u) << 16)) : 0u;
+        uint32_t mw = 0;
+        if constexpr (!HS) {
+            const uint32_t wx01 = (E.metaX & 1u) ? hm[1] : hm[0], wx23 = (E.metaX & 1u) ? hm[3] : hm[2];
+            const uint32_t wy01 = (E.metaY & 1u) ? hm[1] : hm[0], wy23 = (E.metaY & 1u) ? hm[3] : hm[2];
+            const uint32_t wx = (E.metaX & 2u) ? wx23 : wx01, wy = (E.metaY & 2u) ? wy23 : wy01;
+            mw = (wx & 0xffffu) | (wy & 0xffff0000u);
+        }
+        const uint32_t r2 = SC ? E.r2 : HS ? (half_code(E.metaX & 3u) | (half_code(E.metaY & 3u) << 16)) : 0u;
         auto prior = [&](int x) {                  // Eq.3: one select per half
             if constexpr (HS && sizeof(T) == 4) {  // one HSETP2 yields both halves' predicates
                 float a, b;
@@ -147,6 +172,7 @@ template <typename T, int NV, bool HS = false> struct Lane2 {
             U = Un;
         }
         outS = s;
+        if constexpr (SC) return;  // Eq.4 is the s that leaves the group's last lane on the sum entry
         // Eq.4: on the last row G = 1 and gi_{l+1} := 1, so J now holds M_l + I_l; sum this half's real columns
         if ((E.metaX | E.metaY) & META_LAST) {
             if (E.metaX & META_LAST) {

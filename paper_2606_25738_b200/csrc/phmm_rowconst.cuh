@@ -9,6 +9,10 @@
 //              G = gamma_{i+1} g_{i+2}/g_{i+1};  on the last row gi_{l+1} := 1, A := C := 0, G := 1, meta LAST, so
 //              that the step leaves J = M_l + I_l, the summand of Eq.4.
 //   e = l+1    flush entry, all zero: gives the .y half (one entry behind) its step for row l and zeroes J.
+// With sum_entry (the short path, Lane2<.., SC>; l + 3 entries): the last row has A := 1, C := 0, G := 0 instead, which
+// leaves T[x+1] = M_{l,x} + I_{l,x};  e = l+1 is the SUM entry (gamma := 1, pm := 0, px := 1, base code 0, all else 0):
+// U = T on every column with a non-zero code, so the chain s = s + U leaves Eq.4's sum in the group's last lane;
+// e = l+2 is the all-zero flush entry, which clears the J = U the sum entry left behind.
 // Constants are formed in double from the 10^(-q/10) table and rounded once to the working type
 // ("q32"/"q64" tables; Listing 2 :293-295 for which qualities enter which transition).
 #pragma once
@@ -19,8 +23,13 @@ namespace phmm {
 
 struct RowC { double gam, A, C, G, pm, px; uint32_t meta; };
 
-__device__ __forceinline__ RowC row_constants(const DevBatch& b, const double* __restrict__ lut, int64_t off, int l, int e) {
+__device__ __forceinline__ RowC row_constants(const DevBatch& b, const double* __restrict__ lut, int64_t off, int l, int e,
+                                             bool sum_entry = false) {
     RowC c = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0u};
+    if (sum_entry && e == l + 1) {
+        c.gam = 1.0; c.px = 1.0; c.meta = META_SUM;
+        return c;
+    }
     if (e == 0) {
         c.gam = 1.0; c.C = 1.0 - lut[b.qual_gcp[off]]; c.meta = META_FIRST;
     } else if (e >= 1 && e <= l) {
@@ -38,6 +47,8 @@ __device__ __forceinline__ RowC row_constants(const DevBatch& b, const double* _
             c.A = (1.0 - io1 - de1) / gin;
             c.C = g1 * lut[b.qual_del[off + i - 1]] / gin;
             c.G = lut[b.qual_gcp[off + i]] * g2 / g1;
+        } else if (sum_entry) {
+            c.A = 1.0;
         } else {
             c.G = 1.0;
         }

@@ -12,9 +12,6 @@
 #ifndef SHORT_L2_PREFETCH
 #define SHORT_L2_PREFETCH 1  // table loads carry the L2 256-byte prefetch hint: +0.6 %
 #endif
-#ifndef SHORT_HSETP2
-#define SHORT_HSETP2 1  // measured: 2.78 vs 2.60 TCUPS
-#endif
 #ifndef SHORT_FETCH_AHEAD
 #define SHORT_FETCH_AHEAD 2  // with the HSETP2 engine: 3 CTAs x 168 registers + two steps ahead (2.86) beats 4 x 128 + one (2.78)
 #endif
@@ -27,7 +24,9 @@ namespace phmm {
 // ------------------------------------------------------------------ a1: row-constant table
 // Each 64-byte table entry holds the constants of entry e (for the .x half) and of entry e-1 (for .y; zero
 // for e = 0), already paired the way FFMA2 wants them:
-//   float4 0: gamma.x gamma.y A.x A.y | 1: C.x C.y G.x G.y | 2: pm.x px.x pm.y px.y | 3: meta.x meta.y 0 0
+//   float4 0: gamma.x gamma.y A.x A.y | 1: C.x C.y G.x G.y | 2: pm.x px.x pm.y px.y | 3: word 0 0 0
+// word = what HSETP2 compares with the per-column codes, plus the flags: bits 10-14 / 26-30 the read base of e / e-1 as an
+// fp16 number (A,C,G,T = 1..4; 0 on entries that are not read rows), bits 0-7 / 16-23 the META_ flags of e / e-1.
 // The table starts with TABLE_ZERO_RUN all-zero entries (what idle lanes fetch); read r's run starts at
 // entry TABLE_ZERO_RUN + read_off[r] + TABLE_EXTRA_ROWS r.  Constants are formed in double from the
 // 10^(-q/10) table and rounded once ("q32" table; Listing 2 :293-295 for which
@@ -39,6 +38,11 @@ namespace phmm {
 constexpr int TABLE_CHUNK_STRIDE = 32;  // float4 units between the chunk planes of a block
 __host__ __device__ __forceinline__ int64_t table_slot(int64_t pos) {  // float4 index of chunk 0 of entry pos
     return (pos >> 5) * 128 + (pos & 1) * 16 + ((pos >> 1) & 15);
+}
+
+__device__ __forceinline__ uint32_t entry_word(const RowC& c, bool is_row) {  // 16 bits: fp16 base code | flags
+    const uint32_t code = is_row ? (uint32_t)((0x4400420040003C00ull >> (16 * (c.meta & META_CODE_MASK))) & 0xffffull) : 0u;
+    return code | (c.meta & ~META_CODE_MASK & 0xffu);
 }
 
 __global__ void __launch_bounds__(256) k_table_f32(DevBatch b, const double* __restrict__ lut, float* __restrict__ table) {
@@ -53,12 +57,12 @@ __global__ void __launch_bounds__(256) k_table_f32(DevBatch b, const double* __r
     float4* dst = reinterpret_cast<float4*>(table);
     const int64_t first = TABLE_ZERO_RUN + off + TABLE_EXTRA_ROWS * r;
     for (int e = lane; e < l + TABLE_EXTRA_ROWS; e += 32) {
-        const RowC x = row_constants(b, lut, off, l, e), y = row_constants(b, lut, off, l, e - 1);
+        const RowC x = row_constants(b, lut, off, l, e, true), y = row_constants(b, lut, off, l, e - 1, true);
         float4* d = dst + table_slot(first + e);
         d[0 * TABLE_CHUNK_STRIDE] = make_float4((float)x.gam, (float)y.gam, (float)x.A, (float)y.A);
         d[1 * TABLE_CHUNK_STRIDE] = make_float4((float)x.C, (float)y.C, (float)x.G, (float)y.G);
         d[2 * TABLE_CHUNK_STRIDE] = make_float4((float)x.pm, (float)x.px, (float)y.pm, (float)y.px);
-        d[3 * TABLE_CHUNK_STRIDE] = make_float4(__uint_as_float(x.meta), __uint_as_float(y.meta), 0.f, 0.f);
+        d[3 * TABLE_CHUNK_STRIDE] = make_float4(__uint_as_float(entry_word(x, e >= 1 && e <= l) | (entry_word(y, e >= 2 && e <= l + 1) << 16)), 0.f, 0.f, 0.f);
     }
 }
 
@@ -90,11 +94,17 @@ __device__ __forceinline__ float4 ldg_pf(const float4* p) {
     return v;
 }
 
-struct RawEntry { float4 a, b, c; uint2 m; };
+__device__ __forceinline__ uint32_t ldg_pf_u32(const uint32_t* p) {
+    uint32_t v;
+    asm volatile("ld.global.nc.L2::256B.b32 %0, [%1];" : "=r"(v) : "l"(p));
+    return v;
+}
+
+struct RawEntry { float4 a, b, c; uint32_t w; };
 
 template <int NV>
 __global__ void __launch_bounds__(SHORT_WARPS_PER_CTA * 32, SHORT_MIN_CTAS) k_short_f32(DevBatch b, ShortLaunch p) {
-    typedef Lane2<float, NV, SHORT_HSETP2 != 0> L;
+    typedef Lane2<float, NV, true, true> L;  // HSETP2 predicates (2.78 vs 2.60 TCUPS with bit tests), Eq.4 through the s chain
     constexpr int N2 = 2 * NV;
     const int warp = blockIdx.x * SHORT_WARPS_PER_CTA + (threadIdx.x >> 5);
     if (warp >= p.n_warps) return;
@@ -131,6 +141,7 @@ __global__ void __launch_bounds__(SHORT_WARPS_PER_CTA * 32, SHORT_MIN_CTAS) k_sh
     const int lg = ti < 0 ? 0 : lane - m_start;
     const bool is_first = (ti < 0) || lg == 0;
     const bool is_last = (ti >= 0) && lg == m_g - 1;
+    const bool full_last = m_k == m_g * N2;  // no column behind the haplotype's last one
 
     // ---- number of steps of this warp: the last lane's .y half finishes the last entry of its stream
     int steps = (ti < 0) ? 0 : m_rows + TABLE_EXTRA_ROWS * m_np + 2 * m_g - 1;
@@ -164,12 +175,12 @@ __global__ void __launch_bounds__(SHORT_WARPS_PER_CTA * 32, SHORT_MIN_CTAS) k_sh
         r.a = ldg_pf(e);
         r.b = ldg_pf(e + TABLE_CHUNK_STRIDE);
         r.c = ldg_pf(e + 2 * TABLE_CHUNK_STRIDE);
-        { const float4 t = ldg_pf(e + 3 * TABLE_CHUNK_STRIDE); r.m = make_uint2(__float_as_uint(t.x), __float_as_uint(t.y)); }
+        r.w = ldg_pf_u32(reinterpret_cast<const uint32_t*>(e + 3 * TABLE_CHUNK_STRIDE));
 #else
         r.a = __ldg(e);
         r.b = __ldg(e + TABLE_CHUNK_STRIDE);
         r.c = __ldg(e + 2 * TABLE_CHUNK_STRIDE);
-        r.m = __ldg(reinterpret_cast<const uint2*>(e + 3 * TABLE_CHUNK_STRIDE));
+        r.w = __ldg(reinterpret_cast<const uint32_t*>(e + 3 * TABLE_CHUNK_STRIDE));
 #endif
     };
 
@@ -180,19 +191,21 @@ __global__ void __launch_bounds__(SHORT_WARPS_PER_CTA * 32, SHORT_MIN_CTAS) k_sh
         E.gam = make_float2(r.a.x, r.a.y); E.A = make_float2(r.a.z, r.a.w);
         E.C = make_float2(r.b.x, r.b.y); E.G = make_float2(r.b.z, r.b.w);
         E.pmx = r.c.x; E.pxx = r.c.y; E.pmy = r.c.z; E.pxy = r.c.w;
-        E.metaX = r.m.x; E.metaY = r.m.y;
+        E.metaX = r.w & 0xffu; E.metaY = (r.w >> 16) & 0xffu;
+        E.r2 = r.w & 0xff00ff00u;
+        // what the left neighbour's .y half handed out in its last step; a haplotype that fills its last lane completely
+        // has its last column's M+I there when the sum entry arrives, not in a T of its own
+        const float prevT = ln.outT.y;
         float inS = __shfl_up_sync(PHMM_FULL, ln.outS.y, 1);
-        float inT = __shfl_up_sync(PHMM_FULL, ln.outT.y, 1);
-        float inSig = __shfl_up_sync(PHMM_FULL, ln.sigY, 1);
+        float inT = __shfl_up_sync(PHMM_FULL, prevT, 1);
         if (is_first) {  // column-0 boundary, Eq.1
             const bool f = (E.metaX & META_FIRST) != 0;
             inS = f ? Cok : 0.f;
             inT = f ? E.C.x * Cok : 0.f;
-            inSig = 0.f;
         }
-        ln.step(E, inS, inT, inSig);
-        if (is_last && (E.metaY & META_LAST)) {
-            const float sg = ln.sigY;
+        ln.step(E, inS, inT, 0.f);
+        if (is_last && (E.metaY & META_SUM)) {  // Eq.4: the s chain has collected M_l + I_l of every column
+            const float sg = full_last ? ln.outS.y + prevT : ln.outS.y;
             const int pair = p.srt_out[m_first + nout];
             nout++;
             if (isfinite(sg) && sg >= p.rescue_thr) {
