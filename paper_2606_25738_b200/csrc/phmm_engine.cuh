@@ -93,35 +93,35 @@ template <typename T, int NV, bool HS = false, bool SC = false> struct Lane2 {
                 const uint32_t cy = jy < k ? col_code(hap[jy]) : (jy == k ? 0x4500u : 0u);
                 h2[x] = cx | (cy << 16);
             }
-            return;
-        }
+        } else {
 #pragma unroll
-        for (int c = 0; c < 4; c++) hm[c] = 0;
-        nvx = min(max(k - j0, 0), NV);
-        nvy = min(max(k - j0 - NV, 0), NV);
-#pragma unroll
-        for (int x = 0; x < NV; x++) {
-            if (x < nvx) {
-                const int c = base_code(hap[j0 + x]);
-#pragma unroll
-                for (int q = 0; q < 4; q++) hm[q] |= (c == q ? 1u : 0u) << x;
-            }
-            if (x < nvy) {
-                const int c = base_code(hap[j0 + NV + x]);
-#pragma unroll
-                for (int q = 0; q < 4; q++) hm[q] |= (c == q ? 1u : 0u) << (16 + x);
-            }
-        }
-        if (HS) {
+            for (int c = 0; c < 4; c++) hm[c] = 0;
+            nvx = min(max(k - j0, 0), NV);
+            nvy = min(max(k - j0 - NV, 0), NV);
 #pragma unroll
             for (int x = 0; x < NV; x++) {
-                uint32_t v = 0;
+                if (x < nvx) {
+                    const int c = base_code(hap[j0 + x]);
 #pragma unroll
-                for (int q = 0; q < 4; q++) {
-                    if (hm[q] & (1u << x)) v |= half_code(q);
-                    if (hm[q] & (1u << (16 + x))) v |= half_code(q) << 16;
+                    for (int q = 0; q < 4; q++) hm[q] |= (c == q ? 1u : 0u) << x;
                 }
-                h2[x] = v;
+                if (x < nvy) {
+                    const int c = base_code(hap[j0 + NV + x]);
+#pragma unroll
+                    for (int q = 0; q < 4; q++) hm[q] |= (c == q ? 1u : 0u) << (16 + x);
+                }
+            }
+            if (HS) {
+#pragma unroll
+                for (int x = 0; x < NV; x++) {
+                    uint32_t v = 0;
+#pragma unroll
+                    for (int q = 0; q < 4; q++) {
+                        if (hm[q] & (1u << x)) v |= half_code(q);
+                        if (hm[q] & (1u << (16 + x))) v |= half_code(q) << 16;
+                    }
+                    h2[x] = v;
+                }
             }
         }
     }

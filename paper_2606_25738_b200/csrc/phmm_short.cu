@@ -12,11 +12,8 @@
 #ifndef SHORT_L2_PREFETCH
 #define SHORT_L2_PREFETCH 1  // table loads carry the L2 256-byte prefetch hint: +0.6 %
 #endif
-#ifndef SHORT_FETCH_AHEAD
-#define SHORT_FETCH_AHEAD 2  // with the HSETP2 engine: 3 CTAs x 168 registers + two steps ahead (2.86) beats 4 x 128 + one (2.78)
-#endif
 #ifndef SHORT_MIN_CTAS
-#define SHORT_MIN_CTAS 3  // resident CTAs per SM the register allocation is held to (3 x 128 threads -> <= 168 registers)
+#define SHORT_MIN_CTAS 3  // resident CTAs per SM the register allocation is held to (3 x 128 threads -> <= 168 registers); 4 x 128 registers spills: 3.17 vs 3.36 TCUPS
 #endif
 
 namespace phmm {
@@ -78,8 +75,8 @@ cudaError_t launch_lut_table(const DevBatch& b, const double* lut, float* table,
 // Per lane, the .x half walks its task's stream of table entries (run of read 1, run of read 2, ...) starting
 // 2*lg steps after the group's first lane.  While it waits, and after its stream has ended, a lane walks the
 // zero run at the start of the table (all-zero constants decay T and J to 0), so the fetch needs no special
-// cases.  Entries are loaded SHORT_FETCH_AHEAD steps ahead into rotating register sets (the step loop is unrolled
-// by the number of sets, so no register is ever copied).
+// cases.  Entries are loaded one step ahead into two alternating register sets (the step loop is unrolled by two, so
+// no register is ever copied).
 struct Cursor {
     int pos, end;        // next entry to fetch, one past the last entry of the current run
     int npos, nend;      // the run after it: the next read of the task, or the zero run
@@ -167,9 +164,11 @@ __global__ void __launch_bounds__(SHORT_WARPS_PER_CTA * 32, SHORT_MIN_CTAS) k_sh
     };
     c.pos = TABLE_ZERO_RUN - 2 * lg; c.end = TABLE_ZERO_RUN;  // 2*lg idle steps before the stream starts
     load_next();
-    auto fetch = [&](RawEntry& r) {
+    // dep: the word of the entry the CURRENT step works on.  Its top bit is never set, but the address now depends on
+    // it, which keeps the loads behind the wait for that entry (see the step loop).
+    auto fetch = [&](RawEntry& r, uint32_t dep) {
         if (c.pos == c.end) { c.pos = c.npos; c.end = c.nend; load_next(); }
-        const float4* e = tab + table_slot(c.pos);
+        const float4* e = tab + (table_slot(c.pos) + (dep >> 31));
         c.pos++;
 #if SHORT_L2_PREFETCH
         r.a = ldg_pf(e);
@@ -219,28 +218,19 @@ __global__ void __launch_bounds__(SHORT_WARPS_PER_CTA * 32, SHORT_MIN_CTAS) k_sh
             }
         }
     };
-#if SHORT_FETCH_AHEAD == 2
-    RawEntry eA, eB, eC;  // entries are loaded two steps ahead into three rotating register sets
-    fetch(eA);
-    fetch(eB);
-    for (int s = 0; s < steps; s += 3) {  // up to two extra all-idle steps at the end, which are harmless
-        fetch(eC);
-        one_step(eA);
-        fetch(eA);
-        one_step(eB);
-        fetch(eB);
-        one_step(eC);
-    }
-#else
+    // ptxas tracks every table load with ONE scoreboard, so the first use of a loaded entry waits for all loads in
+    // flight, the newest included (seen in the SASS control codes; with three register sets and two steps of fetch-ahead
+    // one step in three stalled for a full memory latency: 10 % of the stall samples).  Each step therefore makes the
+    // address of the next entry depend on its own entry's word (loaded one step ago), so the loads are issued BEHIND the
+    // wait and the wait never covers loads younger than a whole step: 3.31 -> 3.36 TCUPS, 4 fewer registers.
     RawEntry eA, eB;
-    fetch(eA);
+    fetch(eA, 0u);
     for (int s = 0; s < steps; s += 2) {  // an odd step count runs one extra all-idle step, which is harmless
-        fetch(eB);
+        fetch(eB, eA.w);
         one_step(eA);
-        fetch(eA);
+        fetch(eA, eB.w);
         one_step(eB);
     }
-#endif
 }
 
 cudaError_t launch_short_f32(const DevBatch& b, const ShortLaunch& p, cudaStream_t st) {

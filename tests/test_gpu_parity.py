@@ -282,6 +282,32 @@ def test_n_bases_match_nothing_else(B, ctx):
     ref = oracle.forward_batch(b)
     assert np.max(np.abs(out - ref)) <= TOL64
     assert out[0] < out[2] and out[1] < out[2]
+    out32, _ = run(B, ctx, b, B.PHMM_FP32_RESCUE)
+    assert np.max(np.abs(out32 - ref)) <= TOL32
+
+
+def test_sum_entry_column_codes(B, ctx):
+    """The short kernel takes Eq.4 from the running-sum chain on a "sum entry" that selects columns by their base
+    code (phmm_engine.cuh, SC): haplotypes that fill their last lane exactly (k = 32, 64, 96), that end one column
+    short of it or one past it, with an N as last / first / middle column."""
+    rng = np.random.default_rng(25)
+    reads, haps, pairs = [], [], []
+    for k in (31, 32, 33, 64, 95, 96, 97, 160):
+        for variant in range(3):
+            hap = list(_rand_seq(rng, k))
+            if variant == 1:
+                hap[-1] = "N"
+            if variant == 2:
+                hap[0] = "N"; hap[k // 2] = "N"
+            hap = "".join(hap)
+            for l in (1, 7, 30):
+                s = int(rng.integers(0, k - l + 1))
+                pairs.append((hap[s:s + l].replace("N", "A"), hap, list(rng.integers(8, 41, l)), list(rng.integers(20, 50, l)),
+                              list(rng.integers(20, 50, l)), 10))
+    b = W.from_strings(pairs)
+    out, fl, ref = check(B, ctx, b, B.PHMM_FP32_RESCUE)
+    assert not np.any(fl & B.PHMM_FLAG_RESCUED)  # all of these must have come out of the fp32 kernel itself
+    check(B, ctx, b, B.PHMM_FP64, ref=ref)
 
 
 def test_constant_quals_long_read_fp32_error(B, ctx):
