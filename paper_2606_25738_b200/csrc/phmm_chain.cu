@@ -36,7 +36,7 @@ namespace phmm {
 constexpr int RING = 128;  // row-constant ring per warp (entries); covers 63 entries of skew + two 32-entry blocks
 
 template <typename T> struct Rec {  // boundary block of 32 stream entries, SoA
-    T S[32], Tn[32], Sig[32];
+    T S[32], Tn[32];
     int ex[32];
 };
 
@@ -106,7 +106,6 @@ __device__ __forceinline__ int warp_max_i(int m) {
 
 template <typename T, int NV, typename LN> __device__ __forceinline__ T lane_max(const LN& ln) {
     T m = Fx<T>::fmax_(Fx<T>::fmax_(ln.outS.x, ln.outS.y), Fx<T>::fmax_(ln.outT.x, ln.outT.y));
-    m = Fx<T>::fmax_(m, Fx<T>::fmax_(ln.sigX, ln.sigY));
 #pragma unroll
     for (int x = 0; x < NV; x++) {
         m = Fx<T>::fmax_(m, Fx<T>::fmax_(ln.Tt[x].x, ln.Tt[x].y));
@@ -127,14 +126,12 @@ template <typename T, int NV, typename LN> __device__ __forceinline__ void lane_
     }
     ln.outS = P::mul(P::mul(ln.outS, F1), F2);
     ln.outT = P::mul(P::mul(ln.outT, F1), F2);
-    ln.sigX = ln.sigX * f1 * f2;
-    ln.sigY = ln.sigY * f1 * f2;
 }
 
 template <typename T, int NV, int WPC, int MINB>
 __global__ void __launch_bounds__(WPC * 32, MINB)
 k_chain(DevBatch b, ChainLaunch p, int items_are_pairs) {
-    typedef Lane2<T, NV, (CHAIN_HSETP2 != 0) && sizeof(T) == 4 && MINB == 3> L;  // HSETP2 only where the 12 extra registers do not spill
+    typedef Lane2<T, NV, (CHAIN_HSETP2 != 0) && sizeof(T) == 4 && MINB == 3, true> L;  // HSETP2 only where the 12 extra registers do not spill
     typedef RingFmt<T> RF;
     typedef typename W2<T>::V V;
     constexpr int N2 = 2 * NV;
@@ -166,8 +163,8 @@ k_chain(DevBatch b, ChainLaunch p, int items_are_pairs) {
         const int r = p.pair_read[pair], h = p.pair_hap[pair];
         const int64_t ro = b.read_off[r], ho = b.hap_off[h];
         const int l = (int)(b.read_off[r + 1] - ro), k = (int)(b.hap_off[h + 1] - ho);
-        const int n_ent = l + CHAIN_EXTRA_ROWS;  // run-in entry, rows 1..l, flush entry
-        const int nstrips = (k + 32 * N2 - 1) / (32 * N2);
+        const int n_ent = l + CHAIN_EXTRA_ROWS;  // run-in entry, rows 1..l, sum entry, flush entry
+        const int nstrips = k / (32 * N2) + 1;  // always one column behind the haplotype: the sum entry finds (M+I) of column k there
         const int nblk = (n_ent + 31) / 32;  // boundary blocks per buffer
         const int st_lo = strip < 0 ? 0 : strip, st_hi = strip < 0 ? nstrips : strip + 1;
         const T Cok = (T)(ldexp(1.0, p.log2C) / (double)k);
@@ -207,7 +204,7 @@ k_chain(DevBatch b, ChainLaunch p, int items_are_pairs) {
                         // ---- a1: constants of entries s..s+31, one per lane; .x fields to the entry's own slot,
                         //      .y fields to the next entry's slot (whose .y half runs one entry behind)
                         const int e = s + lane;
-                        const RowC c = row_constants(b, p.lut, ro, l, e < n_ent ? e : -1);
+                        const RowC c = row_constants(b, p.lut, ro, l, e < n_ent ? e : -1, true);
                         T* lo = rg + ring_word(e) * RF::SPW;
                         T* hi = rg + ring_word(e + 1) * RF::SPW;
                         constexpr int PL = RING * RF::SPW;  // scalars per chunk plane
@@ -227,8 +224,8 @@ k_chain(DevBatch b, ChainLaunch p, int items_are_pairs) {
                         }
                         {
                             const int a0 = RF::meta_at(0), a1 = RF::meta_at(1);
-                            lo[(a0 / RF::SPW) * PL + a0 % RF::SPW] = RF::meta_val(c.meta);
-                            hi[(a1 / RF::SPW) * PL + a1 % RF::SPW] = RF::meta_val(c.meta);
+                            lo[(a0 / RF::SPW) * PL + a0 % RF::SPW] = RF::meta_val(entry_word16(c));
+                            hi[(a1 / RF::SPW) * PL + a1 % RF::SPW] = RF::meta_val(entry_word16(c));
                         }
                     }
                     // ---- incoming boundary block for entries s..s+31 (lane 0 consumes entry s at step s)
@@ -239,7 +236,7 @@ k_chain(DevBatch b, ChainLaunch p, int items_are_pairs) {
                             while (ld_acquire(inprog) < need) __nanosleep(64);
                         }
                         const Rec<T>* src = inb + (s >> 5);
-                        RI.S[lane] = src->S[lane]; RI.Tn[lane] = src->Tn[lane]; RI.Sig[lane] = src->Sig[lane];
+                        RI.S[lane] = src->S[lane]; RI.Tn[lane] = src->Tn[lane];
                         RI.ex[lane] = src->ex[lane];
                     }
                     // ---- a8: block-floating event of this thread
@@ -274,27 +271,27 @@ k_chain(DevBatch b, ChainLaunch p, int items_are_pairs) {
                         E.pmx = pa.x; E.pxx = pa.y; E.pmy = pb.x; E.pxy = pb.y;
                         E.metaX = RF::meta_get(mm.x); E.metaY = RF::meta_get(mm.y);
                     }
+                    E.r2 = (E.metaX & 0xff00u) | ((E.metaY & 0xff00u) << 16);
                 }
                 // ---- left boundary: neighbour lane (shuffle), first strip (Eq.1 injection) or boundary block
-                T inS = shfl_up1<T>(ln.outS.y), inT = shfl_up1<T>(ln.outT.y), inSig = shfl_up1<T>(ln.sigY);
+                T inS = shfl_up1<T>(ln.outS.y), inT = shfl_up1<T>(ln.outT.y);
                 int exL = __shfl_up_sync(PHMM_FULL, ex, 1);
                 if (lane == 0) {
                     if (has_in) {
                         const int q = s & 31;
                         const bool ok = s < n_ent;
-                        inS = ok ? RI.S[q] : (T)0; inT = ok ? RI.Tn[q] : (T)0; inSig = ok ? RI.Sig[q] : (T)0;
+                        inS = ok ? RI.S[q] : (T)0; inT = ok ? RI.Tn[q] : (T)0;
                         exL = ok ? RI.ex[q] : ex;
                     } else {
                         const bool f = (E.metaX & META_FIRST) != 0;  // Eq.1: only the run-in entry injects, at exponent 0
                         inS = f ? Cok : (T)0;
                         inT = f ? E.C.x * Cok : (T)0;
-                        inSig = (T)0;
                         exL = 0;
                     }
                 }
                 // ---- bring the incoming values to this thread's exponent (exact power-of-two multiply)
                 {
-                    const T mi = Fx<T>::fmax_(Fx<T>::fmax_(inS, inT), inSig);
+                    const T mi = Fx<T>::fmax_(inS, inT);
                     if (zero) {
                         if (mi > (T)0) { ex = exL; zero = false; }
                     } else if (mi > (T)0 && Fx<T>::ilogb(mi) + exL - ex > Win<T>::TGT + Win<T>::UP) {
@@ -305,24 +302,24 @@ k_chain(DevBatch b, ChainLaunch p, int items_are_pairs) {
                     const int d = exL - ex;
                     if (d >= -Fx<T>::CLAMP1 && d <= Fx<T>::CLAMP1) {  // the usual case: one exact factor
                         const T f = Fx<T>::exp2i(d);
-                        inS *= f; inT *= f; inSig *= f;
+                        inS *= f; inT *= f;
                     } else {  // |d| beyond one factor's exponent range
-                        inS = scale_pow2<T>(inS, d); inT = scale_pow2<T>(inT, d); inSig = scale_pow2<T>(inSig, d);
+                        inS = scale_pow2<T>(inS, d); inT = scale_pow2<T>(inT, d);
                     }
                 }
-                ln.step(E, inS, inT, inSig);
+                ln.step(E, inS, inT, (T)0);
                 // ---- right boundary of the strip: lane 31's .y half has just finished entry s - 63
                 const int eo = s - 63;
                 if (eo >= 0 && eo < n_ent) {
                     if (has_out) {
                         if (lane == 31) {
                             const int q = eo & 31;
-                            RO.S[q] = ln.outS.y; RO.Tn[q] = ln.outT.y; RO.Sig[q] = ln.sigY; RO.ex[q] = ex;
+                            RO.S[q] = ln.outS.y; RO.Tn[q] = ln.outT.y; RO.ex[q] = ex;
                         }
                         if ((eo & 31) == 31 || eo == n_ent - 1) {
                             __syncwarp();
                             Rec<T>* dst = outb + (eo >> 5);
-                            dst->S[lane] = RO.S[lane]; dst->Tn[lane] = RO.Tn[lane]; dst->Sig[lane] = RO.Sig[lane];
+                            dst->S[lane] = RO.S[lane]; dst->Tn[lane] = RO.Tn[lane];
                             dst->ex[lane] = RO.ex[lane];
                             __syncwarp();
                             if (outprog && lane == 0) {
@@ -331,8 +328,8 @@ k_chain(DevBatch b, ChainLaunch p, int items_are_pairs) {
                             }
                             __syncwarp();
                         }
-                    } else if (eo == l && lane == 31) {  // entry l = the read's last row: Eq.4, log10 in double
-                        p.out[pair] = log10((double)ln.sigY) + ((double)ex - (double)p.log2C) * LOG10_2;
+                    } else if (eo == l + 1 && lane == 31) {  // the sum entry: s has collected Eq.4; log10 in double
+                        p.out[pair] = log10((double)ln.outS.y) + ((double)ex - (double)p.log2C) * LOG10_2;
                         if (p.flags) p.flags[pair] = p.flag_bits;
                     }
                 }

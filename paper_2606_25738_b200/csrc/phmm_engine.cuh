@@ -57,22 +57,22 @@ template <typename T> struct Entry2 {
 
 // HS (fp32 only): take the Eq.3 predicates of both halves from one HSETP2 on per-column fp16 base codes instead
 // of two bit tests of the match word: 16 fewer ALU instructions per step, 12 more registers.
-// SC (with HS): Eq.4 comes out of the running sum s instead of a per-lane summation of J.  The stream then carries a
+// SC: Eq.4 comes out of the running sum s instead of a per-lane summation of J.  The stream then carries a
 // "sum entry" behind the last row (phmm_rowconst.cuh): the last row leaves T[x+1] = M_{l,x} + I_{l,x} (A := 1, C := 0),
-// and the sum entry has gamma := 1, pm := 0, px := 1 and base code 0, so that U = T on every column whose code is not
-// 0 and the chain s = s + U adds them up across the whole lane group.  Columns behind the haplotype carry code 0
-// (U = 0) except the first one, which holds T = (M+I) of the last real column and carries code 5; a haplotype 'N'
-// carries code 6 (both match no read base).  No divergent per-lane summation, no third value handed from lane to lane.
+// and the sum entry has gamma := 1, pm := 0, px := 1 and base code 0, so that U = T on every column that does not
+// "match" it and the chain s = s + U adds them up across the whole lane group.  What matches the sum entry: the columns
+// behind the haplotype EXCEPT the first one, which holds T = (M+I) of the last real column.  With HS those carry code
+// 0, the first one code 5 and a haplotype 'N' code 6 (5 and 6 match no read base); without HS a fifth match word,
+// hm[4], marks them.  No divergent per-lane summation, no third value handed from lane to lane.
 template <typename T, int NV, bool HS = false, bool SC = false> struct Lane2 {
     typedef W2<T> P;
     typedef typename P::V V;
     static_assert(NV <= 16, "one 32-bit match word per base: 16 columns per half");
-    static_assert(!SC || HS, "the sum entry selects by base code");
 
     V Tt[NV], J[NV];
     V outT, outS;              // what dropped out on the right in the last step: (.x's, .y's)
     T sigX, sigY;              // Eq.4 partial sums (columns <= this half's last) of the read finished last
-    uint32_t hm[4];            // match words, one per base b: bit x <=> .x column x is b, bit 16+x <=> .y column x is b
+    uint32_t hm[SC ? 5 : 4];   // match words, one per base b: bit x <=> .x column x is b, bit 16+x <=> .y column x is b
     uint32_t h2[HS ? NV : 1];  // HS: per column the base codes of (.x, .y) as two fp16 numbers (1..4, 0 = none)
     int nvx, nvy;              // number of real (j <= k) columns in each half
 
@@ -85,7 +85,7 @@ template <typename T, int NV, bool HS = false, bool SC = false> struct Lane2 {
 
     // hap: pointer to the haplotype bytes, k its length, j0 = 0-based first column of this thread
     __device__ __forceinline__ void load_hap(const uint8_t* __restrict__ hap, int k, int j0) {
-        if constexpr (SC) {
+        if constexpr (SC && HS) {
 #pragma unroll
             for (int x = 0; x < NV; x++) {
                 const int jx = j0 + x, jy = j0 + NV + x;
@@ -123,6 +123,15 @@ template <typename T, int NV, bool HS = false, bool SC = false> struct Lane2 {
                     h2[x] = v;
                 }
             }
+            if constexpr (SC) {  // what "matches" the sum entry: columns more than one behind the haplotype's last
+                uint32_t v = 0;
+#pragma unroll
+                for (int x = 0; x < NV; x++) {
+                    if (j0 + x > k) v |= 1u << x;
+                    if (j0 + NV + x > k) v |= 1u << (16 + x);
+                }
+                hm[4] = v;
+            }
         }
     }
     static __device__ __forceinline__ uint32_t half_code(int c) {  // fp16 bit pattern of the number c + 1
@@ -145,7 +154,11 @@ template <typename T, int NV, bool HS = false, bool SC = false> struct Lane2 {
         if constexpr (!HS) {
             const uint32_t wx01 = (E.metaX & 1u) ? hm[1] : hm[0], wx23 = (E.metaX & 1u) ? hm[3] : hm[2];
             const uint32_t wy01 = (E.metaY & 1u) ? hm[1] : hm[0], wy23 = (E.metaY & 1u) ? hm[3] : hm[2];
-            const uint32_t wx = (E.metaX & 2u) ? wx23 : wx01, wy = (E.metaY & 2u) ? wy23 : wy01;
+            uint32_t wx = (E.metaX & 2u) ? wx23 : wx01, wy = (E.metaY & 2u) ? wy23 : wy01;
+            if constexpr (SC) {
+                wx = (E.metaX & META_SUM) ? hm[4] : wx;  // (the other entries that are no read rows have pm = px = 0)
+                wy = (E.metaY & META_SUM) ? hm[4] : wy;
+            }
             mw = (wx & 0xffffu) | (wy & 0xffff0000u);
         }
         const uint32_t r2 = SC ? E.r2 : HS ? (half_code(E.metaX & 3u) | (half_code(E.metaY & 3u) << 16)) : 0u;

@@ -14,7 +14,7 @@ constexpr int CHAIN_NV_F64 = 8;
 constexpr int SHORT_WARPS_PER_CTA = 4;
 constexpr int TABLE_ZERO_RUN = 256;       // all-zero entries at the start of the row-constant table (idle lanes read them)
 constexpr int TABLE_EXTRA_ROWS = 3;       // short path: run-in entry in front of, sum and flush entries behind every read's rows (phmm_rowconst.cuh)
-constexpr int CHAIN_EXTRA_ROWS = 2;       // chain kernel: run-in entry and flush entry
+constexpr int CHAIN_EXTRA_ROWS = 3;       // chain kernel: the same stream
 
 struct DevBatch {  // device mirrors of the batch
     const uint8_t *read_bases, *qual_base, *qual_ins, *qual_del, *qual_gcp, *hap_bases;

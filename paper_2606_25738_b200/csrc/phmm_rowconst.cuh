@@ -9,7 +9,7 @@
 //              G = gamma_{i+1} g_{i+2}/g_{i+1};  on the last row gi_{l+1} := 1, A := C := 0, G := 1, meta LAST, so
 //              that the step leaves J = M_l + I_l, the summand of Eq.4.
 //   e = l+1    flush entry, all zero: gives the .y half (one entry behind) its step for row l and zeroes J.
-// With sum_entry (the short path, Lane2<.., SC>; l + 3 entries): the last row has A := 1, C := 0, G := 0 instead, which
+// With sum_entry (Lane2<.., SC>; l + 3 entries): the last row has A := 1, C := 0, G := 0 instead, which
 // leaves T[x+1] = M_{l,x} + I_{l,x};  e = l+1 is the SUM entry (gamma := 1, pm := 0, px := 1, base code 0, all else 0):
 // U = T on every column with a non-zero code, so the chain s = s + U leaves Eq.4's sum in the group's last lane;
 // e = l+2 is the all-zero flush entry, which clears the J = U the sum entry left behind.
@@ -36,7 +36,7 @@ __device__ __forceinline__ RowC row_constants(const DevBatch& b, const double* _
         const int i = e;  // read row, 1-based
         const double eps = lut[b.qual_base[off + i - 1]];
         const int code = base_code(b.read_bases[off + i - 1]);
-        c.meta = (uint32_t)(code & 3) | (i == l ? META_LAST : 0u);
+        c.meta = (uint32_t)(code & 3) | META_ROW | (i == l ? META_LAST : 0u);
         c.gam = lut[b.qual_gcp[off + i - 1]];
         double gin = 1.0;  // gi_{i+1} = g_{i+2} iota_{i+1};  := 1 behind the last row
         if (i < l) {
@@ -56,6 +56,13 @@ __device__ __forceinline__ RowC row_constants(const DevBatch& b, const double* _
         c.px = eps / 3.0 * gin;
     }
     return c;
+}
+
+// The 16-bit word an entry contributes to the table / ring: low byte = meta, high byte = upper byte of the fp16 number
+// HSETP2 compares with the per-column base codes (A,C,G,T = 1..4 on read rows, 0 on every other entry).
+__device__ __forceinline__ uint32_t entry_word16(const RowC& c) {
+    const uint32_t code = (c.meta & META_ROW) ? (uint32_t)((0x4400420040003C00ull >> (16 * (c.meta & META_CODE_MASK))) & 0xff00ull) : 0u;
+    return code | (c.meta & 0xffu);
 }
 
 }  // namespace phmm

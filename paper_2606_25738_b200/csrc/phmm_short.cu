@@ -22,8 +22,8 @@ namespace phmm {
 // Each 64-byte table entry holds the constants of entry e (for the .x half) and of entry e-1 (for .y; zero
 // for e = 0), already paired the way FFMA2 wants them:
 //   float4 0: gamma.x gamma.y A.x A.y | 1: C.x C.y G.x G.y | 2: pm.x px.x pm.y px.y | 3: word 0 0 0
-// word = what HSETP2 compares with the per-column codes, plus the flags: bits 10-14 / 26-30 the read base of e / e-1 as an
-// fp16 number (A,C,G,T = 1..4; 0 on entries that are not read rows), bits 0-7 / 16-23 the META_ flags of e / e-1.
+// word = entry_word16 of e | entry_word16 of e-1 << 16 (phmm_rowconst.cuh): what HSETP2 compares with the per-column
+// codes in the high bytes, the meta bytes in the low ones.
 // The table starts with TABLE_ZERO_RUN all-zero entries (what idle lanes fetch); read r's run starts at
 // entry TABLE_ZERO_RUN + read_off[r] + TABLE_EXTRA_ROWS r.  Constants are formed in double from the
 // 10^(-q/10) table and rounded once ("q32" table; Listing 2 :293-295 for which
@@ -35,11 +35,6 @@ namespace phmm {
 constexpr int TABLE_CHUNK_STRIDE = 32;  // float4 units between the chunk planes of a block
 __host__ __device__ __forceinline__ int64_t table_slot(int64_t pos) {  // float4 index of chunk 0 of entry pos
     return (pos >> 5) * 128 + (pos & 1) * 16 + ((pos >> 1) & 15);
-}
-
-__device__ __forceinline__ uint32_t entry_word(const RowC& c, bool is_row) {  // 16 bits: fp16 base code | flags
-    const uint32_t code = is_row ? (uint32_t)((0x4400420040003C00ull >> (16 * (c.meta & META_CODE_MASK))) & 0xffffull) : 0u;
-    return code | (c.meta & ~META_CODE_MASK & 0xffu);
 }
 
 __global__ void __launch_bounds__(256) k_table_f32(DevBatch b, const double* __restrict__ lut, float* __restrict__ table) {
@@ -59,7 +54,7 @@ __global__ void __launch_bounds__(256) k_table_f32(DevBatch b, const double* __r
         d[0 * TABLE_CHUNK_STRIDE] = make_float4((float)x.gam, (float)y.gam, (float)x.A, (float)y.A);
         d[1 * TABLE_CHUNK_STRIDE] = make_float4((float)x.C, (float)y.C, (float)x.G, (float)y.G);
         d[2 * TABLE_CHUNK_STRIDE] = make_float4((float)x.pm, (float)x.px, (float)y.pm, (float)y.px);
-        d[3 * TABLE_CHUNK_STRIDE] = make_float4(__uint_as_float(entry_word(x, e >= 1 && e <= l) | (entry_word(y, e >= 2 && e <= l + 1) << 16)), 0.f, 0.f, 0.f);
+        d[3 * TABLE_CHUNK_STRIDE] = make_float4(__uint_as_float(entry_word16(x) | (entry_word16(y) << 16)), 0.f, 0.f, 0.f);
     }
 }
 
