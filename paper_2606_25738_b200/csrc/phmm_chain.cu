@@ -31,7 +31,8 @@ namespace phmm {
 #define CHAIN_HSETP2 1  // fp32: +1-2 %
 #endif
 #ifndef CHAIN_MIN_CTAS_F32
-#define CHAIN_MIN_CTAS_F32 4  // 128 registers; measured +4.5 % over 3 CTAs x 166 registers
+#define CHAIN_MIN_CTAS_F32 3  // 164 registers with HSETP2 predicates; since Eq.4 runs through the s chain this beats 4 CTAs x 128 registers
+                              // (bit-test predicates: 2.17; HSETP2 with 15 spilled registers: 2.20; 3 CTAs: 2.26 TCUPS on configs[3] x0.5)
 #endif
 constexpr int RING = 128;  // row-constant ring per warp (entries); covers 63 entries of skew + two 32-entry blocks
 
@@ -131,7 +132,7 @@ template <typename T, int NV, typename LN> __device__ __forceinline__ void lane_
 template <typename T, int NV, int WPC, int MINB>
 __global__ void __launch_bounds__(WPC * 32, MINB)
 k_chain(DevBatch b, ChainLaunch p, int items_are_pairs) {
-    typedef Lane2<T, NV, (CHAIN_HSETP2 != 0) && sizeof(T) == 4 && MINB == 3, true> L;  // HSETP2 only where the 12 extra registers do not spill
+    typedef Lane2<T, NV, (CHAIN_HSETP2 != 0) && sizeof(T) == 4 && MINB == 3> L;  // HSETP2 only where the 12 extra registers do not spill
     typedef RingFmt<T> RF;
     typedef typename W2<T>::V V;
     constexpr int N2 = 2 * NV;
@@ -307,7 +308,7 @@ k_chain(DevBatch b, ChainLaunch p, int items_are_pairs) {
                         inS = scale_pow2<T>(inS, d); inT = scale_pow2<T>(inT, d);
                     }
                 }
-                ln.step(E, inS, inT, (T)0);
+                ln.step(E, inS, inT);
                 // ---- right boundary of the strip: lane 31's .y half has just finished entry s - 63
                 const int eo = s - 63;
                 if (eo >= 0 && eo < n_ent) {

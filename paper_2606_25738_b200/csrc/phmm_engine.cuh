@@ -23,7 +23,7 @@
 // place.  What crosses a virtual-lane boundary: the T[NV] that drops out on the right (consumed by
 // the neighbour two steps later = when it processes the next row) and the final s (consumed by the
 // neighbour's next step = the same row).  See the row-constant table kernel for the stream of
-// entries (run-in entry, rows 1..l, flush entry) and how Eq.1 and Eq.4 are realised.
+// entries (run-in entry, rows 1..l, sum entry, flush entry) and how Eq.1 and Eq.4 are realised.
 #pragma once
 #include "phmm_common.cuh"
 
@@ -52,40 +52,37 @@ template <typename T> struct Entry2 {
     typename W2<T>::V gam, A, C, G;
     T pmx, pxx, pmy, pxy;
     uint32_t metaX, metaY;
-    uint32_t r2;  // SC only: the fp16 base codes of (.x's row, .y's row), as the table stores them
+    uint32_t r2;  // HS: the fp16 base codes of (.x's row, .y's row), as the table / ring stores them (entry_word16)
 };
 
 // HS (fp32 only): take the Eq.3 predicates of both halves from one HSETP2 on per-column fp16 base codes instead
 // of two bit tests of the match word: 16 fewer ALU instructions per step, 12 more registers.
-// SC: Eq.4 comes out of the running sum s instead of a per-lane summation of J.  The stream then carries a
+// Eq.4 comes out of the running sum s instead of a per-lane summation of J.  The stream then carries a
 // "sum entry" behind the last row (phmm_rowconst.cuh): the last row leaves T[x+1] = M_{l,x} + I_{l,x} (A := 1, C := 0),
 // and the sum entry has gamma := 1, pm := 0, px := 1 and base code 0, so that U = T on every column that does not
 // "match" it and the chain s = s + U adds them up across the whole lane group.  What matches the sum entry: the columns
 // behind the haplotype EXCEPT the first one, which holds T = (M+I) of the last real column.  With HS those carry code
 // 0, the first one code 5 and a haplotype 'N' code 6 (5 and 6 match no read base); without HS a fifth match word,
 // hm[4], marks them.  No divergent per-lane summation, no third value handed from lane to lane.
-template <typename T, int NV, bool HS = false, bool SC = false> struct Lane2 {
+template <typename T, int NV, bool HS = false> struct Lane2 {
     typedef W2<T> P;
     typedef typename P::V V;
     static_assert(NV <= 16, "one 32-bit match word per base: 16 columns per half");
 
     V Tt[NV], J[NV];
     V outT, outS;              // what dropped out on the right in the last step: (.x's, .y's)
-    T sigX, sigY;              // Eq.4 partial sums (columns <= this half's last) of the read finished last
-    uint32_t hm[SC ? 5 : 4];   // match words, one per base b: bit x <=> .x column x is b, bit 16+x <=> .y column x is b
-    uint32_t h2[HS ? NV : 1];  // HS: per column the base codes of (.x, .y) as two fp16 numbers (1..4, 0 = none)
-    int nvx, nvy;              // number of real (j <= k) columns in each half
+    uint32_t hm[HS ? 1 : 5];   // without HS: match words, one per base b: bit x <=> .x column x is b, bit 16+x <=> .y column x is b
+    uint32_t h2[HS ? NV : 1];  // HS: per column the base codes of (.x, .y) as two fp16 numbers (1..4; 5, 6, 0: see above)
 
     __device__ __forceinline__ void init() {
 #pragma unroll
         for (int x = 0; x < NV; x++) { Tt[x] = P::mk((T)0, (T)0); J[x] = P::mk((T)0, (T)0); }
         outT = outS = P::mk((T)0, (T)0);
-        sigX = sigY = (T)0;
     }
 
     // hap: pointer to the haplotype bytes, k its length, j0 = 0-based first column of this thread
     __device__ __forceinline__ void load_hap(const uint8_t* __restrict__ hap, int k, int j0) {
-        if constexpr (SC && HS) {
+        if constexpr (HS) {
 #pragma unroll
             for (int x = 0; x < NV; x++) {
                 const int jx = j0 + x, jy = j0 + NV + x;
@@ -96,8 +93,7 @@ template <typename T, int NV, bool HS = false, bool SC = false> struct Lane2 {
         } else {
 #pragma unroll
             for (int c = 0; c < 4; c++) hm[c] = 0;
-            nvx = min(max(k - j0, 0), NV);
-            nvy = min(max(k - j0 - NV, 0), NV);
+            const int nvx = min(max(k - j0, 0), NV), nvy = min(max(k - j0 - NV, 0), NV);  // real columns of each half
 #pragma unroll
             for (int x = 0; x < NV; x++) {
                 if (x < nvx) {
@@ -111,41 +107,27 @@ template <typename T, int NV, bool HS = false, bool SC = false> struct Lane2 {
                     for (int q = 0; q < 4; q++) hm[q] |= (c == q ? 1u : 0u) << (16 + x);
                 }
             }
-            if (HS) {
+            uint32_t v = 0;  // what "matches" the sum entry: columns more than one behind the haplotype's last
 #pragma unroll
-                for (int x = 0; x < NV; x++) {
-                    uint32_t v = 0;
-#pragma unroll
-                    for (int q = 0; q < 4; q++) {
-                        if (hm[q] & (1u << x)) v |= half_code(q);
-                        if (hm[q] & (1u << (16 + x))) v |= half_code(q) << 16;
-                    }
-                    h2[x] = v;
-                }
+            for (int x = 0; x < NV; x++) {
+                if (j0 + x > k) v |= 1u << x;
+                if (j0 + NV + x > k) v |= 1u << (16 + x);
             }
-            if constexpr (SC) {  // what "matches" the sum entry: columns more than one behind the haplotype's last
-                uint32_t v = 0;
-#pragma unroll
-                for (int x = 0; x < NV; x++) {
-                    if (j0 + x > k) v |= 1u << x;
-                    if (j0 + NV + x > k) v |= 1u << (16 + x);
-                }
-                hm[4] = v;
-            }
+            hm[4] = v;
         }
     }
     static __device__ __forceinline__ uint32_t half_code(int c) {  // fp16 bit pattern of the number c + 1
         return (uint32_t)((0x4400420040003C00ull >> (16 * c)) & 0xffffull);
     }
-    static __device__ __forceinline__ uint32_t col_code(uint8_t b) {  // SC: fp16 1..4 for A,C,G,T; 6 for anything else
+    static __device__ __forceinline__ uint32_t col_code(uint8_t b) {  // fp16 1..4 for A,C,G,T; 6 for anything else
         const int c = base_code(b);
         return c < 4 ? half_code(c) : 0x4600u;
     }
 
-    // One systolic step.  (inS, inT, inSig): the left neighbour thread's (.y) outS, outT, sigY as they stand
+    // One systolic step.  (inS, inT): the left neighbour thread's (.y) outS, outT as they stand
     // after ITS last step, or the column-0 boundary for the first lane of a group (Eq.1 under reading G1:
     // the run-in entry injects s = C/k and T = g_1 C/k, every other entry 0).
-    __device__ __forceinline__ void step(const Entry2<T>& E, T inS, T inT, T inSig) {
+    __device__ __forceinline__ void step(const Entry2<T>& E, T inS, T inT) {
         V s = P::mk(inS, outS.x);                  // .y continues the row .x finished one step ago
         const V tgrab = P::mk(inT, outT.x);        // T[0] of the NEXT step
         // match word of this step: the read base of .x's row picks the low half, that of .y's row the high half;
@@ -155,13 +137,11 @@ template <typename T, int NV, bool HS = false, bool SC = false> struct Lane2 {
             const uint32_t wx01 = (E.metaX & 1u) ? hm[1] : hm[0], wx23 = (E.metaX & 1u) ? hm[3] : hm[2];
             const uint32_t wy01 = (E.metaY & 1u) ? hm[1] : hm[0], wy23 = (E.metaY & 1u) ? hm[3] : hm[2];
             uint32_t wx = (E.metaX & 2u) ? wx23 : wx01, wy = (E.metaY & 2u) ? wy23 : wy01;
-            if constexpr (SC) {
-                wx = (E.metaX & META_SUM) ? hm[4] : wx;  // (the other entries that are no read rows have pm = px = 0)
-                wy = (E.metaY & META_SUM) ? hm[4] : wy;
-            }
+            wx = (E.metaX & META_SUM) ? hm[4] : wx;  // (the other entries that are no read rows have pm = px = 0)
+            wy = (E.metaY & META_SUM) ? hm[4] : wy;
             mw = (wx & 0xffffu) | (wy & 0xffff0000u);
         }
-        const uint32_t r2 = SC ? E.r2 : HS ? (half_code(E.metaX & 3u) | (half_code(E.metaY & 3u) << 16)) : 0u;
+        const uint32_t r2 = E.r2;
         auto prior = [&](int x) {                  // Eq.3: one select per half
             if constexpr (HS && sizeof(T) == 4) {  // one HSETP2 yields both halves' predicates
                 float a, b;
@@ -185,32 +165,7 @@ template <typename T, int NV, bool HS = false, bool SC = false> struct Lane2 {
             U = Un;
         }
         outS = s;
-        if constexpr (SC) return;  // Eq.4 is the s that leaves the group's last lane on the sum entry
-        // Eq.4: on the last row G = 1 and gi_{l+1} := 1, so J now holds M_l + I_l; sum this half's real columns
-        if ((E.metaX | E.metaY) & META_LAST) {
-            if (E.metaX & META_LAST) {
-                T a = (T)0;
-                if (nvx == NV) {
-#pragma unroll
-                    for (int x = 0; x < NV; x++) a += J[x].x;
-                } else {
-#pragma unroll
-                    for (int x = 0; x < NV; x++) a += (x < nvx) ? J[x].x : (T)0;
-                }
-                sigX = inSig + a;
-            }
-            if (E.metaY & META_LAST) {
-                T a = (T)0;
-                if (nvy == NV) {
-#pragma unroll
-                    for (int x = 0; x < NV; x++) a += J[x].y;
-                } else {
-#pragma unroll
-                    for (int x = 0; x < NV; x++) a += (x < nvy) ? J[x].y : (T)0;
-                }
-                sigY = sigX + a;
-            }
-        }
+        // Eq.4 is the s that leaves the group's last lane on the sum entry: nothing to do here
     }
 };
 

@@ -1,7 +1,7 @@
 // Short-pair path: row-constant table prologue + the sub-warp systolic fp32 kernel.
 //
 // Hot path rows of SURVEY.md section 8(a): a1 (quality -> row constants: table kernel), a2 (haplotype
-// staging: match words / fp16 base codes in registers), a3/a4 (row updates), a5 (lane-to-lane carry: 3 shuffles
+// staging: match words / fp16 base codes in registers), a3/a4 (row updates), a5 (lane-to-lane carry: 2 shuffles
 // per row), a9 (final reduction, log10), a10 (underflow detection -> rescue queue).
 #include "phmm_engine.cuh"
 #include "phmm_kernels.h"
@@ -96,7 +96,7 @@ struct RawEntry { float4 a, b, c; uint32_t w; };
 
 template <int NV>
 __global__ void __launch_bounds__(SHORT_WARPS_PER_CTA * 32, SHORT_MIN_CTAS) k_short_f32(DevBatch b, ShortLaunch p) {
-    typedef Lane2<float, NV, true, true> L;  // HSETP2 predicates (2.78 vs 2.60 TCUPS with bit tests), Eq.4 through the s chain
+    typedef Lane2<float, NV, true> L;  // HSETP2 predicates (2.78 vs 2.60 TCUPS with bit tests), Eq.4 through the s chain
     constexpr int N2 = 2 * NV;
     const int warp = blockIdx.x * SHORT_WARPS_PER_CTA + (threadIdx.x >> 5);
     if (warp >= p.n_warps) return;
@@ -197,7 +197,7 @@ __global__ void __launch_bounds__(SHORT_WARPS_PER_CTA * 32, SHORT_MIN_CTAS) k_sh
             inS = f ? Cok : 0.f;
             inT = f ? E.C.x * Cok : 0.f;
         }
-        ln.step(E, inS, inT, 0.f);
+        ln.step(E, inS, inT);
         if (is_last && (E.metaY & META_SUM)) {  // Eq.4: the s chain has collected M_l + I_l of every column
             const float sg = full_last ? ln.outS.y + prevT : ln.outS.y;
             const int pair = p.srt_out[m_first + nout];
