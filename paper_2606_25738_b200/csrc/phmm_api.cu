@@ -325,7 +325,7 @@ extern "C" int phmm_forward_batch(phmm_ctx* ctx, const phmm_batch* b, int precis
         for (int p : strip_pairs) {
             const int r = b->h_pair_read[p], h = b->h_pair_hap[p];
             const int64_t l = b->h_read_off[r + 1] - b->h_read_off[r], k = b->h_hap_off[h + 1] - b->h_hap_off[h];
-            const int ns = (int)(k / strip_cols + 1);  // always one column behind the haplotype (the sum entry needs it)
+            const int ns = (int)((k + strip_cols - 1) / strip_cols);
             const int64_t nblk = (l + CHAIN_EXTRA_ROWS + 31) / 32;
             ps.push_back(PairStrips{p, ns, n_prog, n_bnd_blocks});
             n_bnd_blocks += (int64_t)(ns > 1 ? ns - 1 : 0) * nblk;
@@ -453,7 +453,7 @@ extern "C" int phmm_forward_batch(phmm_ctx* ctx, const phmm_batch* b, int precis
     if (n_warps > 0 || n_seq > 0 || sub) {
         const int grid = ctx->chain_grid[1];
         const int64_t blocks = (max_seq_l + CHAIN_EXTRA_ROWS + 31) / 32 + 1;
-        const int max_strips_seq = ctx->opt.long_min_hap_len / chain_strip_cols(true) + 1;
+        const int max_strips_seq = (ctx->opt.long_min_hap_len + chain_strip_cols(true) - 1) / chain_strip_cols(true);
         size_t scratch = max_strips_seq > 1 ? (size_t)grid * chain_warps_per_cta(true) * 2 * blocks * chain_block_bytes(true) : 256;
         CK(ctx->d_scratch.need(scratch));
         ChainLaunch cl;

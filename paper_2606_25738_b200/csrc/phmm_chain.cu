@@ -165,7 +165,8 @@ k_chain(DevBatch b, ChainLaunch p, int items_are_pairs) {
         const int64_t ro = b.read_off[r], ho = b.hap_off[h];
         const int l = (int)(b.read_off[r + 1] - ro), k = (int)(b.hap_off[h + 1] - ho);
         const int n_ent = l + CHAIN_EXTRA_ROWS;  // run-in entry, rows 1..l, sum entry, flush entry
-        const int nstrips = k / (32 * N2) + 1;  // always one column behind the haplotype: the sum entry finds (M+I) of column k there
+        const int nstrips = (k + 32 * N2 - 1) / (32 * N2);
+        const bool full_last = k == nstrips * 32 * N2;  // no column behind the haplotype's last one (see the output below)
         const int nblk = (n_ent + 31) / 32;  // boundary blocks per buffer
         const int st_lo = strip < 0 ? 0 : strip, st_hi = strip < 0 ? nstrips : strip + 1;
         const T Cok = (T)(ldexp(1.0, p.log2C) / (double)k);
@@ -308,6 +309,7 @@ k_chain(DevBatch b, ChainLaunch p, int items_are_pairs) {
                         inS = scale_pow2<T>(inS, d); inT = scale_pow2<T>(inT, d);
                     }
                 }
+                const T prevT = ln.outT.y;  // at this thread's current exponent (every rescaling of this step is done)
                 ln.step(E, inS, inT);
                 // ---- right boundary of the strip: lane 31's .y half has just finished entry s - 63
                 const int eo = s - 63;
@@ -330,7 +332,10 @@ k_chain(DevBatch b, ChainLaunch p, int items_are_pairs) {
                             __syncwarp();
                         }
                     } else if (eo == l + 1 && lane == 31) {  // the sum entry: s has collected Eq.4; log10 in double
-                        p.out[pair] = log10((double)ln.outS.y) + ((double)ex - (double)p.log2C) * LOG10_2;
+                        // M+I of column j reaches the chain through the T of column j+1; a haplotype that fills its last
+                        // strip has the last one in what this lane handed out one step ago instead
+                        const T sum = full_last ? ln.outS.y + prevT : ln.outS.y;
+                        p.out[pair] = log10((double)sum) + ((double)ex - (double)p.log2C) * LOG10_2;
                         if (p.flags) p.flags[pair] = p.flag_bits;
                     }
                 }
