@@ -1,7 +1,7 @@
 // Generic rescaled path ("chain" kernel): one warp = one strip of 32 lanes x 2NV haplotype columns of
 // one pair; the strips of a pair are chained left to right through boundary-column buffers in
 // global memory (per stream entry: the running sum s and the T that drop out of the strip's last
-// column, the Eq.4 partial sum, and the strip's block exponent), either concurrently (one strip per
+// column, and the producing thread's block exponent), either concurrently (one strip per
 // warp, progress counters; warps take strips in ticket order so a producer always holds an earlier
 // ticket than its consumer => forward progress) or sequentially inside one warp (fp64 rescue of
 // short pairs, PHMM_FP64 mode).
@@ -12,13 +12,14 @@
 //
 // Rescaling (reading G15; absent from the paper).  Block floating point per THREAD: true value = stored
 // value * 2^ex with one integer ex for everything a thread holds (the T/J state of its two halves, the
-// values it hands to the right, its Eq.4 partial sums).  The lanes of a warp are 2 read rows apart, so
+// values it hands to the right).  Eq.4 needs no sum of its own: on the sum entry behind the last row the running
+// sum s collects M_l + I_l of every column (phmm_engine.cuh).  The lanes of a warp are 2 read rows apart, so
 // a warp spans 64 rows and, along a row, 32 columns per lane: with unrelated sequence (3.3 bits lost
 // per row or per deleted column) that is more than fp32's exponent range, hence no coarser unit.
 // Every 16 steps a thread takes the maximum of what it holds and, if that left the window around
 // 2^TGT, multiplies everything by the power of two that brings it back (exact, except that values
 // more than the format's range below the thread maximum flush to zero: G15's documented limit).
-// The three values crossing a lane (or strip) boundary per step come with the producer's ex and are
+// The two values crossing a lane (or strip) boundary per step come with the producer's ex and are
 // converted by one exact multiply; if they would not fit, the consumer first moves its own exponent
 // up.  The recurrence step itself is exactly the short kernel's (phmm_engine.cuh).
 #include "phmm_engine.cuh"
