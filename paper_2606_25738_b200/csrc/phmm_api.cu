@@ -394,7 +394,7 @@ extern "C" int phmm_forward_batch(phmm_ctx* ctx, const phmm_batch* b, int precis
 
     // ---- short path: row-constant table, systolic kernel, then fp64 rescue of what underflowed
     if (n_warps > 0) {
-        const int64_t n_entries = TABLE_ZERO_RUN + b->h_read_off[b->n_reads] + (int64_t)TABLE_EXTRA_ROWS * b->n_reads;
+        const int64_t n_entries = table_run_start(b->h_read_off[b->n_reads], b->n_reads) + 2;
         if (n_entries > INT32_MAX) return PHMM_E_TOOLONG;
         const size_t table_bytes = (size_t)(n_entries + 64) * 64;
         if ((int64_t)table_bytes > ctx->opt.max_table_bytes) return PHMM_E_NOMEM;

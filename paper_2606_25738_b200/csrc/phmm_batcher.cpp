@@ -71,8 +71,8 @@ void plan_short(const HostBatchView& b, const uint8_t* is_short, int N2, int tas
                 const int q = pos[b.pair_hap[p]]++;
                 const int r = b.pair_read[p];
                 out->srt_out[q] = (int)p;
-                out->srt_ent[2 * (size_t)q] = (int)(TABLE_ZERO_RUN + b.read_off[r] + (int64_t)TABLE_EXTRA_ROWS * r);
-                out->srt_ent[2 * (size_t)q + 1] = (int)(b.read_off[r + 1] - b.read_off[r]) + TABLE_EXTRA_ROWS;
+                out->srt_ent[2 * (size_t)q] = (int)table_run_start(b.read_off[r], r);
+                out->srt_ent[2 * (size_t)q + 1] = table_run_len((int)(b.read_off[r + 1] - b.read_off[r]));
             }
     });
     // ---- 2. cut each haplotype's run of reads into tasks of about task_rows read rows (haplotype ranges in parallel)
@@ -89,16 +89,18 @@ void plan_short(const HostBatchView& b, const uint8_t* is_short, int N2, int tas
                 const int lo = cnt[h], hi = cnt[h + 1];
                 if (lo == hi) continue;
                 const int64_t k = b.hap_off[h + 1] - b.hap_off[h];
-                ShortTask tk = {(int)h, lo, 0, 0};
+                ShortTask tk = {(int)h, lo, 0, 0, 0};
                 for (int q = lo; q < hi; q++) {
-                    const int l = out->srt_ent[2 * (size_t)q + 1] - TABLE_EXTRA_ROWS;
+                    const int r = b.pair_read[out->srt_out[q]];
+                    const int l = (int)(b.read_off[r + 1] - b.read_off[r]);
                     cells += (int64_t)l * k;
                     if (l > mx) mx = l;
                     tk.n_pairs++;
                     tk.rows += l;
+                    tk.ents += out->srt_ent[2 * (size_t)q + 1];
                     if (tk.rows >= task_rows) {
                         tv.push_back(tk);
-                        tk.pair_first = q + 1; tk.n_pairs = 0; tk.rows = 0;
+                        tk.pair_first = q + 1; tk.n_pairs = 0; tk.rows = 0; tk.ents = 0;
                     }
                 }
                 if (tk.n_pairs > 0) tv.push_back(tk);
@@ -117,7 +119,7 @@ void plan_short(const HostBatchView& b, const uint8_t* is_short, int N2, int tas
     // ---- 3. pack tasks into warps: duration classes (longest first), lanes bin-packed largest-fit
     const int NCLS = 8 * 40;  // class = floor(8 * log2(duration)), duration < 2^40
     auto cls_of = [&](const ShortTask& t) {
-        const double d = (double)(t.rows + TABLE_EXTRA_ROWS * t.n_pairs);
+        const double d = (double)t.ents;
         int c = (int)floor(8.0 * log2(d < 1 ? 1 : d));
         return c < 0 ? 0 : (c >= NCLS ? NCLS - 1 : c);
     };
@@ -204,7 +206,7 @@ void plan_short(const HostBatchView& b, const uint8_t* is_short, int N2, int tas
                 if (avail[bk] == bstart[bk + 1]) nonempty[c] &= ~(1ull << g);
                 P.tasks.push_back(tk);
                 cap -= g;
-                bin_steps = std::max(bin_steps, tk.rows + TABLE_EXTRA_ROWS * tk.n_pairs + 2 * g - 1);
+                bin_steps = std::max(bin_steps, tk.ents + 2 * g - 1);
                 if (cap == 0) close_bin();
             }
         }

@@ -43,7 +43,7 @@ struct HostBatchView {
 struct ShortPlan {
     std::vector<ShortTask> tasks;   // ordered by warp
     std::vector<int> warp_first;    // n_warps + 1
-    std::vector<int> srt_ent;       // 2 ints per sorted pair: first table entry of its read's run, entries of the run (read length + TABLE_EXTRA_ROWS)
+    std::vector<int> srt_ent;       // 2 ints per sorted pair: first table entry of its read's run, entries of the run (table_run_len)
     std::vector<int> srt_out;       // caller's pair index per sorted pair
     int64_t cells = 0;              // real cells of the short pairs
     int64_t padded_cells = 0;       // lane-cells swept: sum over warps of steps * 32 lanes * columns-per-lane

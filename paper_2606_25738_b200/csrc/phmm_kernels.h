@@ -14,6 +14,17 @@ constexpr int CHAIN_NV_F64 = 8;
 constexpr int SHORT_WARPS_PER_CTA = 4;
 constexpr int TABLE_ZERO_RUN = 256;       // all-zero entries at the start of the row-constant table (idle lanes read them)
 constexpr int TABLE_EXTRA_ROWS = 3;       // short path: run-in entry in front of, sum and flush entries behind every read's rows (phmm_rowconst.cuh)
+// Table positions of the short path.  Every read's run starts at an EVEN entry and has an even length (padded with one
+// more all-zero entry where l + 3 is odd), so that the parity of a lane's table position equals the parity of its step:
+// the kernel's step loop is unrolled by two and the odd step's entry sits 16 slots behind the even one's, always in
+// the same 32-entry block, with no address arithmetic and no run switch in between (phmm_short.cu).
+constexpr int TABLE_SLOTS_PER_READ = 4;   // table entries reserved per read beyond its rows
+inline __host__ __device__ int64_t table_run_start(int64_t read_off_r, int64_t r) {
+    const int64_t b = TABLE_ZERO_RUN + read_off_r + TABLE_SLOTS_PER_READ * r;
+    return b + (b & 1);
+}
+inline __host__ __device__ int table_run_len(int l) { return (l + TABLE_EXTRA_ROWS + 1) & ~1; }
+static_assert(TABLE_ZERO_RUN % 2 == 0, "idle lanes walk the zero run two entries per loop iteration");
 constexpr int CHAIN_EXTRA_ROWS = 3;       // chain kernel: the same stream
 
 struct DevBatch {  // device mirrors of the batch
@@ -49,6 +60,7 @@ __device__ __forceinline__ void rescue_push(const RescueQueue& rq, int pair, int
 
 struct ShortTask {  // one lane group's work: several reads streamed against one haplotype
     int hap, pair_first, n_pairs, rows;  // rows = sum of the read lengths (reset rows not counted)
+    int ents;                            // table entries of its stream = sum of table_run_len(l)
 };
 
 struct ShortLaunch {
@@ -56,7 +68,7 @@ struct ShortLaunch {
     const ShortTask* tasks;    // ordered by warp
     const int* warp_first;     // n_warps+1: first task of each warp
     int n_warps;
-    const int2* srt_ent;       // (first table entry, number of entries = read length + TABLE_EXTRA_ROWS) of each sorted pair
+    const int2* srt_ent;       // (first table entry, number of entries = table_run_len(read length)) of each sorted pair
     const int* srt_out;        // caller's pair index of each sorted pair
     double* out;
     uint8_t* flags;

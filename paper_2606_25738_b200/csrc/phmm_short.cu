@@ -25,7 +25,7 @@ namespace phmm {
 // word = entry_word16 of e | entry_word16 of e-1 << 16 (phmm_rowconst.cuh): what HSETP2 compares with the per-column
 // codes in the high bytes, the meta bytes in the low ones.
 // The table starts with TABLE_ZERO_RUN all-zero entries (what idle lanes fetch); read r's run starts at
-// entry TABLE_ZERO_RUN + read_off[r] + TABLE_EXTRA_ROWS r.  Constants are formed in double from the
+// entry table_run_start(read_off[r], r) (even; phmm_kernels.h).  Constants are formed in double from the
 // 10^(-q/10) table and rounded once ("q32" table; Listing 2 :293-295 for which
 // qualities enter which transition).  One warp per read.
 // Memory layout: the entries are permuted inside blocks of 32 so that the lanes of a warp, which read entries
@@ -47,8 +47,8 @@ __global__ void __launch_bounds__(256) k_table_f32(DevBatch b, const double* __r
     const int64_t off = b.read_off[r];
     const int l = (int)(b.read_off[r + 1] - off);
     float4* dst = reinterpret_cast<float4*>(table);
-    const int64_t first = TABLE_ZERO_RUN + off + TABLE_EXTRA_ROWS * r;
-    for (int e = lane; e < l + TABLE_EXTRA_ROWS; e += 32) {
+    const int64_t first = table_run_start(off, r);
+    for (int e = lane; e < table_run_len(l); e += 32) {  // (an entry behind the flush entry is all zero too)
         const RowC x = row_constants(b, lut, off, l, e, true), y = row_constants(b, lut, off, l, e - 1, true);
         float4* d = dst + table_slot(first + e);
         d[0 * TABLE_CHUNK_STRIDE] = make_float4((float)x.gam, (float)y.gam, (float)x.A, (float)y.A);
@@ -104,7 +104,7 @@ __global__ void __launch_bounds__(SHORT_WARPS_PER_CTA * 32, SHORT_MIN_CTAS) k_sh
 
     // ---- which task does this lane belong to?  tasks of a warp occupy consecutive lane ranges
     const int t0 = p.warp_first[warp], nt = p.warp_first[warp + 1] - t0;
-    ShortTask tk = {0, 0, 0, 0};
+    ShortTask tk = {0, 0, 0, 0, 0};
     int k = 0, g = 0;
     if (lane < nt) {
         tk = p.tasks[t0 + lane];
@@ -126,17 +126,17 @@ __global__ void __launch_bounds__(SHORT_WARPS_PER_CTA * 32, SHORT_MIN_CTAS) k_sh
     }
     const int src = ti < 0 ? 0 : ti;
     const int m_hap = __shfl_sync(PHMM_FULL, tk.hap, src), m_first = __shfl_sync(PHMM_FULL, tk.pair_first, src);
-    int m_np = __shfl_sync(PHMM_FULL, tk.n_pairs, src), m_rows = __shfl_sync(PHMM_FULL, tk.rows, src);
+    int m_np = __shfl_sync(PHMM_FULL, tk.n_pairs, src), m_ents = __shfl_sync(PHMM_FULL, tk.ents, src);
     int m_k = __shfl_sync(PHMM_FULL, k, src);
     const int m_start = __shfl_sync(PHMM_FULL, start, src), m_g = __shfl_sync(PHMM_FULL, g, src);
-    if (ti < 0) { m_np = 0; m_rows = 0; m_k = 0; }
+    if (ti < 0) { m_np = 0; m_ents = 0; m_k = 0; }
     const int lg = ti < 0 ? 0 : lane - m_start;
     const bool is_first = (ti < 0) || lg == 0;
     const bool is_last = (ti >= 0) && lg == m_g - 1;
     const bool full_last = m_k == m_g * N2;  // no column behind the haplotype's last one
 
     // ---- number of steps of this warp: the last lane's .y half finishes the last entry of its stream
-    int steps = (ti < 0) ? 0 : m_rows + TABLE_EXTRA_ROWS * m_np + 2 * m_g - 1;
+    int steps = (ti < 0) ? 0 : m_ents + 2 * m_g - 1;
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) steps = max(steps, __shfl_xor_sync(PHMM_FULL, steps, o));
 
@@ -161,10 +161,11 @@ __global__ void __launch_bounds__(SHORT_WARPS_PER_CTA * 32, SHORT_MIN_CTAS) k_sh
     load_next();
     // dep: the word of the entry the CURRENT step works on.  Its top bit is never set, but the address now depends on
     // it, which keeps the loads behind the wait for that entry (see the step loop).
-    auto fetch = [&](RawEntry& r, uint32_t dep) {
-        if (c.pos == c.end) { c.pos = c.npos; c.end = c.nend; load_next(); }
-        const float4* e = tab + (table_slot(c.pos) + (dep >> 31));
-        c.pos++;
+    // Runs start at even entries and have even lengths, so a lane's position is even at the loop's even steps: only
+    // those look at the cursor and form an address; the odd step's entry is the next one of the same 32-entry block,
+    // 16 slots (256 bytes) further on.
+    const float4* e_even = tab;
+    auto load_entry = [&](RawEntry& r, const float4* e) {
 #if SHORT_L2_PREFETCH
         r.a = ldg_pf(e);
         r.b = ldg_pf(e + TABLE_CHUNK_STRIDE);
@@ -177,6 +178,13 @@ __global__ void __launch_bounds__(SHORT_WARPS_PER_CTA * 32, SHORT_MIN_CTAS) k_sh
         r.w = __ldg(reinterpret_cast<const uint32_t*>(e + 3 * TABLE_CHUNK_STRIDE));
 #endif
     };
+    auto fetch_even = [&](RawEntry& r, uint32_t dep) {
+        if (c.pos == c.end) { c.pos = c.npos; c.end = c.nend; load_next(); }
+        e_even = tab + (table_slot(c.pos) + (dep >> 31));
+        c.pos += 2;
+        load_entry(r, e_even);
+    };
+    auto fetch_odd = [&](RawEntry& r, uint32_t dep) { load_entry(r, e_even + (16 + (dep >> 31))); };
 
     int nout = 0;
     const double LOG10_2 = 0.30102999566398119521;
@@ -205,7 +213,7 @@ __global__ void __launch_bounds__(SHORT_WARPS_PER_CTA * 32, SHORT_MIN_CTAS) k_sh
             if (isfinite(sg) && sg >= p.rescue_thr) {
                 p.out[pair] = log10((double)sg) - 120.0 * LOG10_2;
                 if (p.flags) p.flags[pair] = 0;
-            } else if (m_k <= RESCUE_MAX_K && __ldg(ent + nout - 1).y - TABLE_EXTRA_ROWS <= RESCUE_MAX_L) {
+            } else if (m_k <= RESCUE_MAX_K) {  // (every short-class read has l <= RESCUE_MAX_L)
                 rescue_push(p.rescue, pair, m_k);  // a10: unrescaled fp64 sub-warp kernel
             } else {
                 const int idx = atomicAdd(p.rescue_count, 1);  // rescaled fp64 chain kernel
@@ -219,11 +227,11 @@ __global__ void __launch_bounds__(SHORT_WARPS_PER_CTA * 32, SHORT_MIN_CTAS) k_sh
     // address of the next entry depend on its own entry's word (loaded one step ago), so the loads are issued BEHIND the
     // wait and the wait never covers loads younger than a whole step: 3.31 -> 3.36 TCUPS, 4 fewer registers.
     RawEntry eA, eB;
-    fetch(eA, 0u);
+    fetch_even(eA, 0u);
     for (int s = 0; s < steps; s += 2) {  // an odd step count runs one extra all-idle step, which is harmless
-        fetch(eB, eA.w);
+        fetch_odd(eB, eA.w);
         one_step(eA);
-        fetch(eA, eB.w);
+        fetch_even(eA, eB.w);
         one_step(eB);
     }
 }
