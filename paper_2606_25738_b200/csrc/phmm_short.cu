@@ -133,6 +133,7 @@ __global__ void __launch_bounds__(SHORT_WARPS_PER_CTA * 32, SHORT_MIN_CTAS) k_sh
     const int lg = ti < 0 ? 0 : lane - m_start;
     const bool is_first = (ti < 0) || lg == 0;
     const bool is_last = (ti >= 0) && lg == m_g - 1;
+    const uint32_t sum_bit = is_last ? (META_SUM << 16) : 0u;
     const bool full_last = m_k == m_g * N2;  // no column behind the haplotype's last one
 
     // ---- number of steps of this warp: the last lane's .y half finishes the last entry of its stream
@@ -180,7 +181,7 @@ __global__ void __launch_bounds__(SHORT_WARPS_PER_CTA * 32, SHORT_MIN_CTAS) k_sh
     };
     auto fetch_even = [&](RawEntry& r, uint32_t dep) {
         if (c.pos == c.end) { c.pos = c.npos; c.end = c.nend; load_next(); }
-        e_even = tab + (table_slot(c.pos) + (dep >> 31));
+        e_even = tab + ((((int64_t)(c.pos >> 5)) << 7) + (int64_t)(((c.pos >> 1) & 15) + (dep >> 31)));  // table_slot of an even position
         c.pos += 2;
         load_entry(r, e_even);
     };
@@ -203,10 +204,10 @@ __global__ void __launch_bounds__(SHORT_WARPS_PER_CTA * 32, SHORT_MIN_CTAS) k_sh
         if (is_first) {  // column-0 boundary, Eq.1
             const bool f = (E.metaX & META_FIRST) != 0;
             inS = f ? Cok : 0.f;
-            inT = f ? E.C.x * Cok : 0.f;
+            inT = E.C.x * inS;
         }
         ln.step(E, inS, inT);
-        if (is_last && (E.metaY & META_SUM)) {  // Eq.4: the s chain has collected M_l + I_l of every column
+        if (r.w & sum_bit) {  // the group's last lane, its .y half on the sum entry: s has collected M_l + I_l of every column (Eq.4)
             const float sg = full_last ? ln.outS.y + prevT : ln.outS.y;
             const int pair = p.srt_out[m_first + nout];
             nout++;
