@@ -73,7 +73,7 @@ typedef struct phmm_options {
      * haplotype through one lane group); 0 = chosen per batch between 1024 and 8192 so that the
      * GPU still gets several waves of warps */
     int32_t task_rows;
-    /* upper bound, in bytes, for the row-constant table of the short path (64 bytes per read base + 128 per
+    /* upper bound, in bytes, for the row-constant table of the short path (64 bytes per read base + 256 per
      * read); a batch needing more fails with PHMM_E_NOMEM (split it).  Default 64 GiB. */
     int64_t max_table_bytes;
     /* non-zero: bracket every kernel family of a call with CUDA events on the caller's stream; the
