@@ -47,6 +47,17 @@ struct PinBuf {  // grow-only pinned host staging buffer
 
 }  // namespace
 
+struct DeviceGuard {  // makes `device` current for the duration of an API call, then restores the caller's device
+    int prev = -1;
+    bool ok = false;
+    explicit DeviceGuard(int device) {
+        if (cudaGetDevice(&prev) != cudaSuccess) prev = -1;
+        ok = (prev == device) || cudaSetDevice(device) == cudaSuccess;
+        if (prev == device) prev = -1;
+    }
+    ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
+};
+
 struct phmm_ctx {
     int device = 0;
     int n_sm = 0;
@@ -64,6 +75,8 @@ struct phmm_ctx {
     } set[2];
     int call_idx = 0;
     cudaStream_t copy_stream = nullptr;
+    cudaEvent_t ev_last = nullptr;  // end of the device work of the most recent call: the next call's stream waits for it,
+                                    // because the table, the counters, the queues and the boundary buffers exist once per context
     DevBuf d_lut, d_table;
     DevBuf d_counters, d_rescue, d_boundary, d_progress, d_scratch;
     DevBuf d_rq, d_rq_queue, d_rq_sorted, d_rq_plan;  // fp64 sub-warp recomputation: counters, queue, ordered queue, plan, FP64-mode input list
@@ -105,6 +118,8 @@ extern "C" int phmm_create(phmm_ctx** out, int device, const phmm_options* opt) 
     cudaDeviceProp prop;
     if (cudaGetDeviceProperties(&prop, device) != cudaSuccess) return PHMM_E_CUDA;
     if (prop.major != 10) return PHMM_E_UNSUPPORTED;
+    DeviceGuard guard(device);
+    if (!guard.ok) return PHMM_E_CUDA;
     phmm_ctx* ctx = new (std::nothrow) phmm_ctx();
     if (!ctx) return PHMM_E_NOMEM;
     ctx->device = device;
@@ -116,9 +131,9 @@ extern "C" int phmm_create(phmm_ctx** out, int device, const phmm_options* opt) 
     if (ctx->opt.max_table_bytes <= 0) ctx->opt.max_table_bytes = (int64_t)64 << 30;
     if (ctx->opt.profile_events)
         for (int i = 0; i < 8; i++)
-            if (cudaEventCreate(&ctx->ev_prof[i]) != cudaSuccess) { delete ctx; return PHMM_E_CUDA; }
+            if (cudaEventCreate(&ctx->ev_prof[i]) != cudaSuccess) { phmm_destroy(ctx); return PHMM_E_CUDA; }
     memset(&ctx->stats, 0, sizeof(ctx->stats));
-    if (cudaSetDevice(device) != cudaSuccess) { delete ctx; return PHMM_E_CUDA; }
+    if (cudaEventCreateWithFlags(&ctx->ev_last, cudaEventDisableTiming) != cudaSuccess) { phmm_destroy(ctx); return PHMM_E_CUDA; }
     for (int i = 0; i < 2; i++)
         if (cudaEventCreateWithFlags(&ctx->set[i].ev_free, cudaEventDisableTiming) != cudaSuccess ||
             cudaEventCreateWithFlags(&ctx->set[i].ev_up, cudaEventDisableTiming) != cudaSuccess) { phmm_destroy(ctx); return PHMM_E_CUDA; }
@@ -138,7 +153,7 @@ extern "C" int phmm_create(phmm_ctx** out, int device, const phmm_options* opt) 
 
 extern "C" int phmm_destroy(phmm_ctx* ctx) {
     if (!ctx) return PHMM_E_ARG;
-    cudaSetDevice(ctx->device);
+    DeviceGuard guard(ctx->device);
     cudaDeviceSynchronize();
     DevBuf* bufs[] = {&ctx->d_lut, &ctx->d_table, &ctx->d_counters, &ctx->d_rescue, &ctx->d_boundary, &ctx->d_progress, &ctx->d_scratch,
                       &ctx->d_payload, &ctx->d_out, &ctx->d_flags, &ctx->d_rq, &ctx->d_rq_queue, &ctx->d_rq_sorted, &ctx->d_rq_plan};
@@ -153,6 +168,7 @@ extern "C" int phmm_destroy(phmm_ctx* ctx) {
         if (ps.ev_up) cudaEventDestroy(ps.ev_up);
     }
     if (ctx->copy_stream) cudaStreamDestroy(ctx->copy_stream);
+    if (ctx->ev_last) cudaEventDestroy(ctx->ev_last);
     for (int i = 0; i < 8; i++)
         if (ctx->ev_prof[i]) cudaEventDestroy(ctx->ev_prof[i]);
     delete ctx;
@@ -163,7 +179,7 @@ extern "C" int phmm_get_stats(phmm_ctx* ctx, phmm_stats* out) {
     if (!ctx || !out) return PHMM_E_ARG;
     if (!ctx->stats_final && ctx->d_counters.p && ctx->stats.n_pairs > 0) {  // rescue count lives on the device until the caller has synchronised
         int n = 0;
-        cudaSetDevice(ctx->device);
+        DeviceGuard guard(ctx->device);
         int rq[48];
         if (cudaMemcpy(&n, ctx->d_counters.p, sizeof(int), cudaMemcpyDeviceToHost) == cudaSuccess && ctx->d_rq.p &&
             cudaMemcpy(rq, ctx->d_rq.p, sizeof(rq), cudaMemcpyDeviceToHost) == cudaSuccess && ctx->stats.n_short_warps > 0)
@@ -248,7 +264,8 @@ extern "C" int phmm_forward_batch(phmm_ctx* ctx, const phmm_batch* b, int precis
         return PHMM_E_ARG;
     HostBatchView hv = {b->n_reads, b->n_haps, b->n_pairs, b->h_read_off, b->h_hap_off, b->h_pair_read, b->h_pair_hap};
     RC(validate_batch(hv));
-    CK(cudaSetDevice(ctx->device));
+    DeviceGuard guard(ctx->device);
+    if (!guard.ok) return PHMM_E_CUDA;
     cudaStream_t st = (cudaStream_t)cuda_stream;
     const auto t0 = std::chrono::steady_clock::now();
     const bool fp64 = precision == PHMM_FP64;
@@ -365,6 +382,7 @@ extern "C" int phmm_forward_batch(phmm_ctx* ctx, const phmm_batch* b, int precis
     RC(sg.upload(ps.d_rq_enq, sub_pairs.data(), sub_pairs.size() * 4));
     CK(cudaEventRecord(ps.ev_up, ctx->copy_stream));
     CK(cudaStreamWaitEvent(st, ps.ev_up, 0));
+    CK(cudaStreamWaitEvent(st, ctx->ev_last, 0));  // calls on different streams of one context run one after the other
     // counters: [0] rescue count (= n_items of the rescue launch)  [1] ticket rescue  [2] n strip items  [3] ticket strips
     //           [4] n sequential fp64 items  [5] ticket sequential
     sg.st = st;  // from here on: buffers that kernels write as well, in stream order with them
@@ -380,9 +398,9 @@ extern "C" int phmm_forward_batch(phmm_ctx* ctx, const phmm_batch* b, int precis
     CK(cudaMemsetAsync(ctx->d_rq.p, 0, 48 * 4, st));
     ps.used = true;
     struct FreeMark {  // whatever path leaves the call: the set is free once everything enqueued so far on st has run
-        cudaEvent_t ev; cudaStream_t st;
-        ~FreeMark() { cudaEventRecord(ev, st); }
-    } free_mark{ps.ev_free, st};
+        cudaEvent_t ev, ev_last; cudaStream_t st;
+        ~FreeMark() { cudaEventRecord(ev, st); cudaEventRecord(ev_last, st); }
+    } free_mark{ps.ev_free, ctx->ev_last, st};
 
     DevBatch db;
     db.read_bases = b->d_read_bases; db.qual_base = b->d_qual_base; db.qual_ins = b->d_qual_ins;
@@ -519,7 +537,8 @@ extern "C" int phmm_forward_batch_host(phmm_ctx* ctx, const phmm_batch* b, int p
     if (!h_out || !b->h_read_off || !b->h_hap_off) return PHMM_E_ARG;
     HostBatchView hv = {b->n_reads, b->n_haps, b->n_pairs, b->h_read_off, b->h_hap_off, b->h_pair_read, b->h_pair_hap};
     RC(validate_batch(hv));
-    CK(cudaSetDevice(ctx->device));
+    DeviceGuard guard(ctx->device);
+    if (!guard.ok) return PHMM_E_CUDA;
     const size_t R = (size_t)b->h_read_off[b->n_reads], H = (size_t)b->h_hap_off[b->n_haps];
     const size_t Ra = (R + 255) & ~(size_t)255, Ha = (H + 255) & ~(size_t)255;
     CK(ctx->d_payload.need(5 * Ra + Ha + 256));

@@ -17,10 +17,11 @@
 
 namespace phmm {
 
-// ---- meta word of a stream entry: bits 0-1 read base code (A,C,G,T; other bytes: pm := px, "matches nothing"),
+// ---- meta word of a stream entry: bits 0-2 read base code (A,C,G,T = 0..3, N and every other byte = 4: Eq.3 compares
+// literally, so N matches N and nothing else, reading G17),
 // ROW = a read row (entries 1..l), LAST = the read's last row, FIRST = run-in entry (the group's first lane injects C/k),
 // SUM = the sum entry behind the last row (phmm_rowconst.cuh), on which the running sum s collects Eq.4.
-enum : uint32_t { META_CODE_MASK = 3u, META_ROW = 8u, META_LAST = 16u, META_FIRST = 32u, META_SUM = 64u };
+enum : uint32_t { META_CODE_MASK = 7u, META_ROW = 8u, META_LAST = 16u, META_FIRST = 32u, META_SUM = 64u };
 
 #define PHMM_FULL 0xffffffffu
 

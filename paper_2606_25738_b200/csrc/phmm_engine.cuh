@@ -62,8 +62,8 @@ template <typename T> struct Entry2 {
 // and the sum entry has gamma := 1, pm := 0, px := 1 and base code 0, so that U = T on every column that does not
 // "match" it and the chain s = s + U adds them up across the whole lane group.  What matches the sum entry: the columns
 // behind the haplotype EXCEPT the first one, which holds T = (M+I) of the last real column.  With HS those carry code
-// 0, the first one code 5 and a haplotype 'N' code 6 (5 and 6 match no read base); without HS a fifth match word,
-// hm[4], marks them.  No divergent per-lane summation, no third value handed from lane to lane.
+// 0, the first one code 5 and a haplotype 'N' code 6 (= a read N's code; 5 matches no read base); without HS a sixth match
+// word, hm[5], marks them (hm[4] is the word of N).  No divergent per-lane summation, no third value handed from lane to lane.
 template <typename T, int NV, bool HS = false> struct Lane2 {
     typedef W2<T> P;
     typedef typename P::V V;
@@ -71,7 +71,7 @@ template <typename T, int NV, bool HS = false> struct Lane2 {
 
     V Tt[NV], J[NV];
     V outT, outS;              // what dropped out on the right in the last step: (.x's, .y's)
-    uint32_t hm[HS ? 1 : 5];   // without HS: match words, one per base b: bit x <=> .x column x is b, bit 16+x <=> .y column x is b
+    uint32_t hm[HS ? 1 : 6];   // without HS: match words, one per base b: bit x <=> .x column x is b, bit 16+x <=> .y column x is b
     uint32_t h2[HS ? NV : 1];  // HS: per column the base codes of (.x, .y) as two fp16 numbers (1..4; 5, 6, 0: see above)
 
     __device__ __forceinline__ void init() {
@@ -92,19 +92,19 @@ template <typename T, int NV, bool HS = false> struct Lane2 {
             }
         } else {
 #pragma unroll
-            for (int c = 0; c < 4; c++) hm[c] = 0;
+            for (int c = 0; c < 5; c++) hm[c] = 0;
             const int nvx = min(max(k - j0, 0), NV), nvy = min(max(k - j0 - NV, 0), NV);  // real columns of each half
 #pragma unroll
             for (int x = 0; x < NV; x++) {
                 if (x < nvx) {
                     const int c = base_code(hap[j0 + x]);
 #pragma unroll
-                    for (int q = 0; q < 4; q++) hm[q] |= (c == q ? 1u : 0u) << x;
+                    for (int q = 0; q < 5; q++) hm[q] |= (c == q ? 1u : 0u) << x;
                 }
                 if (x < nvy) {
                     const int c = base_code(hap[j0 + NV + x]);
 #pragma unroll
-                    for (int q = 0; q < 4; q++) hm[q] |= (c == q ? 1u : 0u) << (16 + x);
+                    for (int q = 0; q < 5; q++) hm[q] |= (c == q ? 1u : 0u) << (16 + x);
                 }
             }
             uint32_t v = 0;  // what "matches" the sum entry: columns more than one behind the haplotype's last
@@ -113,7 +113,7 @@ template <typename T, int NV, bool HS = false> struct Lane2 {
                 if (j0 + x > k) v |= 1u << x;
                 if (j0 + NV + x > k) v |= 1u << (16 + x);
             }
-            hm[4] = v;
+            hm[5] = v;
         }
     }
     static __device__ __forceinline__ uint32_t half_code(int c) {  // fp16 bit pattern of the number c + 1
@@ -137,8 +137,10 @@ template <typename T, int NV, bool HS = false> struct Lane2 {
             const uint32_t wx01 = (E.metaX & 1u) ? hm[1] : hm[0], wx23 = (E.metaX & 1u) ? hm[3] : hm[2];
             const uint32_t wy01 = (E.metaY & 1u) ? hm[1] : hm[0], wy23 = (E.metaY & 1u) ? hm[3] : hm[2];
             uint32_t wx = (E.metaX & 2u) ? wx23 : wx01, wy = (E.metaY & 2u) ? wy23 : wy01;
-            wx = (E.metaX & META_SUM) ? hm[4] : wx;  // (the other entries that are no read rows have pm = px = 0)
-            wy = (E.metaY & META_SUM) ? hm[4] : wy;
+            wx = (E.metaX & 4u) ? hm[4] : wx;  // an N row
+            wy = (E.metaY & 4u) ? hm[4] : wy;
+            wx = (E.metaX & META_SUM) ? hm[5] : wx;  // (the other entries that are no read rows have pm = px = 0)
+            wy = (E.metaY & META_SUM) ? hm[5] : wy;
             mw = (wx & 0xffffu) | (wy & 0xffff0000u);
         }
         const uint32_t r2 = E.r2;

@@ -119,11 +119,11 @@ __global__ void __launch_bounds__(RESCUE_WARPS * 32, RESCUE_MIN_CTAS) k_rescue_f
         // ---- haplotype columns of this lane: one match word per base (bit x <=> column x carries that base)
         const int j0 = lg * NV;
         const int nv = active ? min(max(k - j0, 0), NV) : 0;
-        uint32_t hm[4] = {0u, 0u, 0u, 0u};
+        uint32_t hm[5] = {0u, 0u, 0u, 0u, 0u};  // one per base code; [4] = N (Eq.3 compares literally: N matches N only, reading G17)
         for (int x = 0; x < nv; x++) {
             const int c = base_code(b.hap_bases[ho + j0 + x]);
 #pragma unroll
-            for (int q = 0; q < 4; q++) hm[q] |= (c == q ? 1u : 0u) << x;
+            for (int q = 0; q < 5; q++) hm[q] |= (c == q ? 1u : 0u) << x;
         }
         const double Cok = ldexp(1.0, RESCUE_LOG2C) / (double)k;
 
@@ -145,9 +145,9 @@ __global__ void __launch_bounds__(RESCUE_WARPS * 32, RESCUE_MIN_CTAS) k_rescue_f
                     const double eps = s_lut[b.qual_base[ro + e - 1]];
                     const int code = base_code(b.read_bases[ro + e - 1]);
                     px = eps * (1.0 / 3.0);  // within 1 ulp of Eq.3's eps/3; a double division per step would cost ~10 % here
-                    pm = code < 4 ? 1.0 - eps : px;  // a non-ACGT read base matches nothing (reading G17)
+                    pm = 1.0 - eps;
                     const uint32_t m01 = (code & 1) ? hm[1] : hm[0], m23 = (code & 1) ? hm[3] : hm[2];
-                    mw = (code & 2) ? m23 : m01;
+                    mw = (code & 4) ? hm[4] : (code & 2) ? m23 : m01;
                 }
                 if (e < l) {
                     const double io1 = s_lut[b.qual_ins[ro + e]], de1 = s_lut[b.qual_del[ro + e]], ga1 = s_lut[b.qual_gcp[ro + e]];

@@ -36,7 +36,7 @@ __device__ __forceinline__ RowC row_constants(const DevBatch& b, const double* _
         const int i = e;  // read row, 1-based
         const double eps = lut[b.qual_base[off + i - 1]];
         const int code = base_code(b.read_bases[off + i - 1]);
-        c.meta = (uint32_t)(code & 3) | META_ROW | (i == l ? META_LAST : 0u);
+        c.meta = (uint32_t)code | META_ROW | (i == l ? META_LAST : 0u);
         c.gam = lut[b.qual_gcp[off + i - 1]];
         double gin = 1.0;  // gi_{i+1} = g_{i+2} iota_{i+1};  := 1 behind the last row
         if (i < l) {
@@ -52,16 +52,17 @@ __device__ __forceinline__ RowC row_constants(const DevBatch& b, const double* _
         } else {
             c.G = 1.0;
         }
-        c.pm = (code < 4 ? 1.0 - eps : eps / 3.0) * gin;  // a non-ACGT read base matches nothing (reading G17)
+        c.pm = (1.0 - eps) * gin;  // (an N row matches N columns only: literal Eq.3, reading G17)
         c.px = eps / 3.0 * gin;
     }
     return c;
 }
 
 // The 16-bit word an entry contributes to the table / ring: low byte = meta, high byte = upper byte of the fp16 number
-// HSETP2 compares with the per-column base codes (A,C,G,T = 1..4 on read rows, 0 on every other entry).
+// HSETP2 compares with the per-column base codes (A,C,G,T = 1..4, N = 6 on read rows, 0 on every other entry).
 __device__ __forceinline__ uint32_t entry_word16(const RowC& c) {
-    const uint32_t code = (c.meta & META_ROW) ? (uint32_t)((0x4400420040003C00ull >> (16 * (c.meta & META_CODE_MASK))) & 0xff00ull) : 0u;
+    const uint32_t cd = c.meta & META_CODE_MASK;
+    const uint32_t code = !(c.meta & META_ROW) ? 0u : cd < 4 ? (uint32_t)((0x4400420040003C00ull >> (16 * cd)) & 0xff00ull) : 0x4600u;
     return code | (c.meta & 0xffu);
 }
 

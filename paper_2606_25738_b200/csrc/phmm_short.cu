@@ -41,9 +41,6 @@ __global__ void __launch_bounds__(256) k_table_f32(DevBatch b, const double* __r
     const int64_t r = (int64_t)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
     if (r >= b.n_reads) return;
     const int lane = threadIdx.x & 31;
-    const float4 Z = make_float4(0.f, 0.f, 0.f, 0.f);
-    if (blockIdx.x == 0)
-        for (int i = threadIdx.x; i < 4 * TABLE_ZERO_RUN; i += blockDim.x) reinterpret_cast<float4*>(table)[i] = Z;  // whole blocks
     const int64_t off = b.read_off[r];
     const int l = (int)(b.read_off[r + 1] - off);
     float4* dst = reinterpret_cast<float4*>(table);
@@ -62,6 +59,9 @@ cudaError_t launch_lut_table(const DevBatch& b, const double* lut, float* table,
     if (b.n_reads == 0) return cudaSuccess;
     const int wpb = 8;
     int64_t grid = (b.n_reads + wpb - 1) / wpb;
+    // the zero run (whole 32-entry blocks) that idle lanes walk: cleared on every call, whatever the batch size
+    cudaError_t e = cudaMemsetAsync(table, 0, (size_t)TABLE_ZERO_RUN * 64, st);
+    if (e != cudaSuccess) return e;
     k_table_f32<<<(unsigned)grid, wpb * 32, 0, st>>>(b, lut, table);
     return cudaGetLastError();
 }
