@@ -78,12 +78,13 @@ struct phmm_ctx {
     cudaEvent_t ev_last = nullptr;  // end of the device work of the most recent call: the next call's stream waits for it,
                                     // because the table, the counters, the queues and the boundary buffers exist once per context
     DevBuf d_lut, d_table;
-    DevBuf d_counters, d_rescue, d_boundary, d_progress, d_scratch;
+    DevBuf d_counters, d_rescue, d_boundary, d_progress, d_scratch, d_totals;
     DevBuf d_rq, d_rq_queue, d_rq_sorted, d_rq_plan;  // fp64 sub-warp recomputation: counters, queue, ordered queue, plan, FP64-mode input list
     DevBuf d_payload, d_out, d_flags;  // phmm_forward_batch_host only
     std::vector<uint8_t> is_short;
     ShortPlan plan;
-    int chain_grid[2] = {0, 0};
+    int chain_grid[2] = {0, 0};  // resident CTAs of the fp64 chain kernel ([1]; [0] unused)
+    int long_grid = 0, rescue_grid = 0;  // resident CTAs of the fp32 long kernel / of the fp64 sub-warp kernel on this device
     cudaEvent_t ev_prof[8] = {};   // profile_events: [2f], [2f+1] bracket family f (0 table, 1 short, 2 rescue, 3 long)
     bool prof_used[4] = {false, false, false, false};
     bool reuse_table = false;    // host entry, chunks after the first: the row-constant table of this payload is already on the device
@@ -145,8 +146,9 @@ extern "C" int phmm_create(phmm_ctx** out, int device, const phmm_options* opt) 
         phmm_destroy(ctx);
         return PHMM_E_CUDA;
     }
-    ctx->chain_grid[0] = chain_ctas_per_sm(false) * ctx->n_sm;
     ctx->chain_grid[1] = chain_ctas_per_sm(true) * ctx->n_sm;
+    ctx->long_grid = long_ctas_per_sm() * ctx->n_sm;
+    ctx->rescue_grid = rescue_ctas_per_sm() * ctx->n_sm;
     *out = ctx;
     return PHMM_OK;
 }
@@ -155,7 +157,7 @@ extern "C" int phmm_destroy(phmm_ctx* ctx) {
     if (!ctx) return PHMM_E_ARG;
     DeviceGuard guard(ctx->device);
     cudaDeviceSynchronize();
-    DevBuf* bufs[] = {&ctx->d_lut, &ctx->d_table, &ctx->d_counters, &ctx->d_rescue, &ctx->d_boundary, &ctx->d_progress, &ctx->d_scratch,
+    DevBuf* bufs[] = {&ctx->d_lut, &ctx->d_table, &ctx->d_counters, &ctx->d_rescue, &ctx->d_boundary, &ctx->d_progress, &ctx->d_scratch, &ctx->d_totals,
                       &ctx->d_payload, &ctx->d_out, &ctx->d_flags, &ctx->d_rq, &ctx->d_rq_queue, &ctx->d_rq_sorted, &ctx->d_rq_plan};
     for (DevBuf* b : bufs) b->release();
     for (int i = 0; i < 2; i++) {
@@ -276,9 +278,9 @@ extern "C" int phmm_forward_batch(phmm_ctx* ctx, const phmm_batch* b, int precis
     if (ctx->is_short.size() != (size_t)np) ctx->is_short.resize((size_t)np);
     std::vector<int> seq_pairs, strip_pairs, sub_pairs;  // chain kernel work lists, fp64 sub-warp list (caller pair indices)
     int64_t cells = 0, long_cells = 0, lane_rows = 0;  // lane_rows: sum over short pairs of read rows x lanes of the group
-    int max_seq_l = 0;
+    int max_seq_l = 0, max_long_l = 0;  // longest read of the short class / of the long pairs
     {
-        struct Part { std::vector<int> seq, strip, sub; int64_t cells = 0, long_cells = 0, lane_rows = 0; int max_l = 0; };
+        struct Part { std::vector<int> seq, strip, sub; int64_t cells = 0, long_cells = 0, lane_rows = 0; int max_l = 0, max_l_long = 0; };
         Part part[BATCHER_THREADS];
         const int long_k = ctx->opt.long_min_hap_len;
         uint8_t* is_short = ctx->is_short.data();
@@ -289,7 +291,7 @@ extern "C" int phmm_forward_batch(phmm_ctx* ctx, const phmm_batch* b, int precis
                 const int64_t l = b->h_read_off[r + 1] - b->h_read_off[r], k = b->h_hap_off[h + 1] - b->h_hap_off[h];
                 q.cells += l * k;
                 uint8_t sh = 0;
-                if (k > long_k || l > 4096) { q.strip.push_back((int)p); q.long_cells += l * k; }
+                if (k > long_k || l > 4096) { q.strip.push_back((int)p); q.long_cells += l * k; if (l > q.max_l_long) q.max_l_long = (int)l; }
                 else {
                     if (fp64 && k <= RESCUE_MAX_K && l <= RESCUE_MAX_L) q.sub.push_back((int)p);
                     else if (fp64) q.seq.push_back((int)p);
@@ -305,6 +307,7 @@ extern "C" int phmm_forward_batch(phmm_ctx* ctx, const phmm_batch* b, int precis
             sub_pairs.insert(sub_pairs.end(), part[t].sub.begin(), part[t].sub.end());
             cells += part[t].cells; long_cells += part[t].long_cells; lane_rows += part[t].lane_rows;
             if (part[t].max_l > max_seq_l) max_seq_l = part[t].max_l;
+            if (part[t].max_l_long > max_long_l) max_long_l = part[t].max_l_long;
         }
     }
     ctx->stats.n_pairs = np;
@@ -343,7 +346,8 @@ extern "C" int phmm_forward_batch(phmm_ctx* ctx, const phmm_batch* b, int precis
             const int r = b->h_pair_read[p], h = b->h_pair_hap[p];
             const int64_t l = b->h_read_off[r + 1] - b->h_read_off[r], k = b->h_hap_off[h + 1] - b->h_hap_off[h];
             const int ns = (int)((k + strip_cols - 1) / strip_cols);
-            const int64_t nblk = (l + CHAIN_EXTRA_ROWS + 31) / 32;
+            // fp64 chain kernel: 32-row boundary blocks; fp32 long kernel: one 16-byte record per stream entry
+            const int64_t nblk = fp64 ? (l + CHAIN_EXTRA_ROWS + 31) / 32 : l + TABLE_EXTRA_ROWS;
             ps.push_back(PairStrips{p, ns, n_prog, n_bnd_blocks});
             n_bnd_blocks += (int64_t)(ns > 1 ? ns - 1 : 0) * nblk;
             n_prog += ns;  // one counter per strip (the last one is unused)
@@ -410,8 +414,9 @@ extern "C" int phmm_forward_batch(phmm_ctx* ctx, const phmm_batch* b, int precis
     int* counters = (int*)ctx->d_counters.p;
     int launches = 0;
 
-    // ---- short path: row-constant table, systolic kernel, then fp64 rescue of what underflowed
-    if (n_warps > 0) {
+    // ---- fp32: row-constant table of every read (short and long pairs use the same one)
+    const bool long32 = !fp64 && !items.empty();
+    if (n_warps > 0 || long32) {
         const int64_t n_entries = table_run_start(b->h_read_off[b->n_reads], b->n_reads) + 2;
         if (n_entries > INT32_MAX) return PHMM_E_TOOLONG;
         const size_t table_bytes = (size_t)(n_entries + 64) * 64;
@@ -419,8 +424,13 @@ extern "C" int phmm_forward_batch(phmm_ctx* ctx, const phmm_batch* b, int precis
         CK(ctx->d_table.need(table_bytes));
         ctx->stats.table_bytes = (int64_t)table_bytes;
         PROF(0, 0);
-        if (!ctx->reuse_table) CK(launch_lut_table(db, (const double*)ctx->d_lut.p, (float*)ctx->d_table.p, st));
+        if (!ctx->reuse_table)
+            CK(launch_lut_table(db, (const double*)ctx->d_lut.p, (float*)ctx->d_table.p, std::max(max_seq_l, max_long_l), st));
         PROF(0, 1);
+        launches++;
+    }
+    // ---- short path: systolic kernel, then (below) fp64 rescue of what underflowed
+    if (n_warps > 0) {
         ShortLaunch sl;
         sl.table = (const float*)ctx->d_table.p;
         sl.tasks = (const ShortTask*)ps.d_tasks.p;
@@ -439,7 +449,62 @@ extern "C" int phmm_forward_batch(phmm_ctx* ctx, const phmm_batch* b, int precis
         PROF(1, 0);
         CK(launch_short_f32(db, sl, st));
         PROF(1, 1);
-        launches += 2;
+        launches++;
+    }
+    // ---- long path.  fp32: table-driven strips with per-lane exponents (phmm_long.cu); what it cannot represent joins
+    // the rescue list of the fp64 chain launch below.  fp64: concurrent strips of the chain kernel.
+    if (!items.empty()) {
+        CK(ctx->d_progress.need((size_t)n_prog * 4 + 4));
+        CK(cudaMemsetAsync(ctx->d_progress.p, 0, (size_t)n_prog * 4 + 4, st));
+        // no more CTAs than there are strips: with fewer strips than resident warps the block scheduler would fill
+        // some SMs completely and leave others empty (configs[4]: 1648 strips, 2368 slots: 1.36 vs 1.76 TCUPS)
+        const int wpc = fp64 ? chain_warps_per_cta(true) : long_warps_per_cta();
+        const int need_ctas = (int)((items.size() + (size_t)wpc - 1) / (size_t)wpc);
+        PROF(3, 0);
+        if (fp64) {
+            CK(ctx->d_boundary.need((size_t)(n_bnd_blocks + 1) * chain_block_bytes(true)));
+            ChainLaunch cl;
+            memset(&cl, 0, sizeof(cl));
+            cl.items = (const ChainItem*)ps.d_items.p;
+            cl.n_items = counters + 2;
+            cl.ticket = counters + 3;
+            cl.pair_read = (const int*)ps.d_pair_read.p;
+            cl.pair_hap = (const int*)ps.d_pair_hap.p;
+            cl.lut = (const double*)ctx->d_lut.p;
+            cl.boundary = ctx->d_boundary.p;
+            cl.scratch_blocks = 0;
+            cl.progress = (int*)ctx->d_progress.p;
+            cl.out = d_out;
+            cl.flags = d_flags;
+            cl.flag_bits = PHMM_FLAG_LONG;
+            cl.log2C = 0;
+            CK(launch_chain(db, cl, true, false, std::min(ctx->chain_grid[1], need_ctas), st));
+        } else {
+            CK(ctx->d_boundary.need((size_t)(n_bnd_blocks + 1) * 16));
+            CK(ctx->d_totals.need((size_t)n_prog * 16 + 16));
+            LongLaunch ll;
+            memset(&ll, 0, sizeof(ll));
+            ll.table = (const float*)ctx->d_table.p;
+            ll.items = (const ChainItem*)ps.d_items.p;
+            ll.n_items = counters + 2;
+            ll.ticket = counters + 3;
+            ll.pair_read = (const int*)ps.d_pair_read.p;
+            ll.pair_hap = (const int*)ps.d_pair_hap.p;
+            ll.records = (float4*)ctx->d_boundary.p;
+            ll.totals = (float4*)ctx->d_totals.p;
+            ll.progress = (int*)ctx->d_progress.p;
+            ll.out = d_out;
+            ll.flags = d_flags;
+            ll.flag_bits = PHMM_FLAG_LONG;
+            // every strip resident at once (configs[4]): the wavefront's pipeline depth decides, publish often;
+            // many more strips than warp slots: a consumer hardly ever waits, publish (MEMBAR) rarely
+            ll.publish = need_ctas <= ctx->long_grid ? 16 : 64;
+            ll.fallback_count = counters + 0;
+            ll.fallback_list = (int*)ctx->d_rescue.p;
+            CK(launch_long_f32(db, ll, std::min(ctx->long_grid, need_ctas), st));
+        }
+        PROF(3, 1);
+        launches++;
     }
     // fp64 sub-warp kernel: fp32 mode = what the short kernel queued, fp64 mode = the short pairs it can hold
     const bool sub = n_warps > 0 || !sub_pairs.empty();
@@ -463,16 +528,20 @@ extern "C" int phmm_forward_batch(phmm_ctx* ctx, const phmm_batch* b, int precis
         rl.fallback_count = counters + (fp64 ? 4 : 0);
         rl.fallback_list = (int*)ctx->d_rescue.p;
         PROF(2, 0);
-        CK(launch_rescue_f64(db, rl, st));
+        CK(launch_rescue_f64(db, rl, ctx->rescue_grid, st));
         launches += 3 + (fp64 ? 1 : 0);
     }
-    // sequential chain launch: fp32 mode = rescue list (device-side count), fp64 mode = the other non-long pairs;
-    // both also receive what the sub-warp kernel passed on
-    if (n_warps > 0 || n_seq > 0 || sub) {
-        const int grid = ctx->chain_grid[1];
-        const int64_t blocks = (max_seq_l + CHAIN_EXTRA_ROWS + 31) / 32 + 1;
-        const int max_strips_seq = (ctx->opt.long_min_hap_len + chain_strip_cols(true) - 1) / chain_strip_cols(true);
-        size_t scratch = max_strips_seq > 1 ? (size_t)grid * chain_warps_per_cta(true) * 2 * blocks * chain_block_bytes(true) : 256;
+    // sequential chain launch (one warp per pair, its strips in sequence, fp64, rescaled): fp32 mode = the rescue list
+    // (device-side count: short pairs too wide for the sub-warp kernel, what that kernel passed on, long pairs the fp32
+    // long kernel could not represent), fp64 mode = the short-class pairs the sub-warp kernel does not take
+    if (n_warps > 0 || n_seq > 0 || sub || long32) {
+        int grid = ctx->chain_grid[1];
+        const int max_l = long32 ? std::max(max_seq_l, max_long_l) : max_seq_l;
+        const int64_t blocks = (max_l + CHAIN_EXTRA_ROWS + 31) / 32 + 1;
+        const int max_strips_seq = long32 ? 2 : (ctx->opt.long_min_hap_len + chain_strip_cols(true) - 1) / chain_strip_cols(true);
+        const size_t per_cta = (size_t)chain_warps_per_cta(true) * 2 * blocks * chain_block_bytes(true);  // ping-pong boundary buffers
+        if (long32) grid = (int)std::max<size_t>(8, std::min<size_t>((size_t)grid, ((size_t)1 << 30) / per_cta));  // fallbacks of long pairs are rare: at most 1 GiB
+        size_t scratch = max_strips_seq > 1 ? (size_t)grid * per_cta : 256;
         CK(ctx->d_scratch.need(scratch));
         ChainLaunch cl;
         memset(&cl, 0, sizeof(cl));
@@ -488,40 +557,11 @@ extern "C" int phmm_forward_batch(phmm_ctx* ctx, const phmm_batch* b, int precis
         cl.out = d_out;
         cl.flags = d_flags;
         cl.flag_bits = fp64 ? 0 : PHMM_FLAG_RESCUED;
+        cl.long_k = ctx->opt.long_min_hap_len;
         cl.log2C = 0;
         if (!sub) PROF(2, 0);
         CK(launch_chain(db, cl, true, true, grid, st));
         PROF(2, 1);
-        launches++;
-    }
-    // ---- long path: concurrent strips in the requested precision
-    if (!items.empty()) {
-        CK(ctx->d_boundary.need((size_t)(n_bnd_blocks + 1) * chain_block_bytes(fp64)));
-        CK(ctx->d_progress.need((size_t)n_prog * 4 + 4));
-        CK(cudaMemsetAsync(ctx->d_progress.p, 0, (size_t)n_prog * 4 + 4, st));
-        ChainLaunch cl;
-        memset(&cl, 0, sizeof(cl));
-        cl.items = (const ChainItem*)ps.d_items.p;
-        cl.n_items = counters + 2;
-        cl.ticket = counters + 3;
-        cl.pair_read = (const int*)ps.d_pair_read.p;
-        cl.pair_hap = (const int*)ps.d_pair_hap.p;
-        cl.lut = (const double*)ctx->d_lut.p;
-        cl.boundary = ctx->d_boundary.p;
-        cl.scratch_blocks = 0;
-        cl.progress = (int*)ctx->d_progress.p;
-        cl.out = d_out;
-        cl.flags = d_flags;
-        cl.flag_bits = PHMM_FLAG_LONG;
-        cl.log2C = 0;
-        PROF(3, 0);
-        // no more CTAs than there are strips: with fewer strips than resident warps the block scheduler would fill
-        // some SMs completely and leave others empty (configs[4]: 1648 strips, 2368 slots: 1.36 vs 1.76 TCUPS)
-        const int wpc = chain_warps_per_cta(fp64);
-        const int need_ctas = (int)((items.size() + (size_t)wpc - 1) / (size_t)wpc);
-        const bool few = need_ctas <= 3 * ctx->n_sm;  // every strip resident even at 3 CTAs per SM
-        CK(launch_chain(db, cl, fp64, false, std::min(ctx->chain_grid[fp64 ? 1 : 0], need_ctas), st, few));
-        PROF(3, 1);
         launches++;
     }
     ctx->stats.n_kernel_launches = launches;

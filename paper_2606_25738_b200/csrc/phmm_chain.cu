@@ -1,4 +1,4 @@
-// Generic rescaled path ("chain" kernel): one warp = one strip of 32 lanes x 2NV haplotype columns of
+// Rescaled fp64 path ("chain" kernel; the fp32 long path is phmm_long.cu): one warp = one strip of 32 lanes x 2NV haplotype columns of
 // one pair; the strips of a pair are chained left to right through boundary-column buffers in
 // global memory (per stream entry: the running sum s and the T that drop out of the strip's last
 // column, and the producing thread's block exponent), either concurrently (one strip per
@@ -337,7 +337,7 @@ k_chain(DevBatch b, ChainLaunch p, int items_are_pairs) {
                         // strip has the last one in what this lane handed out one step ago instead
                         const T sum = full_last ? ln.outS.y + prevT : ln.outS.y;
                         p.out[pair] = log10((double)sum) + ((double)ex - (double)p.log2C) * LOG10_2;
-                        if (p.flags) p.flags[pair] = p.flag_bits;
+                        if (p.flags) p.flags[pair] = p.flag_bits | ((items_are_pairs && (k > p.long_k || l > 4096)) ? 2u /* PHMM_FLAG_LONG */ : 0u);
                     }
                 }
             }
@@ -346,34 +346,22 @@ k_chain(DevBatch b, ChainLaunch p, int items_are_pairs) {
     }
 }
 
-constexpr int WPC_F32 = 4, WPC_F64 = 2;
-// fp32 comes in two register budgets: 4 CTAs/SM x 128 registers for throughput (many more strips than warp slots),
-// 3 CTAs/SM x ~166 registers when every strip is resident anyway and the pipeline depth of the wavefront decides
-// (configs[4]: 1.76 vs 1.63 TCUPS; configs[3]: 1.93 vs 2.01)
-constexpr int MINB_F32_MANY = CHAIN_MIN_CTAS_F32, MINB_F32_FEW = 3, MINB_F64 = 2;
+constexpr int WPC_F64 = 2, MINB_F64 = 2;
 
-cudaError_t launch_chain(const DevBatch& b, const ChainLaunch& p, bool fp64, bool items_are_pairs, int grid_ctas,
-                         cudaStream_t st, bool few_items) {
+cudaError_t launch_chain(const DevBatch& b, const ChainLaunch& p, bool fp64, bool items_are_pairs, int grid_ctas, cudaStream_t st) {
     if (grid_ctas <= 0) return cudaSuccess;
-    if (fp64)
-        k_chain<double, CHAIN_NV_F64, WPC_F64, MINB_F64><<<grid_ctas, WPC_F64 * 32, 0, st>>>(b, p, items_are_pairs ? 1 : 0);
-    else if (few_items)
-        k_chain<float, CHAIN_NV_F32, WPC_F32, MINB_F32_FEW><<<grid_ctas, WPC_F32 * 32, 0, st>>>(b, p, items_are_pairs ? 1 : 0);
-    else
-        k_chain<float, CHAIN_NV_F32, WPC_F32, MINB_F32_MANY><<<grid_ctas, WPC_F32 * 32, 0, st>>>(b, p, items_are_pairs ? 1 : 0);
+    if (!fp64) return cudaErrorInvalidValue;  // the fp32 long path is phmm_long.cu
+    k_chain<double, CHAIN_NV_F64, WPC_F64, MINB_F64><<<grid_ctas, WPC_F64 * 32, 0, st>>>(b, p, items_are_pairs ? 1 : 0);
     return cudaGetLastError();
 }
 
-int chain_ctas_per_sm(bool fp64) {
+int chain_ctas_per_sm(bool) {
     int n = 0;
-    if (fp64)
-        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, k_chain<double, CHAIN_NV_F64, WPC_F64, MINB_F64>, WPC_F64 * 32, 0);
-    else
-        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, k_chain<float, CHAIN_NV_F32, WPC_F32, MINB_F32_MANY>, WPC_F32 * 32, 0);
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, k_chain<double, CHAIN_NV_F64, WPC_F64, MINB_F64>, WPC_F64 * 32, 0);
     return n > 0 ? n : 1;
 }
-int chain_warps_per_cta(bool fp64) { return fp64 ? WPC_F64 : WPC_F32; }
-size_t chain_block_bytes(bool fp64) { return fp64 ? sizeof(Rec<double>) : sizeof(Rec<float>); }
-int chain_strip_cols(bool fp64) { return 32 * 2 * (fp64 ? CHAIN_NV_F64 : CHAIN_NV_F32); }
+int chain_warps_per_cta(bool) { return WPC_F64; }
+size_t chain_block_bytes(bool) { return sizeof(Rec<double>); }
+int chain_strip_cols(bool fp64) { return fp64 ? 32 * 2 * CHAIN_NV_F64 : SHORT_MAX_K; }
 
 }  // namespace phmm

@@ -101,7 +101,29 @@ struct ChainLaunch {
     uint8_t* flags;
     uint8_t flag_bits;         // written to flags[pair]
     int log2C;                 // scale constant C = 2^log2C of Eq.1 (0 for the rescaled kernels)
+    int long_k;                // items_are_pairs: pairs with a haplotype longer than this (or a read over 4096) also get PHMM_FLAG_LONG
 };
+
+struct LongLaunch {  // fp32 long path (phmm_long.cu): strips of 32 lanes x 32 columns, table-driven like the short kernel
+    const float* table;        // the row-constant table of k_table_f32 (must cover the reads of every long pair)
+    const ChainItem* items;    // strip-major; buf0 = index of the pair's first boundary record
+    const int* n_items;
+    int* ticket;               // zeroed before the launch
+    const int* pair_read;
+    const int* pair_hap;
+    float4* records;           // per pair and strip boundary: l + 3 records {s, T, exponent, -}
+    float4* totals;            // per progress counter: the Eq.4 total of the strips up to this one {lo, hi of a double, exponent, -}
+    int* progress;             // per pair and strip: entries published (l + 4 once the total is there); zeroed before the launch
+    double* out;
+    uint8_t* flags;
+    uint8_t flag_bits;
+    int publish;               // entries per progress publication: a power of two >= 16
+    int* fallback_count;       // pairs whose fp32 result is not a normal positive number: list for the fp64 chain kernel
+    int* fallback_list;
+};
+cudaError_t launch_long_f32(const DevBatch& b, const LongLaunch& p, int grid_ctas, cudaStream_t st);
+int long_ctas_per_sm();
+int long_warps_per_cta();
 
 struct RescueLaunch {
     RescueQueue queue;
@@ -119,16 +141,17 @@ struct RescueLaunch {
     int* fallback_count;       // pairs the unrescaled fp64 pass could not represent: queued for the chain kernel
     int* fallback_list;
 };
-cudaError_t launch_rescue_f64(const DevBatch& b, const RescueLaunch& r, cudaStream_t st);
+cudaError_t launch_rescue_f64(const DevBatch& b, const RescueLaunch& r, int grid_ctas, cudaStream_t st);
+int rescue_ctas_per_sm();
 
-cudaError_t launch_lut_table(const DevBatch& b, const double* lut, float* table, cudaStream_t st);
+cudaError_t launch_lut_table(const DevBatch& b, const double* lut, float* table, int max_read_len, cudaStream_t st);
 cudaError_t launch_short_f32(const DevBatch& b, const ShortLaunch& p, cudaStream_t st);
 // rescue_from_list: items are taken from p.items[...] as plain pair indices in `rescue_list` form
 cudaError_t launch_chain(const DevBatch& b, const ChainLaunch& p, bool fp64, bool items_are_pairs, int grid_ctas,
-                         cudaStream_t st, bool few_items = false);
+                         cudaStream_t st);
 int chain_ctas_per_sm(bool fp64);
 int chain_warps_per_cta(bool fp64);
 size_t chain_block_bytes(bool fp64);  // bytes of one 32-row boundary block
-int chain_strip_cols(bool fp64);      // haplotype columns covered by one strip
+int chain_strip_cols(bool fp64);      // haplotype columns covered by one strip (fp32 long kernel: SHORT_MAX_K)
 
 }  // namespace phmm

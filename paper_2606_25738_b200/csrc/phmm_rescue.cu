@@ -202,16 +202,13 @@ __global__ void __launch_bounds__(RESCUE_WARPS * 32, RESCUE_MIN_CTAS) k_rescue_f
     }
 }
 
-static int g_rescue_grid = 0;
+int rescue_ctas_per_sm() {
+    int n = 0;
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, k_rescue_f64, RESCUE_WARPS * 32, 0);
+    return n > 0 ? n : 1;
+}
 
-cudaError_t launch_rescue_f64(const DevBatch& b, const RescueLaunch& r, cudaStream_t st) {
-    if (g_rescue_grid == 0) {
-        int n = 0, dev = 0, sms = 0;
-        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, k_rescue_f64, RESCUE_WARPS * 32, 0);
-        cudaGetDevice(&dev);
-        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-        g_rescue_grid = (n > 0 ? n : 1) * (sms > 0 ? sms : 148);
-    }
+cudaError_t launch_rescue_f64(const DevBatch& b, const RescueLaunch& r, int grid_ctas, cudaStream_t st) {
     RescueQueue rq = r.queue;
     if (r.enqueue_pairs && r.n_enqueue > 0)
         k_rescue_enqueue<<<(r.n_enqueue + 255) / 256, 256, 0, st>>>(b, rq, r.enqueue_pairs, r.n_enqueue, r.pair_hap);
@@ -221,7 +218,7 @@ cudaError_t launch_rescue_f64(const DevBatch& b, const RescueLaunch& r, cudaStre
     a.sorted = r.sorted; a.cnt = rq.cnt; a.plan = r.plan; a.ticket = rq.cnt + 33;
     a.pair_read = r.pair_read; a.pair_hap = r.pair_hap; a.lut = r.lut; a.out = r.out; a.flags = r.flags; a.flag_bits = r.flag_bits;
     a.fallback_count = r.fallback_count; a.fallback_list = r.fallback_list; a.fallback_stat = rq.cnt + 40;
-    k_rescue_f64<<<g_rescue_grid, RESCUE_WARPS * 32, 0, st>>>(b, a);
+    k_rescue_f64<<<grid_ctas, RESCUE_WARPS * 32, 0, st>>>(b, a);
     return cudaGetLastError();
 }
 

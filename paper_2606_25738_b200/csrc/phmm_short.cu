@@ -6,6 +6,7 @@
 #include "phmm_engine.cuh"
 #include "phmm_kernels.h"
 #include "phmm_rowconst.cuh"
+#include "phmm_table.cuh"
 #include <type_traits>
 
 // Tunables, each with the measurement that chose it (configs[1], in-kernel TCUPS)
@@ -27,16 +28,12 @@ namespace phmm {
 // The table starts with TABLE_ZERO_RUN all-zero entries (what idle lanes fetch); read r's run starts at
 // entry table_run_start(read_off[r], r) (even; phmm_kernels.h).  Constants are formed in double from the
 // 10^(-q/10) table and rounded once ("q32" table; Listing 2 :293-295 for which
-// qualities enter which transition).  One warp per read.
+// qualities enter which transition).  One warp per read and chunk of 1024 entries (blockIdx.y = chunk).
 // Memory layout: the entries are permuted inside blocks of 32 so that the lanes of a warp, which read entries
 // two apart (lane L's .x half is 2L entries behind lane 0's), touch consecutive 16-byte slots: block = 2 KB =
 // 4 chunk planes (the four float4 of an entry) x 2 parities x 16 slots.  A lane-strided LDG.128 then costs
 // ~4 L1 wavefronts instead of 32 (ncu: l1tex throughput 90 % -> see profiles/).
-constexpr int TABLE_CHUNK_STRIDE = 32;  // float4 units between the chunk planes of a block
-__host__ __device__ __forceinline__ int64_t table_slot(int64_t pos) {  // float4 index of chunk 0 of entry pos
-    return (pos >> 5) * 128 + (pos & 1) * 16 + ((pos >> 1) & 15);
-}
-
+constexpr int TABLE_CHUNK_ENTRIES = 1024;
 __global__ void __launch_bounds__(256) k_table_f32(DevBatch b, const double* __restrict__ lut, float* __restrict__ table) {
     const int64_t r = (int64_t)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
     if (r >= b.n_reads) return;
@@ -45,7 +42,8 @@ __global__ void __launch_bounds__(256) k_table_f32(DevBatch b, const double* __r
     const int l = (int)(b.read_off[r + 1] - off);
     float4* dst = reinterpret_cast<float4*>(table);
     const int64_t first = table_run_start(off, r);
-    for (int e = lane; e < table_run_len(l); e += 32) {  // (an entry behind the flush entry is all zero too)
+    const int e_hi = min(table_run_len(l), ((int)blockIdx.y + 1) * TABLE_CHUNK_ENTRIES);
+    for (int e = (int)blockIdx.y * TABLE_CHUNK_ENTRIES + lane; e < e_hi; e += 32) {  // (an entry behind the flush entry is all zero too)
         const RowC x = row_constants(b, lut, off, l, e, true), y = row_constants(b, lut, off, l, e - 1, true);
         float4* d = dst + table_slot(first + e);
         d[0 * TABLE_CHUNK_STRIDE] = make_float4((float)x.gam, (float)y.gam, (float)x.A, (float)y.A);
@@ -55,14 +53,15 @@ __global__ void __launch_bounds__(256) k_table_f32(DevBatch b, const double* __r
     }
 }
 
-cudaError_t launch_lut_table(const DevBatch& b, const double* lut, float* table, cudaStream_t st) {
+cudaError_t launch_lut_table(const DevBatch& b, const double* lut, float* table, int max_read_len, cudaStream_t st) {
     if (b.n_reads == 0) return cudaSuccess;
     const int wpb = 8;
     int64_t grid = (b.n_reads + wpb - 1) / wpb;
+    const int chunks = (table_run_len(max_read_len) + TABLE_CHUNK_ENTRIES - 1) / TABLE_CHUNK_ENTRIES;
     // the zero run (whole 32-entry blocks) that idle lanes walk: cleared on every call, whatever the batch size
     cudaError_t e = cudaMemsetAsync(table, 0, (size_t)TABLE_ZERO_RUN * 64, st);
     if (e != cudaSuccess) return e;
-    k_table_f32<<<(unsigned)grid, wpb * 32, 0, st>>>(b, lut, table);
+    k_table_f32<<<dim3((unsigned)grid, (unsigned)chunks), wpb * 32, 0, st>>>(b, lut, table);
     return cudaGetLastError();
 }
 
@@ -77,22 +76,6 @@ struct Cursor {
     int npos, nend;      // the run after it: the next read of the task, or the zero run
     int q;               // reads of the task already handed to (npos, nend)
 };
-
-// read-only load that asks L2 to fetch the 256-byte pair of lines on a miss: the second line holds the slots this
-// lane group reads 16 steps later
-__device__ __forceinline__ float4 ldg_pf(const float4* p) {
-    float4 v;
-    asm volatile("ld.global.nc.L2::256B.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "l"(p));
-    return v;
-}
-
-__device__ __forceinline__ uint32_t ldg_pf_u32(const uint32_t* p) {
-    uint32_t v;
-    asm volatile("ld.global.nc.L2::256B.b32 %0, [%1];" : "=r"(v) : "l"(p));
-    return v;
-}
-
-struct RawEntry { float4 a, b, c; uint32_t w; };
 
 template <int NV>
 __global__ void __launch_bounds__(SHORT_WARPS_PER_CTA * 32, SHORT_MIN_CTAS) k_short_f32(DevBatch b, ShortLaunch p) {
