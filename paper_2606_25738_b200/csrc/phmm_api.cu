@@ -419,7 +419,7 @@ extern "C" int phmm_forward_batch(phmm_ctx* ctx, const phmm_batch* b, int precis
     if (n_warps > 0 || long32) {
         const int64_t n_entries = table_run_start(b->h_read_off[b->n_reads], b->n_reads) + 2;
         if (n_entries > INT32_MAX) return PHMM_E_TOOLONG;
-        const size_t table_bytes = (size_t)(n_entries + 64) * 64;
+        const size_t table_bytes = (size_t)(n_entries + 192) * 64;  // (slack: the long kernel prefetches up to 96 entries past a run)
         if ((int64_t)table_bytes > ctx->opt.max_table_bytes) return PHMM_E_NOMEM;
         CK(ctx->d_table.need(table_bytes));
         ctx->stats.table_bytes = (int64_t)table_bytes;

@@ -120,6 +120,7 @@ __global__ void __launch_bounds__(LONG_WPC * 32, LONG_MIN_CTAS) k_long_f32(DevBa
         float4* outrec = p.records + it.buf0 + (int64_t)strip * n_ent;
         const int* inprog = p.progress + it.prog0 + strip - 1;
         int* outprog = p.progress + it.prog0 + strip;
+        const bool store_out = has_out && lane == 31;
         const float Cok = (float)(1.0 / (double)k);                // Eq.1 with C = 1 (the exponents do the scaling)
 
         L ln;
@@ -150,6 +151,16 @@ __global__ void __launch_bounds__(LONG_WPC * 32, LONG_MIN_CTAS) k_long_f32(DevBa
 
         // ---- an event: new exponents for all lanes, the next 16 boundary records for lane 0
         auto event = [&](int s) {
+            // what lane 31 has stored so far becomes visible to the next strip (release: MEMBAR + strong store)
+            if (store_out && s > 63 && (s & (p.publish - 1)) == 0) st_release_gpu(outprog, min(s - 63, n_ent));
+            // the table lines lane 0 will reach 64 steps from now: 8 lines (4 chunk planes x 2 parities) of half a 32-entry block
+            {
+                const int t = __shfl_sync(PHMM_FULL, pos, 0) + 64;
+                if (lane < 8) {
+                    const float4* q = tab + (((int64_t)(t >> 5)) << 7) + ((lane >> 1) * TABLE_CHUNK_STRIDE + (lane & 1) * 16 + ((t >> 4) & 1) * 8);
+                    asm volatile("prefetch.global.L2 [%0];" ::"l"(q));
+                }
+            }
             float4 rec = make_float4(0.f, 0.f, 0.f, 0.f);
             int bmax = LONG_FLOOR;
             if (has_in && s < n_ent) {  // (warp-uniform)
@@ -247,11 +258,9 @@ __global__ void __launch_bounds__(LONG_WPC * 32, LONG_MIN_CTAS) k_long_f32(DevBa
                 }
             }
             // ---- right boundary: lane 31's .y half has just finished entry s - 63
-            const int eo = s - 63;
-            if (has_out && lane == 31 && eo >= 0 && eo < n_ent) {
-                st_strong_f4(outrec + eo, make_float4(ln.outS.y, ln.outT.y, __int_as_float(ex), 0.f));
-                if (((eo + 1) & (p.publish - 1)) == 0 || eo == n_ent - 1) st_release_gpu(outprog, eo + 1);
-            }
+            // (published at the next event, or with the Eq.4 total behind the loop)
+            if (store_out && (unsigned)(s - 63) < (unsigned)n_ent)
+                st_strong_f4(outrec + (s - 63), make_float4(ln.outS.y, ln.outT.y, __int_as_float(ex), 0.f));
         };
 
         RawEntry eA, eB;
