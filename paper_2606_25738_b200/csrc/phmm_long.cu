@@ -85,6 +85,7 @@ extern "C" int phmm_debug_read(float* dst, int n) { return (int)cudaMemcpyFromSy
 #endif
 
 struct LongSmem {
+    float4 ring[4 * 128];    // 4 table blocks of 32 entries (2 KB each, in the table's own layout)
     float2 rin[LONG_EVERY];  // the boundary values lane 0 consumes in the next 16 steps, already at its exponent
 };
 
@@ -93,8 +94,11 @@ __global__ void __launch_bounds__(LONG_WPC * 32, LONG_MIN_CTAS) k_long_f32(DevBa
     typedef Lane2<float, NV, true> L;
     constexpr int N2 = 2 * NV;
     constexpr int STRIP = 32 * N2;
-    __shared__ LongSmem sm_all[LONG_WPC];
+    __shared__ __align__(16) LongSmem sm_all[LONG_WPC];
+    __shared__ __align__(16) float4 sm_zero[128];  // an all-zero table block
     LongSmem& sm = sm_all[threadIdx.x >> 5];
+    for (int i = threadIdx.x; i < 128; i += blockDim.x) sm_zero[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+    __syncthreads();
     const int lane = threadIdx.x & 31;
     const double LOG10_2 = 0.30102999566398119521;
     const int n_items = *p.n_items;
@@ -132,35 +136,47 @@ __global__ void __launch_bounds__(LONG_WPC * 32, LONG_MIN_CTAS) k_long_f32(DevBa
         float fin_m = 0.f;     // this lane's share of Eq.4 and its exponent
         int fin_e = LONG_FLOOR;
 
-        // ---- fetch: the zero run until the stream reaches this lane (2*lane steps), the read's run, the zero run again
-        int pos = TABLE_ZERO_RUN - 2 * lane, end = TABLE_ZERO_RUN, npos = run0, nend = run0 + run_len;
-        const float4* e_even = tab;
-        auto load_entry = [&](RawEntry& re, const float4* e) {
-            re.a = ldg_pf(e);
-            re.b = ldg_pf(e + TABLE_CHUNK_STRIDE);
-            re.c = ldg_pf(e + 2 * TABLE_CHUNK_STRIDE);
-            re.w = ldg_pf_u32(reinterpret_cast<const uint32_t*>(e + 3 * TABLE_CHUNK_STRIDE));
+        // ---- fetch.  The table blocks (32 entries = 2 KB, phmm_table.cuh) the warp is walking live in a ring of 4 blocks in
+        // shared memory, filled by cp.async one block (32 steps) ahead of lane 0: the step never waits for L2 or DRAM.
+        // Lane L's .x half is at table position run0 + s - 2L at step s; before its stream starts and after it has ended a
+        // lane reads the all-zero block instead.  Block B sits in ring slot B & 3: when lane 0 enters block B, lane 31 (62
+        // entries behind) is in block B-2, so slot (B+1) & 3 = (B-3) & 3 is free for block B+1.
+        const uint32_t ring_s = (uint32_t)__cvta_generic_to_shared(sm.ring);
+        const uint32_t zero_s = (uint32_t)__cvta_generic_to_shared(sm_zero);
+        auto fill = [&](int blk) {
+            const char* g = reinterpret_cast<const char*>(tab) + ((int64_t)blk << 11) + lane * 16;
+            const uint32_t d = ring_s + ((blk & 3) << 11) + lane * 16;
+#pragma unroll
+            for (int j = 0; j < 4; j++)
+                asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(d + j * 512), "l"(g + j * 512) : "memory");
+            asm volatile("cp.async.commit_group;" ::: "memory");
         };
-        auto fetch_even = [&](RawEntry& re, uint32_t dep) {  // (see phmm_short.cu for the dependent address)
-            if (pos == end) { pos = npos; end = nend; npos = 0; nend = TABLE_ZERO_RUN; }
-            e_even = tab + ((((int64_t)(pos >> 5)) << 7) + (int64_t)(((pos >> 1) & 15) + (dep >> 31)));
-            pos += 2;
+        auto fill_wait = [&]() {
+            asm volatile("cp.async.wait_group 0;" ::: "memory");
+            __syncwarp();
+        };
+        uint32_t e_even = zero_s;  // shared-memory address of chunk 0 of the even entry
+        auto load_entry = [&](RawEntry& re, uint32_t e) {
+            asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(re.a.x), "=f"(re.a.y), "=f"(re.a.z), "=f"(re.a.w) : "r"(e));
+            asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4+512];" : "=f"(re.b.x), "=f"(re.b.y), "=f"(re.b.z), "=f"(re.b.w) : "r"(e));
+            asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4+1024];" : "=f"(re.c.x), "=f"(re.c.y), "=f"(re.c.z), "=f"(re.c.w) : "r"(e));
+            asm volatile("ld.shared.b32 %0, [%1+1536];" : "=r"(re.w) : "r"(e));
+        };
+        auto fetch_even = [&](RawEntry& re, int s) {  // the entry of (even) step s
+            const int v = s - 2 * lane;
+            const int pos = run0 + v;
+            e_even = (unsigned)v < (unsigned)run_len ? ring_s + (((pos >> 5) & 3) << 11) + (((pos >> 1) & 15) << 4) : zero_s;
             load_entry(re, e_even);
         };
-        auto fetch_odd = [&](RawEntry& re, uint32_t dep) { load_entry(re, e_even + (16 + (dep >> 31))); };
+        auto fetch_odd = [&](RawEntry& re) { load_entry(re, e_even + 256); };  // (runs have even lengths: same block, same range)
+        fill(run0 >> 5);
+        fill((run0 >> 5) + 1);
+        fill_wait();
 
         // ---- an event: new exponents for all lanes, the next 16 boundary records for lane 0
         auto event = [&](int s) {
             // what lane 31 has stored so far becomes visible to the next strip (release: MEMBAR + strong store)
             if (store_out && s > 63 && (s & (p.publish - 1)) == 0) st_release_gpu(outprog, min(s - 63, n_ent));
-            // the table lines lane 0 will reach 64 steps from now: 8 lines (4 chunk planes x 2 parities) of half a 32-entry block
-            {
-                const int t = __shfl_sync(PHMM_FULL, pos, 0) + 64;
-                if (lane < 8) {
-                    const float4* q = tab + (((int64_t)(t >> 5)) << 7) + ((lane >> 1) * TABLE_CHUNK_STRIDE + (lane & 1) * 16 + ((t >> 4) & 1) * 8);
-                    asm volatile("prefetch.global.L2 [%0];" ::"l"(q));
-                }
-            }
             float4 rec = make_float4(0.f, 0.f, 0.f, 0.f);
             int bmax = LONG_FLOOR;
             if (has_in && s < n_ent) {  // (warp-uniform)
@@ -264,13 +280,17 @@ __global__ void __launch_bounds__(LONG_WPC * 32, LONG_MIN_CTAS) k_long_f32(DevBa
         };
 
         RawEntry eA, eB;
-        fetch_even(eA, 0u);
+        fetch_even(eA, 0);
         const int steps = run_len + 64;  // even; lane 31's .y half finishes entry run_len - 1 >= n_ent - 1 at step run_len + 62
         for (int s = 0; s < steps; s += 2) {
             if ((s & (LONG_EVERY - 1)) == 0) event(s);
-            fetch_odd(eB, eA.w);
+            if (((run0 + s + 2) & 31) == 0) {  // lane 0's next fetch enters a new block (now complete): the one after it starts its way in
+                fill_wait();
+                fill(((run0 + s + 2) >> 5) + 1);
+            }
+            fetch_odd(eB);
             one_step(eA, s);
-            fetch_even(eA, eB.w);
+            fetch_even(eA, s + 2);
             one_step(eB, s + 1);
         }
 
