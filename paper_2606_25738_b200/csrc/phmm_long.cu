@@ -28,11 +28,10 @@
 // (the incoming s is cut to 0 on the sum entry) at its own exponent; the 32 (sum, exponent) pairs are combined once per
 // strip, and the strips of a pair pass the running total along their chain (one (sum, exponent) slot per strip).
 //
-// Handoff between strips (a6/a7).  Lane 31 stores one 16-byte record {s, T, ex, -} per stream entry and publishes a
-// progress counter every `publish` entries (st.release.gpu: MEMBAR + strong store, no L1 invalidation).  The consumer's
-// lanes 0-15 poll that counter with relaxed loads only when the producer was not known to be finished, and read the
-// records with strong (L2) loads: nothing here invalidates L1, which holds the table windows of every warp of the SM
-// (an acquire load or __threadfence would: CCTL.IVALL).  Items are taken by ticket in strip-major order, so a strip's
+// Handoff between strips (a6/a7).  One 16-byte record {s, T, ex, -} per stream entry from lane 31, and a
+// progress counter every `publish` entries (st.release.gpu: MEMBAR + strong store, no L1 invalidation).  The records are
+// staged in shared memory and flushed, 16 at a time, at the events.  The consumer's lanes 0-15 poll that counter with relaxed
+// loads only when the producer was not known to be far enough, and read the records with strong (L2) loads.  Items are taken by ticket in strip-major order, so a strip's
 // producer always holds an earlier ticket: forward progress without co-residency assumptions.
 #include "phmm_engine.cuh"
 #include "phmm_kernels.h"
@@ -79,14 +78,15 @@ __device__ __forceinline__ float scale2(float v, int d) {
     return v * pow2f(h) * pow2f(d - h);
 }
 
-#ifdef LONG_DEBUG
-__device__ float g_dbg[1 << 16];
-extern "C" int phmm_debug_read(float* dst, int n) { return (int)cudaMemcpyFromSymbol(dst, g_dbg, (size_t)n * 4); }
-#endif
 
+// Shared memory of one warp.  The ring holds the 4 table blocks (32 entries = 2 KB each) the warp is walking, re-laid so
+// that a lane's fetch address advances by 16 bytes per two steps and wraps inside a 1 KB window: chunk plane c (the c-th
+// float4 of an entry) at c * 2048, the odd entries 1024 bytes behind the even ones, entry pos at ((pos >> 1) & 63) * 16.
 struct LongSmem {
-    float4 ring[4 * 128];    // 4 table blocks of 32 entries (2 KB each, in the table's own layout)
-    float2 rin[LONG_EVERY];  // the boundary values lane 0 consumes in the next 16 steps, already at its exponent
+    float4 ring[4 * 128];
+    float2 rin[LONG_EVERY];   // boundary values lane 0 consumes in the next 16 steps, already at its exponent
+    float2 rout[LONG_EVERY];  // what lane 31 handed out in the last 16 steps (flushed to the records at the next event)
+    float2 fin[32];           // per lane: its share of Eq.4 and the exponent it is stored at
 };
 
 template <int NV>
@@ -94,15 +94,18 @@ __global__ void __launch_bounds__(LONG_WPC * 32, LONG_MIN_CTAS) k_long_f32(DevBa
     typedef Lane2<float, NV, true> L;
     constexpr int N2 = 2 * NV;
     constexpr int STRIP = 32 * N2;
-    __shared__ __align__(16) LongSmem sm_all[LONG_WPC];
-    __shared__ __align__(16) float4 sm_zero[128];  // an all-zero table block
+    __shared__ __align__(128) LongSmem sm_all[LONG_WPC];
+    __shared__ __align__(16) float4 sm_zero[512];  // all-zero entries for lanes outside their stream (same offsets as the ring)
     LongSmem& sm = sm_all[threadIdx.x >> 5];
-    for (int i = threadIdx.x; i < 128; i += blockDim.x) sm_zero[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+    for (int i = threadIdx.x; i < 512; i += blockDim.x) sm_zero[i] = make_float4(0.f, 0.f, 0.f, 0.f);
     __syncthreads();
     const int lane = threadIdx.x & 31;
     const double LOG10_2 = 0.30102999566398119521;
     const int n_items = *p.n_items;
-    const float4* tab = reinterpret_cast<const float4*>(p.table);
+    const char* tab = reinterpret_cast<const char*>(p.table);
+    const uint32_t ring_s = (uint32_t)__cvta_generic_to_shared(sm.ring);
+    const uint32_t zero_s = (uint32_t)__cvta_generic_to_shared(sm_zero);
+    const uint32_t rin_s = (uint32_t)__cvta_generic_to_shared(sm.rin);  // rout follows at +128
 
     for (;;) {
         int ticket = 0;
@@ -118,14 +121,6 @@ __global__ void __launch_bounds__(LONG_WPC * 32, LONG_MIN_CTAS) k_long_f32(DevBa
         const int run0 = (int)table_run_start(ro, r), run_len = table_run_len(l);
         const int nstrips = (k + STRIP - 1) / STRIP;
         const bool has_in = strip > 0, has_out = strip + 1 < nstrips;
-        const int k_loc = min(k - strip * STRIP, STRIP);          // real columns of this strip
-        const int out_lane = (k_loc - 1) / N2;                      // the lane that holds the strip's last real column
-        const float4* inrec = p.records + it.buf0 + (int64_t)(strip - 1) * n_ent;
-        float4* outrec = p.records + it.buf0 + (int64_t)strip * n_ent;
-        const int* inprog = p.progress + it.prog0 + strip - 1;
-        int* outprog = p.progress + it.prog0 + strip;
-        const bool store_out = has_out && lane == 31;
-        const float Cok = (float)(1.0 / (double)k);                // Eq.1 with C = 1 (the exponents do the scaling)
 
         L ln;
         ln.init();
@@ -133,72 +128,88 @@ __global__ void __launch_bounds__(LONG_WPC * 32, LONG_MIN_CTAS) k_long_f32(DevBa
         int ex = 0;            // true value = stored value * 2^ex
         float f_in = 1.f;      // 2^(ex of the left neighbour - ex)
         int seen = 0;          // entries the producer strip is known to have published
-        float fin_m = 0.f;     // this lane's share of Eq.4 and its exponent
-        int fin_e = LONG_FLOOR;
+        sm.fin[lane] = make_float2(0.f, 0.f);
 
-        // ---- fetch.  The table blocks (32 entries = 2 KB, phmm_table.cuh) the warp is walking live in a ring of 4 blocks in
-        // shared memory, filled by cp.async one block (32 steps) ahead of lane 0: the step never waits for L2 or DRAM.
-        // Lane L's .x half is at table position run0 + s - 2L at step s; before its stream starts and after it has ended a
-        // lane reads the all-zero block instead.  Block B sits in ring slot B & 3: when lane 0 enters block B, lane 31 (62
+        // ---- fetch.  The table blocks live in the ring, filled by cp.async one block (32 steps) ahead of lane 0: the step
+        // never waits for L2 or DRAM.  Lane L's .x half is at table position run0 + v, v = s - 2L, at step s; outside
+        // [0, run_len) it reads all-zero entries.  Block B sits in ring slot B & 3: when lane 0 enters block B, lane 31 (62
         // entries behind) is in block B-2, so slot (B+1) & 3 = (B-3) & 3 is free for block B+1.
-        const uint32_t ring_s = (uint32_t)__cvta_generic_to_shared(sm.ring);
-        const uint32_t zero_s = (uint32_t)__cvta_generic_to_shared(sm_zero);
         auto fill = [&](int blk) {
-            const char* g = reinterpret_cast<const char*>(tab) + ((int64_t)blk << 11) + lane * 16;
-            const uint32_t d = ring_s + ((blk & 3) << 11) + lane * 16;
+            const char* g = tab + ((int64_t)blk << 11) + lane * 16;
+            const uint32_t d = ring_s + ((lane >> 4) << 10) + ((blk & 3) << 8) + ((lane & 15) << 4);
 #pragma unroll
-            for (int j = 0; j < 4; j++)
-                asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(d + j * 512), "l"(g + j * 512) : "memory");
+            for (int j = 0; j < 4; j++)  // chunk plane j: 512 bytes of the table block, parity halves 256 bytes each
+                asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(d + j * 2048), "l"(g + j * 512) : "memory");
             asm volatile("cp.async.commit_group;" ::: "memory");
         };
         auto fill_wait = [&]() {
             asm volatile("cp.async.wait_group 0;" ::: "memory");
             __syncwarp();
         };
-        uint32_t e_even = zero_s;  // shared-memory address of chunk 0 of the even entry
         auto load_entry = [&](RawEntry& re, uint32_t e) {
             asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(re.a.x), "=f"(re.a.y), "=f"(re.a.z), "=f"(re.a.w) : "r"(e));
-            asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4+512];" : "=f"(re.b.x), "=f"(re.b.y), "=f"(re.b.z), "=f"(re.b.w) : "r"(e));
-            asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4+1024];" : "=f"(re.c.x), "=f"(re.c.y), "=f"(re.c.z), "=f"(re.c.w) : "r"(e));
-            asm volatile("ld.shared.b32 %0, [%1+1536];" : "=r"(re.w) : "r"(e));
+            asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4+2048];" : "=f"(re.b.x), "=f"(re.b.y), "=f"(re.b.z), "=f"(re.b.w) : "r"(e));
+            asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4+4096];" : "=f"(re.c.x), "=f"(re.c.y), "=f"(re.c.z), "=f"(re.c.w) : "r"(e));
+            asm volatile("ld.shared.b32 %0, [%1+6144];" : "=r"(re.w) : "r"(e));
         };
-        auto fetch_even = [&](RawEntry& re, int s) {  // the entry of (even) step s
-            const int v = s - 2 * lane;
-            const int pos = run0 + v;
-            e_even = (unsigned)v < (unsigned)run_len ? ring_s + (((pos >> 5) & 3) << 11) + (((pos >> 1) & 15) << 4) : zero_s;
+        int v = -2 * lane;                                          // stream index of the next even entry to fetch
+        uint32_t off = (uint32_t)(((run0 >> 1) - lane) & 63) << 4;  // its offset in the ring's 1 KB window
+        uint32_t e_even = zero_s;
+        auto fetch_even = [&](RawEntry& re) {
+            e_even = (unsigned)v < (unsigned)run_len ? ring_s + off : zero_s;
+            v += 2;
+            off = (off + 16) & 1023;
             load_entry(re, e_even);
         };
-        auto fetch_odd = [&](RawEntry& re) { load_entry(re, e_even + 256); };  // (runs have even lengths: same block, same range)
+        auto fetch_odd = [&](RawEntry& re) { load_entry(re, e_even + 1024); };  // (runs have even lengths: same range)
         fill(run0 >> 5);
         fill((run0 >> 5) + 1);
         fill_wait();
 
-        // ---- an event: new exponents for all lanes, the next 16 boundary records for lane 0
-        auto event = [&](int s) {
-            // what lane 31 has stored so far becomes visible to the next strip (release: MEMBAR + strong store)
-            if (store_out && s > 63 && (s & (p.publish - 1)) == 0) st_release_gpu(outprog, min(s - 63, n_ent));
+        // ---- an event (every 16 steps): flush what lane 31 handed out, new exponents for all lanes, the next 16 boundary
+        //      records for lane 0.  `last`: behind the loop, only the flush.
+        auto event = [&](int s, bool last) {
+            // 0. records of the steps s-16 .. s-1 (entries s-79 .. s-64), at the exponent lane 31 had during those steps
+            if (has_out) {  // (warp-uniform)
+                const int exo = __shfl_sync(PHMM_FULL, ex, 31);
+                __syncwarp();
+                const int eo = s - 79 + lane;
+                if (lane < LONG_EVERY && (unsigned)eo < (unsigned)n_ent) {
+                    const float2 o = sm.rout[lane];
+                    st_strong_f4(p.records + it.buf0 + (int64_t)strip * n_ent + eo, make_float4(o.x, o.y, __int_as_float(exo), 0.f));
+                }
+                __syncwarp();
+                if (lane == 0 && !last && s > 63 && (s & (p.publish - 1)) == 0)
+                    st_release_gpu(p.progress + it.prog0 + strip, min(s - 63, n_ent));  // release: MEMBAR + strong store
+            }
+            if (last) return;
+            // 1. the boundary records lane 0 consumes in the steps s .. s+15 (their loads fly while the maximum is taken)
             float4 rec = make_float4(0.f, 0.f, 0.f, 0.f);
-            int bmax = LONG_FLOOR;
-            if (has_in && s < n_ent) {  // (warp-uniform)
+            const bool in_now = has_in && s < n_ent;  // (warp-uniform)
+            if (in_now) {
                 const int need = min(s + LONG_EVERY, n_ent);
                 if (need > seen) {  // (the producer is usually far ahead: one look every few hundred steps)
-                    int v = ld_relaxed_gpu(inprog);
-                    while (v < need) { __nanosleep(100); v = ld_relaxed_gpu(inprog); }
-                    seen = v;
+                    const int* inprog = p.progress + it.prog0 + strip - 1;
+                    int q = ld_relaxed_gpu(inprog);
+                    while (q < need) { __nanosleep(100); q = ld_relaxed_gpu(inprog); }
+                    seen = q;
                 }
-                if (lane < LONG_EVERY && s + lane < n_ent) rec = ld_strong_f4(inrec + s + lane);
+                if (lane < LONG_EVERY && s + lane < n_ent) rec = ld_strong_f4(p.records + it.buf0 + (int64_t)(strip - 1) * n_ent + s + lane);
+            }
+            // 2. own proposal (none for a lane that holds nothing)
+            float m = fmax3(ln.outS.x, ln.outS.y, fmaxf(ln.outT.x, ln.outT.y));
+#pragma unroll
+            for (int x = 0; x < NV; x++) m = fmax3(m, fmaxf(ln.Tt[x].x, ln.Tt[x].y), fmaxf(ln.J[x].x, ln.J[x].y));
+            int c = m > 0.f ? ex + Fx<float>::ilogb(m) - LONG_TGT : LONG_FLOOR;
+            int bmax = LONG_FLOOR;
+            if (in_now) {
                 const float mi = fmaxf(rec.x, rec.y);
                 bmax = mi > 0.f ? __float_as_int(rec.z) + Fx<float>::ilogb(mi) : LONG_FLOOR;
 #pragma unroll
                 for (int o = 8; o > 0; o >>= 1) bmax = max(bmax, __shfl_xor_sync(PHMM_FULL, bmax, o));
                 bmax = __shfl_sync(PHMM_FULL, bmax, 0);
             }
-            // 1. own proposal (none for a lane that holds nothing)
-            float m = fmax3(ln.outS.x, ln.outS.y, fmaxf(ln.outT.x, ln.outT.y));
-#pragma unroll
-            for (int x = 0; x < NV; x++) m = fmax3(m, fmaxf(ln.Tt[x].x, ln.Tt[x].y), fmaxf(ln.J[x].x, ln.J[x].y));
-            int c = m > 0.f ? ex + Fx<float>::ilogb(m) - LONG_TGT : LONG_FLOOR;
-            // 2. ex'_L = max(c_L, max over m < L of c_m - KTOT), the boundary records counting as a lane to the left of lane
+            // 3. ex'_L = max(c_L, max over m < L of c_m - KTOT), the boundary records counting as a lane to the left of lane
             //    0: nothing that can reach lane L (values only move right and down, and only shrink in true magnitude) is
             //    stored above 2^(TGT+KTOT) there -- whatever the hop count
             const int bsrc = bmax > LONG_FLOOR ? bmax - LONG_TGT : LONG_FLOOR;
@@ -212,38 +223,40 @@ __global__ void __launch_bounds__(LONG_WPC * 32, LONG_MIN_CTAS) k_long_f32(DevBa
             if (lane == 0) pm = bsrc;
             if (pm > LONG_FLOOR) c = max(c, pm - LONG_KTOT);
             const int exn = c < LONG_FLOOR / 2 ? ex : c;  // nothing held, nothing to the left: keep the exponent
-            // 3. rescale the state: d <= TGT - ilogb(m) <= 127 when something is held, any d when nothing is
-            const int d = m > 0.f ? ex - exn : 0;
-            const int ex_new = exn;
-            const float f = pow2f(d);  // 0 for d < -126: everything held is negligible against what is about to arrive
+            // 4. rescale the state: d <= TGT - ilogb(m) <= 127 when something is held, any d when nothing is
+            const float f = pow2f(m > 0.f ? ex - exn : 0);  // 0 for d < -126: what is held is negligible against what arrives
             const float2 F = make_float2(f, f);
 #pragma unroll
             for (int x = 0; x < NV; x++) { ln.Tt[x] = __fmul2_rn(ln.Tt[x], F); ln.J[x] = __fmul2_rn(ln.J[x], F); }
             ln.outS = __fmul2_rn(ln.outS, F);
             ln.outT = __fmul2_rn(ln.outT, F);
-            ex = ex_new;
-#ifdef LONG_DEBUG
-            if (pair == 0 && s / 16 < 60) {
-                float* q = g_dbg + ((strip * 60 + s / 16) * 32 + lane) * 4;
-                q[0] = m; q[1] = (float)ex; q[2] = f; q[3] = (float)c;
-            }
-#endif
+            ex = exn;
             const int exl = __shfl_up_sync(PHMM_FULL, ex, 1);
             f_in = pow2f(exl - ex);  // (exl - ex <= KTOT by construction; lane 0 does not use it)
-            // 4. lane 0's next 16 boundary values at its new exponent
-            if (has_in) {
+            // 5. lane 0's next 16 boundary values at its new exponent; in the first strip: Eq.1 (reading G1), the run-in
+            //    entry injects s = C/k = 1/k and T = g_1 C/k at exponent 0, every other entry nothing
+            {
                 const int ex0 = __shfl_sync(PHMM_FULL, ex, 0);
-                __syncwarp();
                 if (lane < LONG_EVERY) {
-                    const int dd = __float_as_int(rec.z) - ex0;
-                    sm.rin[lane] = make_float2(scale2(rec.x, dd), scale2(rec.y, dd));
+                    float2 o = make_float2(0.f, 0.f);
+                    if (has_in) {
+                        const int dd = __float_as_int(rec.z) - ex0;
+                        o = make_float2(scale2(rec.x, dd), scale2(rec.y, dd));
+                    } else if (s == 0 && lane == 0) {
+                        const float Cok = __frcp_rn((float)k);  // (k < 2^24: the correctly rounded 1/k)
+                        float g1;  // C of the run-in entry = g_1: chunk plane 1, first float of the entry at run0
+                        asm volatile("ld.shared.f32 %0, [%1+2048];" : "=f"(g1) : "r"(ring_s + ((uint32_t)((run0 >> 1) & 63) << 4)));
+                        o = make_float2(Cok, g1 * Cok);
+                    }
+                    sm.rin[lane] = o;
                 }
                 __syncwarp();
             }
         };
 
         const uint32_t sum_y = META_SUM << 16;
-        auto one_step = [&](const RawEntry& re, int s) {
+        const bool lane0 = lane == 0, lane31 = lane == 31;
+        auto one_step = [&](const RawEntry& re, uint32_t slot) {  // slot: shared-memory address of rin[step & 15]
             Entry2<float> E;
             E.gam = make_float2(re.a.x, re.a.y); E.A = make_float2(re.a.z, re.a.w);
             E.C = make_float2(re.b.x, re.b.y); E.G = make_float2(re.b.z, re.b.w);
@@ -251,50 +264,51 @@ __global__ void __launch_bounds__(LONG_WPC * 32, LONG_MIN_CTAS) k_long_f32(DevBa
             E.metaX = re.w & 0xffu; E.metaY = (re.w >> 16) & 0xffu;
             E.r2 = re.w & 0xff00ff00u;
             const float prevT = ln.outT.y;
+            float2 bin;
+            asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(bin.x), "=f"(bin.y) : "r"(slot));
             float inS = __shfl_up_sync(PHMM_FULL, ln.outS.y, 1) * f_in;
             float inT = __shfl_up_sync(PHMM_FULL, prevT, 1) * f_in;
-            if (lane == 0) {
-                if (has_in) {
-                    const float2 v = sm.rin[s & (LONG_EVERY - 1)];
-                    inS = v.x; inT = v.y;
-                } else {  // column-0 boundary, Eq.1 (reading G1): only the run-in entry injects, at exponent 0
-                    inS = (E.metaX & META_FIRST) ? Cok : 0.f;
-                    inT = E.C.x * inS;
-                }
-            }
+            inS = lane0 ? bin.x : inS;
+            inT = lane0 ? bin.y : inT;
             if (E.metaX & META_SUM) inS = 0.f;  // Eq.4: every lane sums its own columns only
             ln.step(E, inS, inT);
             if (re.w & sum_y) {  // this lane's .y half has just finished the sum entry: its share of Eq.4
+                // M+I of column j reaches the sum through the T of column j+1; a strip whose last real column is the last
+                // column of its lane has that one in what the lane handed out one step ago (unless the next strip counts it)
+                const int k_loc = min(k - strip * STRIP, STRIP), out_lane = (k_loc - 1) / N2;
                 if (lane <= out_lane) {
-                    // M+I of column j reaches the sum through the T of column j+1; a strip whose last real column is the last
-                    // column of its lane has that one in what the lane handed out one step ago
-                    const bool full = !has_out && lane == out_lane && (k_loc % N2) == 0;  // (else the next strip counts it)
-                    fin_m = full ? ln.outS.y + prevT : ln.outS.y;
-                    fin_e = ex;
+                    const bool full = !has_out && lane == out_lane && (k_loc % N2) == 0;
+                    sm.fin[lane] = make_float2(full ? ln.outS.y + prevT : ln.outS.y, __int_as_float(ex));
                 }
             }
-            // ---- right boundary: lane 31's .y half has just finished entry s - 63
-            // (published at the next event, or with the Eq.4 total behind the loop)
-            if (store_out && (unsigned)(s - 63) < (unsigned)n_ent)
-                st_strong_f4(outrec + (s - 63), make_float4(ln.outS.y, ln.outT.y, __int_as_float(ex), 0.f));
+            if (lane31) {  // right boundary of the strip: staged, flushed to the records at the next event
+                asm volatile("st.shared.f32 [%0+128], %1;" ::"r"(slot), "f"(ln.outS.y) : "memory");
+                asm volatile("st.shared.f32 [%0+132], %1;" ::"r"(slot), "f"(ln.outT.y) : "memory");
+            }
         };
 
         RawEntry eA, eB;
-        fetch_even(eA, 0);
-        const int steps = run_len + 64;  // even; lane 31's .y half finishes entry run_len - 1 >= n_ent - 1 at step run_len + 62
+        fetch_even(eA);
+        // lane 31's .y half finishes entry run_len - 1 >= n_ent - 1 at step run_len + 62; a multiple of 16 steps
+        const int steps = (run_len + 64 + 15) & ~15;
         for (int s = 0; s < steps; s += 2) {
-            if ((s & (LONG_EVERY - 1)) == 0) event(s);
+            if ((s & (LONG_EVERY - 1)) == 0) event(s, false);
             if (((run0 + s + 2) & 31) == 0) {  // lane 0's next fetch enters a new block (now complete): the one after it starts its way in
                 fill_wait();
                 fill(((run0 + s + 2) >> 5) + 1);
             }
+            const uint32_t slot = rin_s + ((s & (LONG_EVERY - 2)) << 3);
             fetch_odd(eB);
-            one_step(eA, s);
-            fetch_even(eA, s + 2);
-            one_step(eB, s + 1);
+            one_step(eA, slot);
+            fetch_even(eA);
+            one_step(eB, slot + 8);
         }
+        event(steps, true);
 
         // ---- Eq.4: combine the lanes' shares, then the strips' (each strip waits for the total of the strips to its left)
+        const float2 fin = sm.fin[lane];
+        const float fin_m = fin.x;
+        const int fin_e = __float_as_int(fin.y);
         int em = fin_m > 0.f ? fin_e + Fx<float>::ilogb(fin_m) : LONG_FLOOR;  // exponent of the largest share
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) em = max(em, __shfl_xor_sync(PHMM_FULL, em, o));
@@ -302,12 +316,13 @@ __global__ void __launch_bounds__(LONG_WPC * 32, LONG_MIN_CTAS) k_long_f32(DevBa
         double tot = fin_m > 0.f ? ldexp((double)fin_m, max(fin_e - em, -1000)) : (fin_m == 0.f ? 0.0 : (double)fin_m);
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) tot += __shfl_xor_sync(PHMM_FULL, tot, o);
-        if (lane == 31) {  // (the lane that published the records, so the progress counter has one writer)
+        if (lane == 0) {  // (the lane that publishes the progress counter)
             double acc = tot;
             int acc_e = em;
             if (has_in) {  // total of the strips to the left: (double mantissa, exponent), published behind the last record
-                int v = seen;
-                while (v < n_ent + 1) { v = ld_relaxed_gpu(inprog); if (v < n_ent + 1) __nanosleep(100); }
+                const int* inprog = p.progress + it.prog0 + strip - 1;
+                int q = seen;
+                while (q < n_ent + 1) { q = ld_relaxed_gpu(inprog); if (q < n_ent + 1) __nanosleep(100); }
                 const float4 t = ld_strong_f4(p.totals + it.prog0 + strip - 1);
                 const double lm = __hiloint2double(__float_as_int(t.y), __float_as_int(t.x));
                 const int le = __float_as_int(t.z);
@@ -321,18 +336,13 @@ __global__ void __launch_bounds__(LONG_WPC * 32, LONG_MIN_CTAS) k_long_f32(DevBa
             if (has_out) {
                 st_strong_f4(p.totals + it.prog0 + strip,
                              make_float4(__int_as_float(__double2loint(acc)), __int_as_float(__double2hiint(acc)), __int_as_float(acc_e), 0.f));
-                st_release_gpu(outprog, n_ent + 1);
+                st_release_gpu(p.progress + it.prog0 + strip, n_ent + 1);
             } else if (acc > 0.0 && acc < 1e300) {  // (finite and positive; acc is a sum of normal floats)
                 p.out[pair] = log10(acc) + (double)acc_e * LOG10_2;
                 if (p.flags) p.flags[pair] = p.flag_bits;
             } else {  // overflow or a vanished sum: the fp64 chain kernel recomputes the pair
-#ifdef LONG_DEBUG
-                p.out[pair] = acc != acc ? -1e9 : (acc >= 1e300 ? -2e9 : (acc == 0.0 ? -3e9 : -4e9));
-                if (p.flags) p.flags[pair] = 64;
-#else
                 const int idx = atomicAdd(p.fallback_count, 1);
                 p.fallback_list[idx] = pair;
-#endif
             }
         }
         __syncwarp();
