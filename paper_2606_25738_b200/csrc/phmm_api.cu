@@ -182,10 +182,10 @@ extern "C" int phmm_get_stats(phmm_ctx* ctx, phmm_stats* out) {
     if (!ctx->stats_final && ctx->d_counters.p && ctx->stats.n_pairs > 0) {  // rescue count lives on the device until the caller has synchronised
         int n = 0;
         DeviceGuard guard(ctx->device);
-        int rq[48];
+        int rq[16];
         if (cudaMemcpy(&n, ctx->d_counters.p, sizeof(int), cudaMemcpyDeviceToHost) == cudaSuccess && ctx->d_rq.p &&
-            cudaMemcpy(rq, ctx->d_rq.p, sizeof(rq), cudaMemcpyDeviceToHost) == cudaSuccess && ctx->stats.n_short_warps > 0)
-            ctx->stats.n_rescued = (int64_t)n + rq[34] - rq[40];  // chain-kernel queue + sub-warp queue - passed on from one to the other
+            cudaMemcpy(rq, (int*)ctx->d_rq.p + RESCUE_NB, sizeof(rq), cudaMemcpyDeviceToHost) == cudaSuccess && ctx->stats.n_short_warps > 0)
+            ctx->stats.n_rescued = (int64_t)n + rq[RQ_NQUEUE - RESCUE_NB] - rq[RQ_FALLBACK - RESCUE_NB];  // chain-kernel queue + sub-warp queue - passed on from one to the other
     }
     if (ctx->opt.profile_events) {
         double* dst[4] = {&ctx->stats.ms_table, &ctx->stats.ms_short, &ctx->stats.ms_rescue, &ctx->stats.ms_long};
@@ -395,11 +395,11 @@ extern "C" int phmm_forward_batch(phmm_ctx* ctx, const phmm_batch* b, int precis
     // rescue list (fp32 mode: filled by the short kernel) / sequential list (fp64 mode: all non-long pairs)
     CK(ctx->d_rescue.need((size_t)np * 4 + 4));
     RC(sg.upload(ctx->d_rescue, seq_pairs.data(), n_seq * 4));
-    CK(ctx->d_rq.need(48 * 4));
-    CK(ctx->d_rq_plan.need(68 * 4));
+    CK(ctx->d_rq.need(RQ_INTS * 4));
+    CK(ctx->d_rq_plan.need(RESCUE_PLAN_INTS * 4));
     CK(ctx->d_rq_queue.need((size_t)np * 16 + 16));
     CK(ctx->d_rq_sorted.need((size_t)np * 4 + 4));
-    CK(cudaMemsetAsync(ctx->d_rq.p, 0, 48 * 4, st));
+    CK(cudaMemsetAsync(ctx->d_rq.p, 0, RQ_INTS * 4, st));
     ps.used = true;
     struct FreeMark {  // whatever path leaves the call: the set is free once everything enqueued so far on st has run
         cudaEvent_t ev, ev_last; cudaStream_t st;
@@ -443,7 +443,7 @@ extern "C" int phmm_forward_batch(phmm_ctx* ctx, const phmm_batch* b, int precis
         sl.rescue_thr = (float)ldexp(1.0, ctx->opt.rescue_log2_threshold);
         sl.rescue.queue = (int4*)ctx->d_rq_queue.p;
         sl.rescue.cnt = (int*)ctx->d_rq.p;
-        sl.rescue.n_queue = (int*)ctx->d_rq.p + 34;
+        sl.pair_read = (const int*)ps.d_pair_read.p;
         sl.rescue_count = counters + 0;
         sl.rescue_list = (int*)ctx->d_rescue.p;
         PROF(1, 0);
@@ -513,7 +513,7 @@ extern "C" int phmm_forward_batch(phmm_ctx* ctx, const phmm_batch* b, int precis
         memset(&rl, 0, sizeof(rl));
         rl.queue.queue = (int4*)ctx->d_rq_queue.p;
         rl.queue.cnt = (int*)ctx->d_rq.p;
-        rl.queue.n_queue = (int*)ctx->d_rq.p + 34;
+        rl.table = fp64 ? nullptr : (const float*)ctx->d_table.p;
         rl.max_queue = (int)(fp64 ? (int64_t)sub_pairs.size() : ctx->stats.n_short_pairs);
         rl.enqueue_pairs = fp64 ? (const int*)ps.d_rq_enq.p : nullptr;
         rl.n_enqueue = fp64 ? (int)sub_pairs.size() : 0;

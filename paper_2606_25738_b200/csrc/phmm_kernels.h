@@ -43,18 +43,23 @@ constexpr int RESCUE_MAX_L = 4096;              // = the short class.  Unrescale
                                                 // thousands of related ones; a result below 1e-290 is passed on to the rescaled chain kernel,
                                                 // and above it the flushed cells weigh < 2^-36 of the sum
 
+// Device-side binning of the pairs to recompute: bucket = (lane-group size g = ceil(k / RESCUE_NV), read-length class l >> 3),
+// g-major, so that the pairs sharing a warp (same g) also have similar lengths and finish together.
+constexpr int RESCUE_LCLS = RESCUE_MAX_L / 8 + 1;   // read-length classes
+constexpr int RESCUE_NB = 33 * RESCUE_LCLS;         // buckets
+enum { RQ_TICKET = RESCUE_NB, RQ_NQUEUE = RESCUE_NB + 1, RQ_FALLBACK = RESCUE_NB + 2, RQ_INTS = RESCUE_NB + 16 };
 struct RescueQueue {
-    int4* queue;      // (pair, lane-group size g, ticket within bucket g, -)
-    int* n_queue;     // items in queue
-    int* cnt;         // 48 ints, zeroed per call: [0..32] items per bucket g, [33] warp ticket of k_rescue_f64, [34] = *n_queue,
-                      // [40] pairs passed on to the chain kernel
+    int4* queue;      // (pair, bucket, ticket within the bucket, -)
+    int* cnt;         // RQ_INTS ints, zeroed per call: [0..RESCUE_NB) items per bucket, [RQ_TICKET] warp ticket of the kernel,
+                      // [RQ_NQUEUE] items in queue, [RQ_FALLBACK] pairs passed on to the chain kernel
 };
 #ifdef __CUDACC__
-__device__ __forceinline__ void rescue_push(const RescueQueue& rq, int pair, int k) {
+__device__ __forceinline__ void rescue_push(const RescueQueue& rq, int pair, int k, int l) {
     const int g = (k + RESCUE_NV - 1) / RESCUE_NV;
-    const int n = atomicAdd(rq.cnt + g, 1);
-    const int i = atomicAdd(rq.n_queue, 1);
-    rq.queue[i] = make_int4(pair, g, n, 0);
+    const int bk = g * RESCUE_LCLS + (l >> 3);
+    const int n = atomicAdd(rq.cnt + bk, 1);
+    const int i = atomicAdd(rq.cnt + RQ_NQUEUE, 1);
+    rq.queue[i] = make_int4(pair, bk, n, 0);
 }
 #endif
 
@@ -74,6 +79,7 @@ struct ShortLaunch {
     uint8_t* flags;
     float rescue_thr;          // scaled sums below this (or non-finite) are queued for fp64
     RescueQueue rescue;        // underflowed pairs with k <= RESCUE_MAX_K and l <= RESCUE_MAX_L: sub-warp fp64 kernel
+    const int* pair_read;      // device copy of the caller's pair list (the queue is binned by read length)
     int* rescue_count;         // the others: device counter and
     int* rescue_list;          // caller pair indices for the rescaled chain kernel
 };
@@ -125,13 +131,17 @@ cudaError_t launch_long_f32(const DevBatch& b, const LongLaunch& p, int grid_cta
 int long_ctas_per_sm();
 int long_warps_per_cta();
 
+constexpr int RESCUE_PLAN_INTS = 68 + RESCUE_NB;  // [0..33] first warp of bucket g, [34..67] first list slot of bucket g, [68..) first slot of each (g, length class) bucket
 struct RescueLaunch {
     RescueQueue queue;
     int max_queue;             // upper bound of the queue length (grid of the scatter kernel)
     const int* enqueue_pairs;  // PHMM_FP64 mode: device list of pairs to queue first (else nullptr)
     int n_enqueue;
-    int* plan;                 // 68 ints of scratch
+    int* plan;                 // RESCUE_PLAN_INTS ints of scratch
     int* sorted;               // max_queue ints of scratch
+    const float* table;        // fp32 mode: the row-constant table of the short path (the recomputation runs in double on
+                               // the fp32-rounded constants: it needs the range, not the precision); nullptr: constants are
+                               // formed in double from the quality bytes (PHMM_FP64)
     const int* pair_read;
     const int* pair_hap;
     const double* lut;

@@ -198,7 +198,8 @@ __global__ void __launch_bounds__(SHORT_WARPS_PER_CTA * 32, SHORT_MIN_CTAS) k_sh
                 p.out[pair] = log10((double)sg) - 120.0 * LOG10_2;
                 if (p.flags) p.flags[pair] = 0;
             } else if (m_k <= RESCUE_MAX_K) {  // (every short-class read has l <= RESCUE_MAX_L)
-                rescue_push(p.rescue, pair, m_k);  // a10: unrescaled fp64 sub-warp kernel
+                const int rr = p.pair_read[pair];
+                rescue_push(p.rescue, pair, m_k, (int)(b.read_off[rr + 1] - b.read_off[rr]));  // a10: unrescaled fp64 sub-warp kernel
             } else {
                 const int idx = atomicAdd(p.rescue_count, 1);  // rescaled fp64 chain kernel
                 p.rescue_list[idx] = pair;
