@@ -300,6 +300,12 @@ __global__ void __launch_bounds__(RESCUE_WARPS * 32, RESCUE_MIN_CTAS) k_rescue_f
         fetch(cur, -lg);
         for (int s = 0; s < steps; s++) {
             fetch(nxt, s + 1 - lg);
+            if (lg == 0 && active) {  // the group's leading lane asks L2 for the entry 24 steps ahead (4 chunk planes)
+                const int pos = run0 + s + 24;
+                const float* q = table + 4 * ((((int64_t)(pos >> 5)) << 7) + (int64_t)((pos & 1) * 16 + ((pos >> 1) & 15)));
+#pragma unroll
+                for (int c = 0; c < 4; c++) asm volatile("prefetch.global.L2 [%0];" ::"l"(q + 128 * c));
+            }
             const double gam = (double)cur.gam, A = (double)cur.A, C = (double)cur.C, G = (double)cur.G;
             const double pm = (double)cur.pm, px = (double)cur.px;
             const uint32_t meta = cur.w & 0xffu;
