@@ -64,30 +64,37 @@ struct phmm_ctx {
     phmm_options opt;
     phmm_stats stats;
     int last_cuda = 0;
-    // The read-only plan arrays of a call live in one of two sets, uploaded on a copy stream of the context: the
-    // uploads of call s+1 overlap the kernels of call s.  A set (and its pinned staging buffer) is reused once the
-    // call that used it two calls ago has completed (ev_free, recorded on the caller's stream at the end of a call).
-    struct PlanSet {
-        DevBuf d_read_off, d_hap_off, d_pair_read, d_pair_hap, d_tasks, d_warp_first, d_srt_ent, d_srt_out, d_items, d_rq_enq;
+    // Read-only arrays live in double-buffered sets, uploaded on a copy stream of the context so that the uploads of the
+    // next call / slice overlap the kernels of the current one.  A set (and its pinned staging buffer) is reused once the
+    // work that used it two calls / slices ago has completed (ev_free, recorded on the caller's stream).
+    struct CallSet {  // per call: the batch's offset arrays and pair list
+        DevBuf d_read_off, d_hap_off, d_pair_read, d_pair_hap;
+        PinBuf h_stage;
+        cudaEvent_t ev_free = nullptr, ev_up = nullptr;
+        bool used = false;
+    } cset[2];
+    struct PlanSet {  // per slice of a call: the work plan
+        DevBuf d_tasks, d_warp_first, d_srt_ent, d_srt_out, d_items, d_rq_enq, d_seq;
         PinBuf h_stage;
         cudaEvent_t ev_free = nullptr, ev_up = nullptr;
         bool used = false;
     } set[2];
-    int call_idx = 0;
+    int call_idx = 0, slice_idx = 0;
     cudaStream_t copy_stream = nullptr;
     cudaEvent_t ev_last = nullptr;  // end of the device work of the most recent call: the next call's stream waits for it,
                                     // because the table, the counters, the queues and the boundary buffers exist once per context
     DevBuf d_lut, d_table;
-    DevBuf d_counters, d_rescue, d_boundary, d_progress, d_scratch, d_totals;
-    DevBuf d_rq, d_rq_queue, d_rq_sorted, d_rq_plan;  // fp64 sub-warp recomputation: counters, queue, ordered queue, plan, FP64-mode input list
+    DevBuf d_counters, d_rescue, d_boundary, d_progress, d_scratch, d_totals, d_acc;
+    DevBuf d_rq, d_rq_queue, d_rq_sorted, d_rq_plan;  // fp64 sub-warp recomputation: counters, queue, ordered queue, plan
     DevBuf d_payload, d_out, d_flags;  // phmm_forward_batch_host only
-    std::vector<uint8_t> is_short;
+    std::vector<uint8_t> is_short, read_slice;
+    std::vector<int> sorted_all, sorted_split;
     ShortPlan plan;
     int chain_grid[2] = {0, 0};  // resident CTAs of the fp64 chain kernel ([1]; [0] unused)
     int long_grid = 0, rescue_grid = 0;  // resident CTAs of the fp32 long kernel / of the fp64 sub-warp kernel on this device
-    cudaEvent_t ev_prof[8] = {};   // profile_events: [2f], [2f+1] bracket family f (0 table, 1 short, 2 rescue, 3 long)
-    bool prof_used[4] = {false, false, false, false};
-    bool reuse_table = false;    // host entry, chunks after the first: the row-constant table of this payload is already on the device
+    // profile_events: per slice s and kernel family f (0 table, 1 short, 2 rescue, 3 long) the events [8s + 2f], [8s + 2f + 1]
+    std::vector<cudaEvent_t> ev_prof;
+    std::vector<uint8_t> prof_used;  // [4s + f]
     bool stats_final = false;    // host entry: n_rescued was counted from the flags, do not re-read the device counters
 };
 
@@ -129,15 +136,14 @@ extern "C" int phmm_create(phmm_ctx** out, int device, const phmm_options* opt) 
     if (opt) memcpy(&ctx->opt, opt, opt->size < sizeof(phmm_options) ? opt->size : sizeof(phmm_options));
     if (ctx->opt.rescue_log2_threshold == 0) ctx->opt.rescue_log2_threshold = -90;
     if (ctx->opt.long_min_hap_len <= 0 || ctx->opt.long_min_hap_len > SHORT_MAX_K) ctx->opt.long_min_hap_len = SHORT_MAX_K;
-    if (ctx->opt.max_table_bytes <= 0) ctx->opt.max_table_bytes = (int64_t)64 << 30;
-    if (ctx->opt.profile_events)
-        for (int i = 0; i < 8; i++)
-            if (cudaEventCreate(&ctx->ev_prof[i]) != cudaSuccess) { phmm_destroy(ctx); return PHMM_E_CUDA; }
+    if (ctx->opt.max_table_bytes <= 0) ctx->opt.max_table_bytes = (int64_t)4 << 30;
     memset(&ctx->stats, 0, sizeof(ctx->stats));
     if (cudaEventCreateWithFlags(&ctx->ev_last, cudaEventDisableTiming) != cudaSuccess) { phmm_destroy(ctx); return PHMM_E_CUDA; }
     for (int i = 0; i < 2; i++)
         if (cudaEventCreateWithFlags(&ctx->set[i].ev_free, cudaEventDisableTiming) != cudaSuccess ||
-            cudaEventCreateWithFlags(&ctx->set[i].ev_up, cudaEventDisableTiming) != cudaSuccess) { phmm_destroy(ctx); return PHMM_E_CUDA; }
+            cudaEventCreateWithFlags(&ctx->set[i].ev_up, cudaEventDisableTiming) != cudaSuccess ||
+            cudaEventCreateWithFlags(&ctx->cset[i].ev_free, cudaEventDisableTiming) != cudaSuccess ||
+            cudaEventCreateWithFlags(&ctx->cset[i].ev_up, cudaEventDisableTiming) != cudaSuccess) { phmm_destroy(ctx); return PHMM_E_CUDA; }
     if (cudaStreamCreateWithFlags(&ctx->copy_stream, cudaStreamNonBlocking) != cudaSuccess) { phmm_destroy(ctx); return PHMM_E_CUDA; }
     // 10^(-q/10) for q = 0..255, the paper's "q64" table
     double lut[256];
@@ -157,43 +163,46 @@ extern "C" int phmm_destroy(phmm_ctx* ctx) {
     if (!ctx) return PHMM_E_ARG;
     DeviceGuard guard(ctx->device);
     cudaDeviceSynchronize();
-    DevBuf* bufs[] = {&ctx->d_lut, &ctx->d_table, &ctx->d_counters, &ctx->d_rescue, &ctx->d_boundary, &ctx->d_progress, &ctx->d_scratch, &ctx->d_totals,
+    DevBuf* bufs[] = {&ctx->d_lut, &ctx->d_table, &ctx->d_counters, &ctx->d_rescue, &ctx->d_boundary, &ctx->d_progress, &ctx->d_scratch, &ctx->d_totals, &ctx->d_acc,
                       &ctx->d_payload, &ctx->d_out, &ctx->d_flags, &ctx->d_rq, &ctx->d_rq_queue, &ctx->d_rq_sorted, &ctx->d_rq_plan};
     for (DevBuf* b : bufs) b->release();
     for (int i = 0; i < 2; i++) {
         phmm_ctx::PlanSet& ps = ctx->set[i];
-        DevBuf* sb[] = {&ps.d_read_off, &ps.d_hap_off, &ps.d_pair_read, &ps.d_pair_hap, &ps.d_tasks, &ps.d_warp_first,
-                        &ps.d_srt_ent, &ps.d_srt_out, &ps.d_items, &ps.d_rq_enq};
+        DevBuf* sb[] = {&ps.d_tasks, &ps.d_warp_first, &ps.d_srt_ent, &ps.d_srt_out, &ps.d_items, &ps.d_rq_enq, &ps.d_seq};
         for (DevBuf* b : sb) b->release();
         ps.h_stage.release();
         if (ps.ev_free) cudaEventDestroy(ps.ev_free);
         if (ps.ev_up) cudaEventDestroy(ps.ev_up);
+        phmm_ctx::CallSet& cs = ctx->cset[i];
+        DevBuf* cb[] = {&cs.d_read_off, &cs.d_hap_off, &cs.d_pair_read, &cs.d_pair_hap};
+        for (DevBuf* b : cb) b->release();
+        cs.h_stage.release();
+        if (cs.ev_free) cudaEventDestroy(cs.ev_free);
+        if (cs.ev_up) cudaEventDestroy(cs.ev_up);
     }
     if (ctx->copy_stream) cudaStreamDestroy(ctx->copy_stream);
     if (ctx->ev_last) cudaEventDestroy(ctx->ev_last);
-    for (int i = 0; i < 8; i++)
-        if (ctx->ev_prof[i]) cudaEventDestroy(ctx->ev_prof[i]);
+    for (cudaEvent_t e : ctx->ev_prof)
+        if (e) cudaEventDestroy(e);
     delete ctx;
     return PHMM_OK;
 }
 
 extern "C" int phmm_get_stats(phmm_ctx* ctx, phmm_stats* out) {
     if (!ctx || !out) return PHMM_E_ARG;
-    if (!ctx->stats_final && ctx->d_counters.p && ctx->stats.n_pairs > 0) {  // rescue count lives on the device until the caller has synchronised
-        int n = 0;
+    if (!ctx->stats_final && ctx->d_acc.p && ctx->stats.n_pairs > 0) {  // the rescue count lives on the device until the caller has synchronised
         DeviceGuard guard(ctx->device);
-        int rq[16];
-        if (cudaMemcpy(&n, ctx->d_counters.p, sizeof(int), cudaMemcpyDeviceToHost) == cudaSuccess && ctx->d_rq.p &&
-            cudaMemcpy(rq, (int*)ctx->d_rq.p + RESCUE_NB, sizeof(rq), cudaMemcpyDeviceToHost) == cudaSuccess && ctx->stats.n_short_warps > 0)
-            ctx->stats.n_rescued = (int64_t)n + rq[RQ_NQUEUE - RESCUE_NB] - rq[RQ_FALLBACK - RESCUE_NB];  // chain-kernel queue + sub-warp queue - passed on from one to the other
+        long long acc[2] = {0, 0};
+        if (cudaMemcpy(acc, ctx->d_acc.p, sizeof(acc), cudaMemcpyDeviceToHost) == cudaSuccess) ctx->stats.n_rescued = (int64_t)acc[0];
     }
     if (ctx->opt.profile_events) {
         double* dst[4] = {&ctx->stats.ms_table, &ctx->stats.ms_short, &ctx->stats.ms_rescue, &ctx->stats.ms_long};
-        for (int f = 0; f < 4; f++) {
+        for (int f = 0; f < 4; f++) *dst[f] = 0.0;
+        for (size_t i = 0; i < ctx->prof_used.size(); i++) {  // summed over the slices of the call
             float ms = 0.f;
-            if (ctx->prof_used[f] && cudaEventSynchronize(ctx->ev_prof[2 * f + 1]) == cudaSuccess &&
-                cudaEventElapsedTime(&ms, ctx->ev_prof[2 * f], ctx->ev_prof[2 * f + 1]) == cudaSuccess)
-                *dst[f] = ms;
+            if (ctx->prof_used[i] && cudaEventSynchronize(ctx->ev_prof[2 * i + 1]) == cudaSuccess &&
+                cudaEventElapsedTime(&ms, ctx->ev_prof[2 * i], ctx->ev_prof[2 * i + 1]) == cudaSuccess)
+                *dst[i & 3] += ms;
         }
     }
     *out = ctx->stats;
@@ -251,36 +260,79 @@ struct Stager {  // packs several host arrays into the pinned buffer and copies 
 };
 }  // namespace
 
-#define PROF(f, second) do { if (ctx->opt.profile_events) { CK(cudaEventRecord(ctx->ev_prof[2 * (f) + (second)], st)); ctx->prof_used[f] = true; } } while (0)
+#define PROF(f, second) do { if (ctx->opt.profile_events) { CK(cudaEventRecord(ctx->ev_prof[8 * (size_t)sw.slice + 2 * (f) + (second)], st)); ctx->prof_used[4 * (size_t)sw.slice + (f)] = 1; } } while (0)
 
-extern "C" int phmm_forward_batch(phmm_ctx* ctx, const phmm_batch* b, int precision, double* d_out, uint8_t* d_flags,
-                                  void* cuda_stream) {
-    if (!ctx || !b) return PHMM_E_ARG;
-    if (precision != PHMM_FP32_RESCUE && precision != PHMM_FP64) return PHMM_E_ARG;
-    if (b->n_pairs < 0 || b->n_reads < 0 || b->n_haps < 0) return PHMM_E_ARG;
-    memset(&ctx->stats, 0, sizeof(ctx->stats));
-    ctx->stats_final = false;
-    for (int f = 0; f < 4; f++) ctx->prof_used[f] = false;
-    if (b->n_pairs == 0) return PHMM_OK;
-    if (!d_out || !b->d_read_bases || !b->d_qual_base || !b->d_qual_ins || !b->d_qual_del || !b->d_qual_gcp || !b->d_hap_bases)
-        return PHMM_E_ARG;
+namespace {
+
+__global__ void k_accumulate_rescued(long long* acc, const int* counters, const int* rq) {
+    // chain-kernel queue + sub-warp queue - what the sub-warp kernel passed on to the chain kernel
+    acc[0] += (long long)counters[0] + rq[RQ_NQUEUE] - rq[RQ_FALLBACK];
+}
+
+struct HostPayload {  // phmm_forward_batch_host: where the payload comes from (host) and goes to (device)
+    const uint8_t* src[5];
+    uint8_t* dst[5];
+};
+
+struct SliceWork {  // one slice of reads [r0, r1) of a call and the pairs that use them
+    int slice = 0, n_slices = 1;
+    int64_t r0 = 0, r1 = 0;
+    int64_t table_base = 0;     // absolute table position of the slice's zero run
+    int64_t table_entries = 0;  // entries of the slice's table (zero run and slack included)
+    const int* short_sorted = nullptr;  // haplotype-major short pairs (fp32 mode)
+    int64_t n_short = 0;
+    std::vector<int> seq_pairs, strip_pairs, sub_pairs;  // chain kernel work lists, fp64 sub-warp list (caller pair indices)
+    int64_t n_pairs = 0, lane_rows = 0;
+    int max_seq_l = 0, max_long_l = 0;  // longest read of the short class / of the long pairs
+};
+
+}  // namespace
+
+static int run_slice(phmm_ctx* ctx, const phmm_batch* b, const HostBatchView& hv, bool fp64, double* d_out, uint8_t* d_flags,
+                     cudaStream_t st, const phmm_ctx::CallSet& cs, SliceWork& sw, const HostPayload* hp);
+
+// The whole call: validation, classification, the global haplotype-major order of the short pairs, the cut into slices of
+// reads (so that the row-constant table of a slice fits the workspace budget), then slice after slice: host plan, uploads
+// and launches.  Everything is enqueued; the host work of slice s+1 runs while the GPU works on slice s.
+static int forward_impl(phmm_ctx* ctx, const phmm_batch* b, int precision, double* d_out, uint8_t* d_flags, cudaStream_t st,
+                        const HostPayload* hp, int min_slices) {
     HostBatchView hv = {b->n_reads, b->n_haps, b->n_pairs, b->h_read_off, b->h_hap_off, b->h_pair_read, b->h_pair_hap};
-    RC(validate_batch(hv));
-    DeviceGuard guard(ctx->device);
-    if (!guard.ok) return PHMM_E_CUDA;
-    cudaStream_t st = (cudaStream_t)cuda_stream;
     const auto t0 = std::chrono::steady_clock::now();
     const bool fp64 = precision == PHMM_FP64;
-    const int64_t np = b->n_pairs;
+    const int64_t np = b->n_pairs, nr = b->n_reads;
 
-    // ---- classify: short (sub-warp systolic fp32 kernel) / chain-sequential (one warp per pair) / chain-strips
-    const int strip_cols = chain_strip_cols(fp64);
+    // ---- slices of reads: equal shares of the table, each within the budget (fp64 uses no table: one slice unless asked)
+    const int64_t total_entries = table_run_start(b->h_read_off[nr], nr) - TABLE_ZERO_RUN;
+    const int64_t budget_entries = std::max<int64_t>(ctx->opt.max_table_bytes / 64 - 1024, 1 << 16);
+    int n_slices = fp64 ? 1 : (int)std::min<int64_t>(250, (total_entries + budget_entries - 1) / budget_entries);
+    n_slices = (int)std::max<int64_t>(1, std::min<int64_t>(std::max(n_slices, min_slices), nr));
+    std::vector<int64_t> bound((size_t)n_slices + 1, 0);
+    bound[(size_t)n_slices] = nr;
+    for (int s = 1; s < n_slices; s++) {  // first read whose run starts at or behind the s-th share
+        const int64_t want = TABLE_ZERO_RUN + total_entries * s / n_slices;
+        int64_t lo = bound[(size_t)s - 1], hi = nr;
+        while (lo < hi) { const int64_t mid = (lo + hi) / 2; if (table_run_start(b->h_read_off[mid], mid) < want) lo = mid + 1; else hi = mid; }
+        bound[(size_t)s] = lo;
+    }
+    if (n_slices > 1) {
+        ctx->read_slice.resize((size_t)nr);
+        for (int s = 0; s < n_slices; s++) memset(ctx->read_slice.data() + bound[(size_t)s], s, (size_t)(bound[(size_t)s + 1] - bound[(size_t)s]));
+    }
+    std::vector<SliceWork> sl((size_t)n_slices);
+    for (int s = 0; s < n_slices; s++) {
+        SliceWork& w = sl[(size_t)s];
+        w.slice = s; w.n_slices = n_slices; w.r0 = bound[(size_t)s]; w.r1 = bound[(size_t)s + 1];
+        w.table_base = table_run_start(b->h_read_off[w.r0], w.r0) - TABLE_ZERO_RUN;
+        w.table_entries = table_run_start(b->h_read_off[w.r1], w.r1) - w.table_base + 192;  // (slack: prefetches run past a run)
+        if (!fp64 && w.table_entries > INT32_MAX) return PHMM_E_TOOLONG;
+        if (!fp64 && w.table_entries * 64 > ctx->opt.max_table_bytes && n_slices >= std::min<int64_t>(250, nr)) return PHMM_E_NOMEM;
+    }
+
+    // ---- classify: short (sub-warp systolic fp32 kernel) / fp64 sub-warp / chain-sequential (one warp per pair) / strips
     if (ctx->is_short.size() != (size_t)np) ctx->is_short.resize((size_t)np);
-    std::vector<int> seq_pairs, strip_pairs, sub_pairs;  // chain kernel work lists, fp64 sub-warp list (caller pair indices)
-    int64_t cells = 0, long_cells = 0, lane_rows = 0;  // lane_rows: sum over short pairs of read rows x lanes of the group
-    int max_seq_l = 0, max_long_l = 0;  // longest read of the short class / of the long pairs
+    int64_t cells = 0, n_long = 0;
     {
-        struct Part { std::vector<int> seq, strip, sub; int64_t cells = 0, long_cells = 0, lane_rows = 0; int max_l = 0, max_l_long = 0; };
+        struct Part { std::vector<int> seq, strip, sub; int64_t cells = 0; };
         Part part[BATCHER_THREADS];
         const int long_k = ctx->opt.long_min_hap_len;
         uint8_t* is_short = ctx->is_short.data();
@@ -291,58 +343,140 @@ extern "C" int phmm_forward_batch(phmm_ctx* ctx, const phmm_batch* b, int precis
                 const int64_t l = b->h_read_off[r + 1] - b->h_read_off[r], k = b->h_hap_off[h + 1] - b->h_hap_off[h];
                 q.cells += l * k;
                 uint8_t sh = 0;
-                if (k > long_k || l > 4096) { q.strip.push_back((int)p); q.long_cells += l * k; if (l > q.max_l_long) q.max_l_long = (int)l; }
-                else {
-                    if (fp64 && k <= RESCUE_MAX_K && l <= RESCUE_MAX_L) q.sub.push_back((int)p);
-                    else if (fp64) q.seq.push_back((int)p);
-                    else { sh = 1; q.lane_rows += l * ((k + SHORT_N2 - 1) / SHORT_N2); }
-                    if (l > q.max_l) q.max_l = (int)l;
-                }
+                if (k > long_k || l > 4096) q.strip.push_back((int)p);
+                else if (fp64 && k <= RESCUE_MAX_K && l <= RESCUE_MAX_L) q.sub.push_back((int)p);
+                else if (fp64) q.seq.push_back((int)p);
+                else sh = 1;
                 is_short[p] = sh;
             }
         });
-        for (int t = 0; t < T; t++) {  // chunks are contiguous and in order: the lists stay sorted by pair index
-            seq_pairs.insert(seq_pairs.end(), part[t].seq.begin(), part[t].seq.end());
-            strip_pairs.insert(strip_pairs.end(), part[t].strip.begin(), part[t].strip.end());
-            sub_pairs.insert(sub_pairs.end(), part[t].sub.begin(), part[t].sub.end());
-            cells += part[t].cells; long_cells += part[t].long_cells; lane_rows += part[t].lane_rows;
-            if (part[t].max_l > max_seq_l) max_seq_l = part[t].max_l;
-            if (part[t].max_l_long > max_long_l) max_long_l = part[t].max_l_long;
+        // chunks are contiguous and in order: the per-slice lists stay sorted by pair index
+        auto deal = [&](const std::vector<int>& v, int which) {
+            for (int p : v) {
+                const int r = b->h_pair_read[p];
+                SliceWork& w = sl[n_slices > 1 ? ctx->read_slice[(size_t)r] : 0];
+                const int l = (int)(b->h_read_off[r + 1] - b->h_read_off[r]);
+                if (which == 0) { w.strip_pairs.push_back(p); if (l > w.max_long_l) w.max_long_l = l; }
+                else { (which == 1 ? w.sub_pairs : w.seq_pairs).push_back(p); if (l > w.max_seq_l) w.max_seq_l = l; }
+            }
+        };
+        for (int t = 0; t < T; t++) {
+            deal(part[t].strip, 0); deal(part[t].sub, 1); deal(part[t].seq, 2);
+            cells += part[t].cells; n_long += (int64_t)part[t].strip.size();
         }
     }
     ctx->stats.n_pairs = np;
     ctx->stats.cells = cells;
-    ctx->stats.n_long_pairs = (int64_t)strip_pairs.size();
-    ctx->stats.n_short_pairs = np - (int64_t)strip_pairs.size();
+    ctx->stats.n_long_pairs = n_long;
+    ctx->stats.n_short_pairs = np - n_long;
+    ctx->stats.n_slices = n_slices;
+
+    // ---- fp32: the short pairs in haplotype-major order, split (stably) by slice
+    std::vector<int64_t> short_first((size_t)n_slices + 1, 0);
+    if (!fp64) {
+        sort_pairs_by_hap(hv, ctx->is_short.data(), &ctx->sorted_all);
+        const std::vector<int>* order = &ctx->sorted_all;
+        if (n_slices > 1) {
+            split_by_slice(hv, ctx->sorted_all, ctx->read_slice.data(), n_slices, &ctx->sorted_split, &short_first);
+            order = &ctx->sorted_split;
+        } else {
+            short_first[1] = (int64_t)ctx->sorted_all.size();
+        }
+        for (int s = 0; s < n_slices; s++) {
+            SliceWork& w = sl[(size_t)s];
+            w.short_sorted = order->data() + short_first[(size_t)s];
+            w.n_short = short_first[(size_t)s + 1] - short_first[(size_t)s];
+            int64_t lane_rows = 0;
+            int mx = 0;
+            for (int64_t q = 0; q < w.n_short; q += 16) {  // (a 1-in-16 sample is enough for the task-size heuristic)
+                const int p = w.short_sorted[q];
+                const int r = b->h_pair_read[p], h = b->h_pair_hap[p];
+                const int64_t l = b->h_read_off[r + 1] - b->h_read_off[r], k = b->h_hap_off[h + 1] - b->h_hap_off[h];
+                lane_rows += 16 * l * ((k + SHORT_N2 - 1) / SHORT_N2);
+                if (l > mx) mx = (int)l;
+            }
+            w.lane_rows = lane_rows;
+            (void)mx;
+        }
+    }
+    for (int s = 0; s < n_slices; s++) {
+        SliceWork& w = sl[(size_t)s];
+        w.n_pairs = w.n_short + (int64_t)(w.strip_pairs.size() + w.sub_pairs.size() + w.seq_pairs.size());
+    }
+    ctx->stats.host_batch_ms = std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - t0).count();
+
+    // ---- per call: offsets and pair list to the device, on the copy stream (under the kernels of the previous call)
+    phmm_ctx::CallSet& cs = ctx->cset[ctx->call_idx & 1];
+    ctx->call_idx++;
+    if (cs.used) CK(cudaEventSynchronize(cs.ev_free));  // the call that used this set (two calls ago) has completed
+    CK(cs.h_stage.need(4096 + (size_t)(nr + 1) * 8 + (size_t)(b->n_haps + 1) * 8 + (size_t)np * 8));
+    {
+        Stager sg{ctx, &cs.h_stage, ctx->copy_stream};
+        RC(sg.upload(cs.d_read_off, b->h_read_off, (size_t)(nr + 1) * 8));
+        RC(sg.upload(cs.d_hap_off, b->h_hap_off, (size_t)(b->n_haps + 1) * 8));
+        RC(sg.upload(cs.d_pair_read, b->h_pair_read, (size_t)np * 4));
+        RC(sg.upload(cs.d_pair_hap, b->h_pair_hap, (size_t)np * 4));
+    }
+    CK(cudaStreamWaitEvent(st, ctx->ev_last, 0));  // calls on different streams of one context run one after the other
+    cs.used = true;
+    struct CallMark {  // whatever path leaves the call: the set is free once everything enqueued so far on st has run
+        cudaEvent_t ev, ev_last; cudaStream_t st;
+        ~CallMark() { cudaEventRecord(ev, st); cudaEventRecord(ev_last, st); }
+    } call_mark{cs.ev_free, ctx->ev_last, st};
+    CK(ctx->d_acc.need(16));
+    CK(cudaMemsetAsync(ctx->d_acc.p, 0, 16, st));
+    if (ctx->opt.profile_events) {
+        while (ctx->ev_prof.size() < 8 * (size_t)n_slices) {
+            cudaEvent_t e = nullptr;
+            CK(cudaEventCreate(&e));
+            ctx->ev_prof.push_back(e);
+        }
+        ctx->prof_used.assign(4 * (size_t)n_slices, 0);
+    }
+
+    // ---- slice after slice
+    for (int s = 0; s < n_slices; s++) {
+        if (sl[(size_t)s].n_pairs == 0) continue;
+        RC(run_slice(ctx, b, hv, fp64, d_out, d_flags, st, cs, sl[(size_t)s], hp));
+    }
+    return PHMM_OK;
+}
+
+static int run_slice(phmm_ctx* ctx, const phmm_batch* b, const HostBatchView& hv, bool fp64, double* d_out, uint8_t* d_flags,
+                     cudaStream_t st, const phmm_ctx::CallSet& cs, SliceWork& sw, const HostPayload* hp) {
+    const auto t0 = std::chrono::steady_clock::now();
+    const int64_t np_slice = sw.n_pairs;
     // task size: as large as possible (fewer run-ins, pipeline fills and host work; 8192 rows measured best on
     // configs[1]) while leaving at least ~6 warps of work per resident warp slot
     int task_rows = ctx->opt.task_rows;
     if (task_rows <= 0) {
         const int64_t slots = (int64_t)ctx->n_sm * 12;
-        task_rows = (int)std::max<int64_t>(1024, std::min<int64_t>(8192, lane_rows / 32 / (6 * slots)));
+        task_rows = (int)std::max<int64_t>(1024, std::min<int64_t>(8192, sw.lane_rows / 32 / (6 * slots)));
     }
-    if (!fp64) plan_short(hv, ctx->is_short.data(), SHORT_N2, task_rows, &ctx->plan);
-    else { ctx->plan.tasks.clear(); ctx->plan.warp_first.assign(1, 0); ctx->plan.srt_out.clear(); ctx->plan.srt_ent.clear(); ctx->plan.cells = 0; ctx->plan.padded_cells = 0; }
+    if (!fp64) plan_tasks(hv, sw.short_sorted, sw.n_short, sw.table_base, SHORT_N2, task_rows, &ctx->plan);
+    else { ctx->plan.tasks.clear(); ctx->plan.warp_first.assign(1, 0); ctx->plan.srt_out.clear(); ctx->plan.srt_ent.clear(); ctx->plan.cells = 0; ctx->plan.padded_cells = 0; ctx->plan.max_read_len = 0; }
     const ShortPlan& pl = ctx->plan;
     const int n_warps = (int)pl.warp_first.size() - 1;
-    ctx->stats.short_cells = pl.cells;
-    ctx->stats.short_padded_cells = pl.padded_cells;
-    ctx->stats.n_short_warps = n_warps;
+    const int max_seq_l = std::max(sw.max_seq_l, pl.max_read_len), max_long_l = sw.max_long_l;
+    ctx->stats.short_cells += pl.cells;
+    ctx->stats.short_padded_cells += pl.padded_cells;
+    ctx->stats.n_short_warps += n_warps;
 
     // ---- strip items of the long pairs, STRIP-major: strip s of every pair before strip s+1 of any.  A strip's
     // producer still holds an earlier ticket (forward progress), but it is far ahead or done by the time the
     // consumer starts, so consumers do not run in lock step with their producers and hardly ever poll (pair-major
     // order: 4.6 polls per step, 19 % of the stall samples; profiles/).  Boundary buffers are full-length per strip.
+    const int strip_cols = chain_strip_cols(fp64);
     std::vector<ChainItem> items;
     int64_t n_bnd_blocks = 0;
     int n_prog = 0;
     {
         struct PairStrips { int pair, ns, prog0; int64_t buf0; };
         std::vector<PairStrips> ps;
-        ps.reserve(strip_pairs.size());
+        ps.reserve(sw.strip_pairs.size());
         int max_ns = 0;
         size_t total = 0;
-        for (int p : strip_pairs) {
+        for (int p : sw.strip_pairs) {
             const int r = b->h_pair_read[p], h = b->h_pair_hap[p];
             const int64_t l = b->h_read_off[r + 1] - b->h_read_off[r], k = b->h_hap_off[h + 1] - b->h_hap_off[h];
             const int ns = (int)((k + strip_cols - 1) / strip_cols);
@@ -359,73 +493,71 @@ extern "C" int phmm_forward_batch(phmm_ctx* ctx, const phmm_batch* b, int precis
             for (const PairStrips& q : ps)
                 if (s < q.ns) items.push_back(ChainItem{q.pair, s, q.prog0, 0, q.buf0});
     }
-    const auto t1 = std::chrono::steady_clock::now();
-    ctx->stats.host_batch_ms = std::chrono::duration<double, std::milli>(t1 - t0).count();
+    ctx->stats.host_batch_ms += std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - t0).count();
 
-    // ---- uploads.  The plan arrays go to this call's plan set on the context's copy stream (overlapping the kernels
-    // of the previous call, which read the other set); the small per-call counters and lists that kernels also write
+    // ---- uploads.  The plan arrays go to this slice's plan set on the context's copy stream (overlapping the kernels
+    // of the previous slice / call, which read the other set); the small counters and lists that kernels also write
     // stay on the caller's stream.
-    phmm_ctx::PlanSet& ps = ctx->set[ctx->call_idx & 1];
-    ctx->call_idx++;
-    if (ps.used) CK(cudaEventSynchronize(ps.ev_free));  // the call that used this set (two calls ago) has completed
-    const size_t n_seq = fp64 ? seq_pairs.size() : 0;
-    size_t stage_bytes = 4096 + (size_t)(b->n_reads + 1) * 8 + (size_t)(b->n_haps + 1) * 8 + (size_t)np * 8 +
-                         pl.tasks.size() * sizeof(ShortTask) + pl.warp_first.size() * 4 + pl.srt_out.size() * 16 +
-                         items.size() * sizeof(ChainItem) + n_seq * 4 + sub_pairs.size() * 4 + 20 * 256;
+    phmm_ctx::PlanSet& ps = ctx->set[ctx->slice_idx & 1];
+    ctx->slice_idx++;
+    if (ps.used) CK(cudaEventSynchronize(ps.ev_free));  // the slice that used this set (two slices ago) has completed
+    const size_t n_seq = fp64 ? sw.seq_pairs.size() : 0;
+    size_t stage_bytes = 4096 + pl.tasks.size() * sizeof(ShortTask) + pl.warp_first.size() * 4 + pl.srt_out.size() * 16 +
+                         items.size() * sizeof(ChainItem) + n_seq * 4 + sw.sub_pairs.size() * 4 + 20 * 256;
     CK(ps.h_stage.need(stage_bytes));
     Stager sg{ctx, &ps.h_stage, ctx->copy_stream};
-    RC(sg.upload(ps.d_read_off, b->h_read_off, (size_t)(b->n_reads + 1) * 8));
-    RC(sg.upload(ps.d_hap_off, b->h_hap_off, (size_t)(b->n_haps + 1) * 8));
-    RC(sg.upload(ps.d_pair_read, b->h_pair_read, (size_t)np * 4));
-    RC(sg.upload(ps.d_pair_hap, b->h_pair_hap, (size_t)np * 4));
+    if (hp) {  // host entry: this slice's share of the read arrays (pinned or pageable host memory), ahead of its kernels
+        const int64_t o0 = b->h_read_off[sw.r0], o1 = b->h_read_off[sw.r1];
+        for (int i = 0; i < 5 && o1 > o0; i++)
+            CK(cudaMemcpyAsync(hp->dst[i] + o0, hp->src[i] + o0, (size_t)(o1 - o0), cudaMemcpyHostToDevice, ctx->copy_stream));
+    }
     RC(sg.upload(ps.d_tasks, pl.tasks.data(), pl.tasks.size() * sizeof(ShortTask)));
     RC(sg.upload(ps.d_warp_first, pl.warp_first.data(), pl.warp_first.size() * 4));
     RC(sg.upload(ps.d_srt_ent, pl.srt_ent.data(), pl.srt_ent.size() * 4));
     RC(sg.upload(ps.d_srt_out, pl.srt_out.data(), pl.srt_out.size() * 4));
     RC(sg.upload(ps.d_items, items.data(), items.size() * sizeof(ChainItem)));
-    RC(sg.upload(ps.d_rq_enq, sub_pairs.data(), sub_pairs.size() * 4));
+    RC(sg.upload(ps.d_rq_enq, sw.sub_pairs.data(), sw.sub_pairs.size() * 4));
+    RC(sg.upload(ps.d_seq, sw.seq_pairs.data(), n_seq * 4));
     CK(cudaEventRecord(ps.ev_up, ctx->copy_stream));
-    CK(cudaStreamWaitEvent(st, ps.ev_up, 0));
-    CK(cudaStreamWaitEvent(st, ctx->ev_last, 0));  // calls on different streams of one context run one after the other
+    CK(cudaStreamWaitEvent(st, ps.ev_up, 0));  // (covers the call's offset arrays and pair list too: same stream, earlier)
+    ps.used = true;
+    struct FreeMark {
+        cudaEvent_t ev; cudaStream_t st;
+        ~FreeMark() { cudaEventRecord(ev, st); }
+    } free_mark{ps.ev_free, st};
     // counters: [0] rescue count (= n_items of the rescue launch)  [1] ticket rescue  [2] n strip items  [3] ticket strips
     //           [4] n sequential fp64 items  [5] ticket sequential
     sg.st = st;  // from here on: buffers that kernels write as well, in stream order with them
     int h_counters[8] = {0, 0, (int)items.size(), 0, (int)n_seq, 0, 0, 0};
     RC(sg.upload(ctx->d_counters, h_counters, sizeof(h_counters)));
-    // rescue list (fp32 mode: filled by the short kernel) / sequential list (fp64 mode: all non-long pairs)
-    CK(ctx->d_rescue.need((size_t)np * 4 + 4));
-    RC(sg.upload(ctx->d_rescue, seq_pairs.data(), n_seq * 4));
+    // rescue list (fp32 mode: filled by the kernels) / sequential list (fp64 mode: the short-class pairs the sub-warp kernel does not take)
+    CK(ctx->d_rescue.need((size_t)np_slice * 4 + 4));
+    if (n_seq) CK(cudaMemcpyAsync(ctx->d_rescue.p, ps.d_seq.p, n_seq * 4, cudaMemcpyDeviceToDevice, st));
     CK(ctx->d_rq.need(RQ_INTS * 4));
     CK(ctx->d_rq_plan.need(RESCUE_PLAN_INTS * 4));
-    CK(ctx->d_rq_queue.need((size_t)np * 16 + 16));
-    CK(ctx->d_rq_sorted.need((size_t)np * 4 + 4));
+    CK(ctx->d_rq_queue.need((size_t)np_slice * 16 + 16));
+    CK(ctx->d_rq_sorted.need((size_t)np_slice * 4 + 4));
     CK(cudaMemsetAsync(ctx->d_rq.p, 0, RQ_INTS * 4, st));
-    ps.used = true;
-    struct FreeMark {  // whatever path leaves the call: the set is free once everything enqueued so far on st has run
-        cudaEvent_t ev, ev_last; cudaStream_t st;
-        ~FreeMark() { cudaEventRecord(ev, st); cudaEventRecord(ev_last, st); }
-    } free_mark{ps.ev_free, ctx->ev_last, st};
 
     DevBatch db;
     db.read_bases = b->d_read_bases; db.qual_base = b->d_qual_base; db.qual_ins = b->d_qual_ins;
     db.qual_del = b->d_qual_del; db.qual_gcp = b->d_qual_gcp; db.hap_bases = b->d_hap_bases;
-    db.read_off = (const int64_t*)ps.d_read_off.p; db.hap_off = (const int64_t*)ps.d_hap_off.p;
+    db.read_off = (const int64_t*)cs.d_read_off.p; db.hap_off = (const int64_t*)cs.d_hap_off.p;
     db.n_reads = b->n_reads; db.n_haps = b->n_haps;
+    db.table_base = sw.table_base;
+    const int* d_pair_read = (const int*)cs.d_pair_read.p;
+    const int* d_pair_hap = (const int*)cs.d_pair_hap.p;
     int* counters = (int*)ctx->d_counters.p;
     int launches = 0;
 
-    // ---- fp32: row-constant table of every read (short and long pairs use the same one)
+    // ---- fp32: row-constant table of the slice's reads (short and long pairs use the same one)
     const bool long32 = !fp64 && !items.empty();
     if (n_warps > 0 || long32) {
-        const int64_t n_entries = table_run_start(b->h_read_off[b->n_reads], b->n_reads) + 2;
-        if (n_entries > INT32_MAX) return PHMM_E_TOOLONG;
-        const size_t table_bytes = (size_t)(n_entries + 192) * 64;  // (slack: the long kernel prefetches up to 96 entries past a run)
-        if ((int64_t)table_bytes > ctx->opt.max_table_bytes) return PHMM_E_NOMEM;
+        const size_t table_bytes = (size_t)sw.table_entries * 64;
         CK(ctx->d_table.need(table_bytes));
-        ctx->stats.table_bytes = (int64_t)table_bytes;
+        ctx->stats.table_bytes = std::max<int64_t>(ctx->stats.table_bytes, (int64_t)table_bytes);
         PROF(0, 0);
-        if (!ctx->reuse_table)
-            CK(launch_lut_table(db, (const double*)ctx->d_lut.p, (float*)ctx->d_table.p, std::max(max_seq_l, max_long_l), st));
+        CK(launch_lut_table(db, (const double*)ctx->d_lut.p, (float*)ctx->d_table.p, sw.r0, sw.r1, std::max(max_seq_l, max_long_l), st));
         PROF(0, 1);
         launches++;
     }
@@ -443,7 +575,7 @@ extern "C" int phmm_forward_batch(phmm_ctx* ctx, const phmm_batch* b, int precis
         sl.rescue_thr = (float)ldexp(1.0, ctx->opt.rescue_log2_threshold);
         sl.rescue.queue = (int4*)ctx->d_rq_queue.p;
         sl.rescue.cnt = (int*)ctx->d_rq.p;
-        sl.pair_read = (const int*)ps.d_pair_read.p;
+        sl.pair_read = d_pair_read;
         sl.rescue_count = counters + 0;
         sl.rescue_list = (int*)ctx->d_rescue.p;
         PROF(1, 0);
@@ -468,8 +600,8 @@ extern "C" int phmm_forward_batch(phmm_ctx* ctx, const phmm_batch* b, int precis
             cl.items = (const ChainItem*)ps.d_items.p;
             cl.n_items = counters + 2;
             cl.ticket = counters + 3;
-            cl.pair_read = (const int*)ps.d_pair_read.p;
-            cl.pair_hap = (const int*)ps.d_pair_hap.p;
+            cl.pair_read = d_pair_read;
+            cl.pair_hap = d_pair_hap;
             cl.lut = (const double*)ctx->d_lut.p;
             cl.boundary = ctx->d_boundary.p;
             cl.scratch_blocks = 0;
@@ -488,8 +620,8 @@ extern "C" int phmm_forward_batch(phmm_ctx* ctx, const phmm_batch* b, int precis
             ll.items = (const ChainItem*)ps.d_items.p;
             ll.n_items = counters + 2;
             ll.ticket = counters + 3;
-            ll.pair_read = (const int*)ps.d_pair_read.p;
-            ll.pair_hap = (const int*)ps.d_pair_hap.p;
+            ll.pair_read = d_pair_read;
+            ll.pair_hap = d_pair_hap;
             ll.records = (float4*)ctx->d_boundary.p;
             ll.totals = (float4*)ctx->d_totals.p;
             ll.progress = (int*)ctx->d_progress.p;
@@ -507,20 +639,20 @@ extern "C" int phmm_forward_batch(phmm_ctx* ctx, const phmm_batch* b, int precis
         launches++;
     }
     // fp64 sub-warp kernel: fp32 mode = what the short kernel queued, fp64 mode = the short pairs it can hold
-    const bool sub = n_warps > 0 || !sub_pairs.empty();
+    const bool sub = n_warps > 0 || !sw.sub_pairs.empty();
     if (sub) {
         RescueLaunch rl;
         memset(&rl, 0, sizeof(rl));
         rl.queue.queue = (int4*)ctx->d_rq_queue.p;
         rl.queue.cnt = (int*)ctx->d_rq.p;
         rl.table = fp64 ? nullptr : (const float*)ctx->d_table.p;
-        rl.max_queue = (int)(fp64 ? (int64_t)sub_pairs.size() : ctx->stats.n_short_pairs);
+        rl.max_queue = (int)(fp64 ? (int64_t)sw.sub_pairs.size() : sw.n_short);
         rl.enqueue_pairs = fp64 ? (const int*)ps.d_rq_enq.p : nullptr;
-        rl.n_enqueue = fp64 ? (int)sub_pairs.size() : 0;
+        rl.n_enqueue = fp64 ? (int)sw.sub_pairs.size() : 0;
         rl.plan = (int*)ctx->d_rq_plan.p;
         rl.sorted = (int*)ctx->d_rq_sorted.p;
-        rl.pair_read = (const int*)ps.d_pair_read.p;
-        rl.pair_hap = (const int*)ps.d_pair_hap.p;
+        rl.pair_read = d_pair_read;
+        rl.pair_hap = d_pair_hap;
         rl.lut = (const double*)ctx->d_lut.p;
         rl.out = d_out;
         rl.flags = d_flags;
@@ -548,8 +680,8 @@ extern "C" int phmm_forward_batch(phmm_ctx* ctx, const phmm_batch* b, int precis
         cl.items = (const ChainItem*)ctx->d_rescue.p;
         cl.n_items = counters + (fp64 ? 4 : 0);
         cl.ticket = counters + (fp64 ? 5 : 1);
-        cl.pair_read = (const int*)ps.d_pair_read.p;
-        cl.pair_hap = (const int*)ps.d_pair_hap.p;
+        cl.pair_read = d_pair_read;
+        cl.pair_hap = d_pair_hap;
         cl.lut = (const double*)ctx->d_lut.p;
         cl.boundary = ctx->d_scratch.p;
         cl.scratch_blocks = blocks;
@@ -564,16 +696,41 @@ extern "C" int phmm_forward_batch(phmm_ctx* ctx, const phmm_batch* b, int precis
         PROF(2, 1);
         launches++;
     }
-    ctx->stats.n_kernel_launches = launches;
-    ctx->stats.n_slices = 1;
+    if (!fp64 && (n_warps > 0 || long32)) {  // pairs recomputed in fp64 so far (phmm_get_stats)
+        k_accumulate_rescued<<<1, 1, 0, st>>>((long long*)ctx->d_acc.p, counters, (const int*)ctx->d_rq.p);
+        CK(cudaGetLastError());
+    }
+    ctx->stats.n_kernel_launches += launches;
     return PHMM_OK;
+}
+
+extern "C" int phmm_forward_batch(phmm_ctx* ctx, const phmm_batch* b, int precision, double* d_out, uint8_t* d_flags,
+                                  void* cuda_stream) {
+    if (!ctx || !b) return PHMM_E_ARG;
+    if (precision != PHMM_FP32_RESCUE && precision != PHMM_FP64) return PHMM_E_ARG;
+    if (b->n_pairs < 0 || b->n_reads < 0 || b->n_haps < 0) return PHMM_E_ARG;
+    memset(&ctx->stats, 0, sizeof(ctx->stats));
+    ctx->stats_final = false;
+    ctx->prof_used.clear();
+    if (b->n_pairs == 0) return PHMM_OK;
+    if (!d_out || !b->d_read_bases || !b->d_qual_base || !b->d_qual_ins || !b->d_qual_del || !b->d_qual_gcp || !b->d_hap_bases)
+        return PHMM_E_ARG;
+    HostBatchView hv = {b->n_reads, b->n_haps, b->n_pairs, b->h_read_off, b->h_hap_off, b->h_pair_read, b->h_pair_hap};
+    RC(validate_batch(hv));
+    DeviceGuard guard(ctx->device);
+    if (!guard.ok) return PHMM_E_CUDA;
+    return forward_impl(ctx, b, precision, d_out, d_flags, (cudaStream_t)cuda_stream, nullptr, 1);
 }
 
 // ---------------------------------------------------------------- end-to-end entry with host buffers
 extern "C" int phmm_forward_batch_host(phmm_ctx* ctx, const phmm_batch* b, int precision, double* h_out, uint8_t* h_flags) {
     if (!ctx || !b) return PHMM_E_ARG;
+    if (precision != PHMM_FP32_RESCUE && precision != PHMM_FP64) return PHMM_E_ARG;
     if (b->n_pairs < 0 || b->n_reads < 0 || b->n_haps < 0) return PHMM_E_ARG;
-    if (b->n_pairs == 0) { memset(&ctx->stats, 0, sizeof(ctx->stats)); return PHMM_OK; }
+    memset(&ctx->stats, 0, sizeof(ctx->stats));
+    ctx->stats_final = false;
+    ctx->prof_used.clear();
+    if (b->n_pairs == 0) return PHMM_OK;
     if (!h_out || !b->h_read_off || !b->h_hap_off) return PHMM_E_ARG;
     HostBatchView hv = {b->n_reads, b->n_haps, b->n_pairs, b->h_read_off, b->h_hap_off, b->h_pair_read, b->h_pair_hap};
     RC(validate_batch(hv));
@@ -585,63 +742,36 @@ extern "C" int phmm_forward_batch_host(phmm_ctx* ctx, const phmm_batch* b, int p
     CK(ctx->d_out.need((size_t)b->n_pairs * 8));
     CK(ctx->d_flags.need((size_t)b->n_pairs));
     uint8_t* base = (uint8_t*)ctx->d_payload.p;
+    HostPayload hp;
     const uint8_t* src[5] = {b->d_read_bases, b->d_qual_base, b->d_qual_ins, b->d_qual_del, b->d_qual_gcp};
-    cudaStream_t st = nullptr;
     for (int i = 0; i < 5; i++) {
         if (!src[i]) return PHMM_E_ARG;
-        CK(cudaMemcpyAsync(base + i * Ra, src[i], R, cudaMemcpyHostToDevice, st));
+        hp.src[i] = src[i] - b->h_read_off[0];  // (indexed by absolute read offsets)
+        hp.dst[i] = base + i * Ra - b->h_read_off[0];
     }
     if (!b->d_hap_bases) return PHMM_E_ARG;
-    CK(cudaMemcpyAsync(base + 5 * Ra, b->d_hap_bases, H, cudaMemcpyHostToDevice, st));
+    cudaStream_t st = nullptr;
+    // the payload buffer may still be read by the kernels of an earlier call: the copy stream waits for them
+    CK(cudaStreamWaitEvent(ctx->copy_stream, ctx->ev_last, 0));
+    CK(cudaMemcpyAsync(base + 5 * Ra, b->d_hap_bases, H, cudaMemcpyHostToDevice, ctx->copy_stream));
     phmm_batch db = *b;
-    db.d_read_bases = base; db.d_qual_base = base + Ra; db.d_qual_ins = base + 2 * Ra; db.d_qual_del = base + 3 * Ra;
-    db.d_qual_gcp = base + 4 * Ra; db.d_hap_bases = base + 5 * Ra;
-    // The pair list is processed in chunks: phmm_forward_batch only enqueues, so the host batcher of chunk c+1 runs
-    // while the GPU works on chunk c, and each chunk's results start their way back as soon as it is done.  The
-    // row-constant table depends on the payload only and is built with the first chunk.
+    db.d_read_bases = hp.dst[0]; db.d_qual_base = hp.dst[1]; db.d_qual_ins = hp.dst[2]; db.d_qual_del = hp.dst[3];
+    db.d_qual_gcp = hp.dst[4]; db.d_hap_bases = base + 5 * Ra - b->h_hap_off[0];
+    // The reads are processed in slices (at least one per 32 MB of read payload, up to 16): the copy of slice s+1 and its
+    // host plan run while the GPU works on slice s (the "with transfers" convention).
+    const int min_slices = (int)std::max<size_t>(1, std::min<size_t>(16, 5 * R / ((size_t)32 << 20)));
     const int64_t np = b->n_pairs;
-    int n_chunks = (int)std::max<int64_t>(1, std::min<int64_t>(8, np / 400000));
-    if (n_chunks > 1) {  // only worth it if the chunks use disjoint haplotypes: a shuffled list would split every task
-        int hmin[8], hmax[8];
-        for (int c = 0; c < n_chunks; c++) {
-            const int64_t lo = np * c / n_chunks, hi = np * (c + 1) / n_chunks;
-            int mn = INT32_MAX, mx = -1;
-            for (int64_t p = lo; p < hi; p++) { const int h = b->h_pair_hap[p]; mn = std::min(mn, h); mx = std::max(mx, h); }
-            hmin[c] = mn; hmax[c] = mx;
-        }
-        for (int c = 0; c + 1 < n_chunks; c++)
-            if (hmax[c] >= hmin[c + 1]) { n_chunks = 1; break; }
-    }
-    phmm_stats sum;
-    memset(&sum, 0, sizeof(sum));
-    int rc = PHMM_OK;
-    for (int c = 0; c < n_chunks && rc == PHMM_OK; c++) {
-        const int64_t lo = np * c / n_chunks, hi = np * (c + 1) / n_chunks;
-        phmm_batch cb = db;
-        cb.n_pairs = hi - lo;
-        cb.h_pair_read = b->h_pair_read + lo;
-        cb.h_pair_hap = b->h_pair_hap + lo;
-        ctx->reuse_table = c > 0 && sum.n_short_warps > 0;
-        rc = phmm_forward_batch(ctx, &cb, precision, (double*)ctx->d_out.p + lo, (uint8_t*)ctx->d_flags.p + lo, st);
-        ctx->reuse_table = false;
-        if (rc != PHMM_OK) break;
-        const phmm_stats& t = ctx->stats;
-        sum.n_pairs += t.n_pairs; sum.cells += t.cells; sum.n_short_pairs += t.n_short_pairs; sum.n_long_pairs += t.n_long_pairs;
-        sum.short_cells += t.short_cells; sum.short_padded_cells += t.short_padded_cells; sum.n_short_warps += t.n_short_warps;
-        sum.n_kernel_launches += t.n_kernel_launches; sum.host_batch_ms += t.host_batch_ms;
-        if (t.table_bytes > sum.table_bytes) sum.table_bytes = t.table_bytes;
-        if (cudaMemcpyAsync(h_out + lo, (double*)ctx->d_out.p + lo, (size_t)(hi - lo) * 8, cudaMemcpyDeviceToHost, st) != cudaSuccess) rc = PHMM_E_CUDA;
-    }
+    int rc = forward_impl(ctx, &db, precision, (double*)ctx->d_out.p, (uint8_t*)ctx->d_flags.p, st, &hp, min_slices);
     if (rc != PHMM_OK) { cudaStreamSynchronize(st); return rc; }
     std::vector<uint8_t> tmp_flags;
     uint8_t* fl = h_flags;
     if (!fl) { tmp_flags.resize((size_t)np); fl = tmp_flags.data(); }
+    CK(cudaMemcpyAsync(h_out, ctx->d_out.p, (size_t)np * 8, cudaMemcpyDeviceToHost, st));
     CK(cudaMemcpyAsync(fl, ctx->d_flags.p, (size_t)np, cudaMemcpyDeviceToHost, st));
     CK(cudaStreamSynchronize(st));
-    sum.n_slices = n_chunks;
-    for (int64_t p = 0; p < np; p++) sum.n_rescued += fl[p] & PHMM_FLAG_RESCUED;
-    ctx->stats = sum;
+    int64_t n_resc = 0;
+    for (int64_t p = 0; p < np; p++) n_resc += fl[p] & PHMM_FLAG_RESCUED;
+    ctx->stats.n_rescued = n_resc;
     ctx->stats_final = true;
     return PHMM_OK;
 }
-

@@ -38,14 +38,10 @@ int validate_batch(const HostBatchView& b) {
     return PHMM_OK;
 }
 
-void plan_short(const HostBatchView& b, const uint8_t* is_short, int N2, int task_rows, ShortPlan* out) {
-    out->tasks.clear(); out->warp_first.clear();  // the sorted arrays keep their size: they are overwritten in full
-    out->cells = 0; out->padded_cells = 0; out->max_read_len = 0;
-    const int64_t np = b.n_pairs;
-    // ---- 1. stable counting sort of the selected pairs by haplotype (chunks of the pair list in parallel:
-    //         per-chunk histograms, then every chunk scatters into its own slice of each haplotype's run)
-    const int64_t nh = b.n_haps;
-    std::vector<int> cnt((size_t)nh + 1, 0);
+// Stable counting sort of the selected pairs by haplotype (chunks of the pair list in parallel: per-chunk histograms,
+// then every chunk scatters into its own slice of each haplotype's run).  sorted: caller pair indices, haplotype-major.
+void sort_pairs_by_hap(const HostBatchView& b, const uint8_t* is_short, std::vector<int>* sorted) {
+    const int64_t np = b.n_pairs, nh = b.n_haps;
     std::vector<std::vector<int>> hist(BATCHER_THREADS);
     const int T = parallel_chunks(np, 1 << 17, [&](int t, int64_t lo, int64_t hi) {
         std::vector<int>& hs = hist[t];
@@ -54,44 +50,88 @@ void plan_short(const HostBatchView& b, const uint8_t* is_short, int N2, int tas
             if (is_short[p]) hs[b.pair_hap[p]]++;
     });
     int64_t n_sel = 0;
-    for (int64_t h = 0; h < nh; h++) {  // cnt[h] = start of haplotype h's run; hist[t][h] = start of chunk t's slice of it
-        cnt[h] = (int)n_sel;
+    for (int64_t h = 0; h < nh; h++)  // hist[t][h] = start of chunk t's slice of haplotype h's run
         for (int t = 0; t < T; t++) { const int c = hist[t][h]; hist[t][h] = (int)n_sel; n_sel += c; }
+    if (sorted->size() != (size_t)n_sel) sorted->resize((size_t)n_sel);  // steady state: same size as the last call
+    if (n_sel == 0) return;
+    int* out = sorted->data();
+    parallel_chunks(np, 1 << 17, [&](int t, int64_t lo, int64_t hi) {
+        std::vector<int>& pos = hist[t];
+        for (int64_t p = lo; p < hi; p++)
+            if (is_short[p]) out[pos[b.pair_hap[p]]++] = (int)p;
+    });
+}
+
+// Stable split of a haplotype-major pair list into slices of reads: slice_first[s] = first position of slice s in `out`.
+void split_by_slice(const HostBatchView& b, const std::vector<int>& sorted, const uint8_t* read_slice, int n_slices,
+                    std::vector<int>* out, std::vector<int64_t>* slice_first) {
+    const int64_t n = (int64_t)sorted.size();
+    out->resize((size_t)n);
+    slice_first->assign((size_t)n_slices + 1, 0);
+    std::vector<int64_t> hist((size_t)BATCHER_THREADS * (size_t)n_slices, 0);
+    const int T = parallel_chunks(n, 1 << 17, [&](int t, int64_t lo, int64_t hi) {
+        int64_t* hs = hist.data() + (size_t)t * n_slices;
+        for (int64_t i = lo; i < hi; i++) hs[read_slice[b.pair_read[sorted[(size_t)i]]]]++;
+    });
+    int64_t run = 0;
+    for (int s = 0; s < n_slices; s++) {
+        (*slice_first)[(size_t)s] = run;
+        for (int t = 0; t < T; t++) { int64_t& c = hist[(size_t)t * n_slices + s]; const int64_t v = c; c = run; run += v; }
     }
-    cnt[nh] = (int)n_sel;
+    (*slice_first)[(size_t)n_slices] = run;
+    parallel_chunks(n, 1 << 17, [&](int t, int64_t lo, int64_t hi) {
+        int64_t* pos = hist.data() + (size_t)t * n_slices;
+        for (int64_t i = lo; i < hi; i++) { const int p = sorted[(size_t)i]; (*out)[(size_t)pos[read_slice[b.pair_read[p]]]++] = p; }
+    });
+}
+
+void plan_short(const HostBatchView& b, const uint8_t* is_short, int N2, int task_rows, ShortPlan* out) {
+    std::vector<int> sorted;
+    sort_pairs_by_hap(b, is_short, &sorted);
+    plan_tasks(b, sorted.data(), (int64_t)sorted.size(), 0, N2, task_rows, out);
+}
+
+// Tasks and warps for a haplotype-major list of n short pairs (`sorted`: caller pair indices).  table_base: what is
+// subtracted from a read's absolute table position (the slice's table starts at its first read).
+void plan_tasks(const HostBatchView& b, const int* sorted, int64_t n_sel, int64_t table_base, int N2, int task_rows, ShortPlan* out) {
+    out->tasks.clear(); out->warp_first.clear();  // the sorted arrays keep their size: they are overwritten in full
+    out->cells = 0; out->padded_cells = 0; out->max_read_len = 0;
     if (n_sel == 0) { out->srt_out.clear(); out->srt_ent.clear(); out->warp_first.push_back(0); return; }
     if (out->srt_out.size() != (size_t)n_sel) {  // steady state: same size as the last call, nothing to (re)initialise
         out->srt_out.resize((size_t)n_sel);
         out->srt_ent.resize((size_t)n_sel * 2);
     }
-    parallel_chunks(np, 1 << 17, [&](int t, int64_t lo, int64_t hi) {
-        std::vector<int>& pos = hist[t];
-        for (int64_t p = lo; p < hi; p++)
-            if (is_short[p]) {
-                const int q = pos[b.pair_hap[p]]++;
-                const int r = b.pair_read[p];
-                out->srt_out[q] = (int)p;
-                out->srt_ent[2 * (size_t)q] = (int)table_run_start(b.read_off[r], r);
-                out->srt_ent[2 * (size_t)q + 1] = table_run_len((int)(b.read_off[r + 1] - b.read_off[r]));
-            }
+    // ---- 1. positions of the reads' runs in the table
+    parallel_chunks(n_sel, 1 << 17, [&](int, int64_t lo, int64_t hi) {
+        for (int64_t q = lo; q < hi; q++) {
+            const int p = sorted[q];
+            const int r = b.pair_read[p];
+            out->srt_out[(size_t)q] = p;
+            out->srt_ent[2 * (size_t)q] = (int)(table_run_start(b.read_off[r], r) - table_base);
+            out->srt_ent[2 * (size_t)q + 1] = table_run_len((int)(b.read_off[r + 1] - b.read_off[r]));
+        }
     });
-    // ---- 2. cut each haplotype's run of reads into tasks of about task_rows read rows (haplotype ranges in parallel)
+    // ---- 2. cut each haplotype's run of reads into tasks of about task_rows read rows (chunks of the list in parallel,
+    //         every chunk starting where the haplotype changes)
     std::vector<ShortTask> tasks;
     {
         std::vector<ShortTask> part[BATCHER_THREADS];
         int64_t pcells[BATCHER_THREADS] = {0};
         int pmax[BATCHER_THREADS] = {0};
-        const int T2 = parallel_chunks(nh, 1 << 12, [&](int t, int64_t hlo, int64_t hhi) {
+        const int T2 = parallel_chunks(n_sel, 1 << 15, [&](int t, int64_t lo, int64_t hi) {
+            auto hap_at = [&](int64_t q) { return b.pair_hap[sorted[q]]; };
+            while (lo > 0 && lo < n_sel && hap_at(lo) == hap_at(lo - 1)) lo++;  // this run belongs to the chunk before
+            while (hi > 0 && hi < n_sel && hap_at(hi) == hap_at(hi - 1)) hi++;
             std::vector<ShortTask>& tv = part[t];
             int64_t cells = 0;
             int mx = 0;
-            for (int64_t h = hlo; h < hhi; h++) {
-                const int lo = cnt[h], hi = cnt[h + 1];
-                if (lo == hi) continue;
+            int64_t q = lo;
+            while (q < hi) {
+                const int h = hap_at(q);
                 const int64_t k = b.hap_off[h + 1] - b.hap_off[h];
-                ShortTask tk = {(int)h, lo, 0, 0, 0};
-                for (int q = lo; q < hi; q++) {
-                    const int r = b.pair_read[out->srt_out[q]];
+                ShortTask tk = {h, (int)q, 0, 0, 0};
+                for (; q < n_sel && hap_at(q) == h; q++) {
+                    const int r = b.pair_read[sorted[q]];
                     const int l = (int)(b.read_off[r + 1] - b.read_off[r]);
                     cells += (int64_t)l * k;
                     if (l > mx) mx = l;
@@ -100,7 +140,7 @@ void plan_short(const HostBatchView& b, const uint8_t* is_short, int N2, int tas
                     tk.ents += out->srt_ent[2 * (size_t)q + 1];
                     if (tk.rows >= task_rows) {
                         tv.push_back(tk);
-                        tk.pair_first = q + 1; tk.n_pairs = 0; tk.rows = 0; tk.ents = 0;
+                        tk.pair_first = (int)q + 1; tk.n_pairs = 0; tk.rows = 0; tk.ents = 0;
                     }
                 }
                 if (tk.n_pairs > 0) tv.push_back(tk);

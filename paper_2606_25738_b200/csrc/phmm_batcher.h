@@ -52,6 +52,12 @@ struct ShortPlan {
 
 // is_short[p] != 0 selects the pairs to plan.  cols_per_lane = 2*NV of the kernel.
 void plan_short(const HostBatchView& b, const uint8_t* is_short, int cols_per_lane, int task_rows, ShortPlan* out);
+// The three stages of plan_short, for batches that are processed in slices of reads (phmm_api.cu):
+void sort_pairs_by_hap(const HostBatchView& b, const uint8_t* is_short, std::vector<int>* sorted);
+void split_by_slice(const HostBatchView& b, const std::vector<int>& sorted, const uint8_t* read_slice, int n_slices,
+                    std::vector<int>* out, std::vector<int64_t>* slice_first);
+void plan_tasks(const HostBatchView& b, const int* sorted, int64_t n_sel, int64_t table_base, int cols_per_lane, int task_rows,
+                ShortPlan* out);
 
 // Validation of offsets / indices / lengths; returns a PHMM_E_* code or 0.
 int validate_batch(const HostBatchView& b);

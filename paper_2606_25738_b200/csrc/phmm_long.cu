@@ -118,7 +118,7 @@ __global__ void __launch_bounds__(LONG_WPC * 32, LONG_MIN_CTAS) k_long_f32(DevBa
         const int64_t ro = b.read_off[r], ho = b.hap_off[h];
         const int l = (int)(b.read_off[r + 1] - ro), k = (int)(b.hap_off[h + 1] - ho);
         const int n_ent = l + TABLE_EXTRA_ROWS;        // run-in entry, rows 1..l, sum entry, flush entry
-        const int run0 = (int)table_run_start(ro, r), run_len = table_run_len(l);
+        const int run0 = (int)(table_run_start(ro, r) - b.table_base), run_len = table_run_len(l);
         const int nstrips = (k + STRIP - 1) / STRIP;
         const bool has_in = strip > 0, has_out = strip + 1 < nstrips;
 

@@ -259,7 +259,7 @@ __global__ void __launch_bounds__(RESCUE_WARPS * 32, RESCUE_MIN_CTAS) k_rescue_f
             const int64_t ro = b.read_off[r];
             ho = b.hap_off[h];
             l = (int)(b.read_off[r + 1] - ro); k = (int)(b.hap_off[h + 1] - ho);
-            run0 = (int)table_run_start(ro, r);
+            run0 = (int)(table_run_start(ro, r) - b.table_base);
         }
         const int n_ent = l + 2;  // run-in entry, rows 1..l, sum entry
         int steps = active ? n_ent + g - 1 : 0;

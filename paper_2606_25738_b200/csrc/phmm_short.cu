@@ -34,14 +34,14 @@ namespace phmm {
 // 4 chunk planes (the four float4 of an entry) x 2 parities x 16 slots.  A lane-strided LDG.128 then costs
 // ~4 L1 wavefronts instead of 32 (ncu: l1tex throughput 90 % -> see profiles/).
 constexpr int TABLE_CHUNK_ENTRIES = 1024;
-__global__ void __launch_bounds__(256) k_table_f32(DevBatch b, const double* __restrict__ lut, float* __restrict__ table) {
-    const int64_t r = (int64_t)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
-    if (r >= b.n_reads) return;
+__global__ void __launch_bounds__(256) k_table_f32(DevBatch b, const double* __restrict__ lut, float* __restrict__ table, int64_t r0, int64_t r1) {
+    const int64_t r = r0 + (int64_t)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+    if (r >= r1) return;
     const int lane = threadIdx.x & 31;
     const int64_t off = b.read_off[r];
     const int l = (int)(b.read_off[r + 1] - off);
     float4* dst = reinterpret_cast<float4*>(table);
-    const int64_t first = table_run_start(off, r);
+    const int64_t first = table_run_start(off, r) - b.table_base;
     const int e_hi = min(table_run_len(l), ((int)blockIdx.y + 1) * TABLE_CHUNK_ENTRIES);
     for (int e = (int)blockIdx.y * TABLE_CHUNK_ENTRIES + lane; e < e_hi; e += 32) {  // (an entry behind the flush entry is all zero too)
         const RowC x = row_constants(b, lut, off, l, e, true), y = row_constants(b, lut, off, l, e - 1, true);
@@ -53,15 +53,15 @@ __global__ void __launch_bounds__(256) k_table_f32(DevBatch b, const double* __r
     }
 }
 
-cudaError_t launch_lut_table(const DevBatch& b, const double* lut, float* table, int max_read_len, cudaStream_t st) {
-    if (b.n_reads == 0) return cudaSuccess;
+cudaError_t launch_lut_table(const DevBatch& b, const double* lut, float* table, int64_t r0, int64_t r1, int max_read_len, cudaStream_t st) {
+    if (r1 <= r0) return cudaSuccess;
     const int wpb = 8;
-    int64_t grid = (b.n_reads + wpb - 1) / wpb;
+    int64_t grid = (r1 - r0 + wpb - 1) / wpb;
     const int chunks = (table_run_len(max_read_len) + TABLE_CHUNK_ENTRIES - 1) / TABLE_CHUNK_ENTRIES;
     // the zero run (whole 32-entry blocks) that idle lanes walk: cleared on every call, whatever the batch size
     cudaError_t e = cudaMemsetAsync(table, 0, (size_t)TABLE_ZERO_RUN * 64, st);
     if (e != cudaSuccess) return e;
-    k_table_f32<<<dim3((unsigned)grid, (unsigned)chunks), wpb * 32, 0, st>>>(b, lut, table);
+    k_table_f32<<<dim3((unsigned)grid, (unsigned)chunks), wpb * 32, 0, st>>>(b, lut, table, r0, r1);
     return cudaGetLastError();
 }
 

@@ -237,6 +237,28 @@ def test_async_calls_back_to_back_bitwise(B, ctx):
                 assert np.array_equal(o.cpu().numpy(), a[0]) and np.array_equal(f.cpu().numpy(), a[1]), "call %d differs" % i
 
 
+def test_slices_of_reads_match_one_slice(B, ctx):
+    """A batch whose row-constant table exceeds the workspace budget (phmm_options.max_table_bytes) is processed in slices
+    of reads, each with its own table, plan and launches (stats.n_slices > 1): outputs and flags must be bitwise those of
+    the one-slice run, through both entries and in both precisions; long pairs and rescued pairs included."""
+    b = W.generate(2, n=40000)
+    out1, fl1 = run(B, ctx, b, B.PHMM_FP32_RESCUE)
+    assert ctx.stats()["n_slices"] == 1
+    n_resc = ctx.stats()["n_rescued"]
+    c = B.Context(0, max_table_bytes=24 << 20)
+    try:
+        out2, fl2 = run(B, c, b, B.PHMM_FP32_RESCUE)
+        st = c.stats()
+        assert st["n_slices"] >= 5 and st["table_bytes"] <= 24 << 20
+        assert np.array_equal(out1, out2) and np.array_equal(fl1, fl2)
+        assert st["n_rescued"] == n_resc and st["n_pairs"] == b.n_pairs and st["cells"] == b.cells()
+        oh, fh = c.forward_batch_host(b, B.PHMM_FP32_RESCUE)
+        assert np.array_equal(oh, out1) and np.array_equal(fh, fl1)
+        assert c.stats()["n_rescued"] == n_resc
+    finally:
+        c.close()
+
+
 def test_host_entry_matches_device_entry(B, ctx):
     b = W.generate(1, n=3)
     out, fl = run(B, ctx, b, B.PHMM_FP32_RESCUE)
