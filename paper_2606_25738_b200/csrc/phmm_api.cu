@@ -88,7 +88,7 @@ struct phmm_ctx {
     DevBuf d_rq, d_rq_queue, d_rq_sorted, d_rq_plan;  // fp64 sub-warp recomputation: counters, queue, ordered queue, plan
     DevBuf d_payload, d_out, d_flags;  // phmm_forward_batch_host only
     std::vector<uint8_t> is_short, read_slice;
-    std::vector<int> sorted_all, sorted_split;
+    std::vector<int> sorted_all, slice_ids, short_ids;
     ShortPlan plan;
     int chain_grid[2] = {0, 0};  // resident CTAs of the fp64 chain kernel ([1]; [0] unused)
     int long_grid = 0, rescue_grid = 0;  // resident CTAs of the fp32 long kernel / of the fp64 sub-warp kernel on this device
@@ -279,8 +279,9 @@ struct SliceWork {  // one slice of reads [r0, r1) of a call and the pairs that 
     int64_t r0 = 0, r1 = 0;
     int64_t table_base = 0;     // absolute table position of the slice's zero run
     int64_t table_entries = 0;  // entries of the slice's table (zero run and slack included)
-    const int* short_sorted = nullptr;  // haplotype-major short pairs (fp32 mode)
-    int64_t n_short = 0;
+    const int* ids = nullptr;   // the slice's pairs (caller pair indices, ascending); nullptr: all pairs of the batch
+    int64_t n_ids = 0;
+    int64_t n_short = 0;        // pairs of the sub-warp systolic fp32 kernel
     std::vector<int> seq_pairs, strip_pairs, sub_pairs;  // chain kernel work lists, fp64 sub-warp list (caller pair indices)
     int64_t n_pairs = 0, lane_rows = 0;
     int max_seq_l = 0, max_long_l = 0;  // longest read of the short class / of the long pairs
@@ -328,81 +329,16 @@ static int forward_impl(phmm_ctx* ctx, const phmm_batch* b, int precision, doubl
         if (!fp64 && w.table_entries * 64 > ctx->opt.max_table_bytes && n_slices >= std::min<int64_t>(250, nr)) return PHMM_E_NOMEM;
     }
 
-    // ---- classify: short (sub-warp systolic fp32 kernel) / fp64 sub-warp / chain-sequential (one warp per pair) / strips
-    if (ctx->is_short.size() != (size_t)np) ctx->is_short.resize((size_t)np);
-    int64_t cells = 0, n_long = 0;
-    {
-        struct Part { std::vector<int> seq, strip, sub; int64_t cells = 0; };
-        Part part[BATCHER_THREADS];
-        const int long_k = ctx->opt.long_min_hap_len;
-        uint8_t* is_short = ctx->is_short.data();
-        const int T = parallel_chunks(np, 1 << 16, [&](int t, int64_t lo, int64_t hi) {
-            Part& q = part[t];
-            for (int64_t p = lo; p < hi; p++) {
-                const int r = b->h_pair_read[p], h = b->h_pair_hap[p];
-                const int64_t l = b->h_read_off[r + 1] - b->h_read_off[r], k = b->h_hap_off[h + 1] - b->h_hap_off[h];
-                q.cells += l * k;
-                uint8_t sh = 0;
-                if (k > long_k || l > 4096) q.strip.push_back((int)p);
-                else if (fp64 && k <= RESCUE_MAX_K && l <= RESCUE_MAX_L) q.sub.push_back((int)p);
-                else if (fp64) q.seq.push_back((int)p);
-                else sh = 1;
-                is_short[p] = sh;
-            }
-        });
-        // chunks are contiguous and in order: the per-slice lists stay sorted by pair index
-        auto deal = [&](const std::vector<int>& v, int which) {
-            for (int p : v) {
-                const int r = b->h_pair_read[p];
-                SliceWork& w = sl[n_slices > 1 ? ctx->read_slice[(size_t)r] : 0];
-                const int l = (int)(b->h_read_off[r + 1] - b->h_read_off[r]);
-                if (which == 0) { w.strip_pairs.push_back(p); if (l > w.max_long_l) w.max_long_l = l; }
-                else { (which == 1 ? w.sub_pairs : w.seq_pairs).push_back(p); if (l > w.max_seq_l) w.max_seq_l = l; }
-            }
-        };
-        for (int t = 0; t < T; t++) {
-            deal(part[t].strip, 0); deal(part[t].sub, 1); deal(part[t].seq, 2);
-            cells += part[t].cells; n_long += (int64_t)part[t].strip.size();
-        }
+    // ---- the pairs of each slice (stable: ascending pair index within a slice)
+    std::vector<int64_t> first((size_t)n_slices + 1, 0);
+    if (n_slices > 1) {
+        bucket_pairs_by_slice(hv, ctx->read_slice.data(), n_slices, &ctx->slice_ids, &first);
+        for (int s = 0; s < n_slices; s++) { sl[(size_t)s].ids = ctx->slice_ids.data() + first[(size_t)s]; sl[(size_t)s].n_ids = first[(size_t)s + 1] - first[(size_t)s]; }
+    } else {
+        sl[0].n_ids = np;
     }
     ctx->stats.n_pairs = np;
-    ctx->stats.cells = cells;
-    ctx->stats.n_long_pairs = n_long;
-    ctx->stats.n_short_pairs = np - n_long;
     ctx->stats.n_slices = n_slices;
-
-    // ---- fp32: the short pairs in haplotype-major order, split (stably) by slice
-    std::vector<int64_t> short_first((size_t)n_slices + 1, 0);
-    if (!fp64) {
-        sort_pairs_by_hap(hv, ctx->is_short.data(), &ctx->sorted_all);
-        const std::vector<int>* order = &ctx->sorted_all;
-        if (n_slices > 1) {
-            split_by_slice(hv, ctx->sorted_all, ctx->read_slice.data(), n_slices, &ctx->sorted_split, &short_first);
-            order = &ctx->sorted_split;
-        } else {
-            short_first[1] = (int64_t)ctx->sorted_all.size();
-        }
-        for (int s = 0; s < n_slices; s++) {
-            SliceWork& w = sl[(size_t)s];
-            w.short_sorted = order->data() + short_first[(size_t)s];
-            w.n_short = short_first[(size_t)s + 1] - short_first[(size_t)s];
-            int64_t lane_rows = 0;
-            int mx = 0;
-            for (int64_t q = 0; q < w.n_short; q += 16) {  // (a 1-in-16 sample is enough for the task-size heuristic)
-                const int p = w.short_sorted[q];
-                const int r = b->h_pair_read[p], h = b->h_pair_hap[p];
-                const int64_t l = b->h_read_off[r + 1] - b->h_read_off[r], k = b->h_hap_off[h + 1] - b->h_hap_off[h];
-                lane_rows += 16 * l * ((k + SHORT_N2 - 1) / SHORT_N2);
-                if (l > mx) mx = (int)l;
-            }
-            w.lane_rows = lane_rows;
-            (void)mx;
-        }
-    }
-    for (int s = 0; s < n_slices; s++) {
-        SliceWork& w = sl[(size_t)s];
-        w.n_pairs = w.n_short + (int64_t)(w.strip_pairs.size() + w.sub_pairs.size() + w.seq_pairs.size());
-    }
     ctx->stats.host_batch_ms = std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - t0).count();
 
     // ---- per call: offsets and pair list to the device, on the copy stream (under the kernels of the previous call)
@@ -436,7 +372,7 @@ static int forward_impl(phmm_ctx* ctx, const phmm_batch* b, int precision, doubl
 
     // ---- slice after slice
     for (int s = 0; s < n_slices; s++) {
-        if (sl[(size_t)s].n_pairs == 0) continue;
+        if (sl[(size_t)s].n_ids == 0) continue;
         RC(run_slice(ctx, b, hv, fp64, d_out, d_flags, st, cs, sl[(size_t)s], hp));
     }
     return PHMM_OK;
@@ -445,7 +381,44 @@ static int forward_impl(phmm_ctx* ctx, const phmm_batch* b, int precision, doubl
 static int run_slice(phmm_ctx* ctx, const phmm_batch* b, const HostBatchView& hv, bool fp64, double* d_out, uint8_t* d_flags,
                      cudaStream_t st, const phmm_ctx::CallSet& cs, SliceWork& sw, const HostPayload* hp) {
     const auto t0 = std::chrono::steady_clock::now();
-    const int64_t np_slice = sw.n_pairs;
+    const int64_t np_slice = sw.n_ids;
+    // ---- classify: short (sub-warp systolic fp32 kernel) / fp64 sub-warp / chain-sequential (one warp per pair) / strips
+    {
+        struct Part { std::vector<int> seq, strip, sub, sh; int64_t cells = 0, lane_rows = 0; int max_l = 0, max_l_long = 0; };
+        Part part[BATCHER_THREADS];
+        const int long_k = ctx->opt.long_min_hap_len;
+        const int* ids = sw.ids;
+        const int T = parallel_chunks(np_slice, 1 << 16, [&](int t, int64_t lo, int64_t hi) {
+            Part& q = part[t];
+            for (int64_t i = lo; i < hi; i++) {
+                const int p = ids ? ids[i] : (int)i;
+                const int r = b->h_pair_read[p], h = b->h_pair_hap[p];
+                const int64_t l = b->h_read_off[r + 1] - b->h_read_off[r], k = b->h_hap_off[h + 1] - b->h_hap_off[h];
+                q.cells += l * k;
+                if (k > long_k || l > 4096) { q.strip.push_back(p); if (l > q.max_l_long) q.max_l_long = (int)l; }
+                else {
+                    if (fp64 && k <= RESCUE_MAX_K && l <= RESCUE_MAX_L) q.sub.push_back(p);
+                    else if (fp64) q.seq.push_back(p);
+                    else { q.sh.push_back(p); q.lane_rows += l * ((k + SHORT_N2 - 1) / SHORT_N2); }
+                    if (l > q.max_l) q.max_l = (int)l;
+                }
+            }
+        });
+        ctx->short_ids.clear();
+        for (int t = 0; t < T; t++) {  // chunks are contiguous and in order: the lists stay sorted by pair index
+            sw.seq_pairs.insert(sw.seq_pairs.end(), part[t].seq.begin(), part[t].seq.end());
+            sw.strip_pairs.insert(sw.strip_pairs.end(), part[t].strip.begin(), part[t].strip.end());
+            sw.sub_pairs.insert(sw.sub_pairs.end(), part[t].sub.begin(), part[t].sub.end());
+            ctx->short_ids.insert(ctx->short_ids.end(), part[t].sh.begin(), part[t].sh.end());
+            ctx->stats.cells += part[t].cells; sw.lane_rows += part[t].lane_rows;
+            if (part[t].max_l > sw.max_seq_l) sw.max_seq_l = part[t].max_l;
+            if (part[t].max_l_long > sw.max_long_l) sw.max_long_l = part[t].max_l_long;
+        }
+        sw.n_short = (int64_t)ctx->short_ids.size();
+        ctx->stats.n_long_pairs += (int64_t)sw.strip_pairs.size();
+        ctx->stats.n_short_pairs += np_slice - (int64_t)sw.strip_pairs.size();
+        if (!fp64) sort_ids_by_hap(hv, ctx->short_ids.data(), sw.n_short, &ctx->sorted_all);  // haplotype-major
+    }
     // task size: as large as possible (fewer run-ins, pipeline fills and host work; 8192 rows measured best on
     // configs[1]) while leaving at least ~6 warps of work per resident warp slot
     int task_rows = ctx->opt.task_rows;
@@ -453,7 +426,7 @@ static int run_slice(phmm_ctx* ctx, const phmm_batch* b, const HostBatchView& hv
         const int64_t slots = (int64_t)ctx->n_sm * 12;
         task_rows = (int)std::max<int64_t>(1024, std::min<int64_t>(8192, sw.lane_rows / 32 / (6 * slots)));
     }
-    if (!fp64) plan_tasks(hv, sw.short_sorted, sw.n_short, sw.table_base, SHORT_N2, task_rows, &ctx->plan);
+    if (!fp64) plan_tasks(hv, ctx->sorted_all.data(), sw.n_short, sw.table_base, SHORT_N2, task_rows, &ctx->plan);
     else { ctx->plan.tasks.clear(); ctx->plan.warp_first.assign(1, 0); ctx->plan.srt_out.clear(); ctx->plan.srt_ent.clear(); ctx->plan.cells = 0; ctx->plan.padded_cells = 0; ctx->plan.max_read_len = 0; }
     const ShortPlan& pl = ctx->plan;
     const int n_warps = (int)pl.warp_first.size() - 1;

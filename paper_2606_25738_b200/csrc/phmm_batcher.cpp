@@ -62,16 +62,16 @@ void sort_pairs_by_hap(const HostBatchView& b, const uint8_t* is_short, std::vec
     });
 }
 
-// Stable split of a haplotype-major pair list into slices of reads: slice_first[s] = first position of slice s in `out`.
-void split_by_slice(const HostBatchView& b, const std::vector<int>& sorted, const uint8_t* read_slice, int n_slices,
-                    std::vector<int>* out, std::vector<int64_t>* slice_first) {
-    const int64_t n = (int64_t)sorted.size();
+// Stable counting sort of all pair indices by the slice their read belongs to: slice_first[s] = first position of slice s.
+void bucket_pairs_by_slice(const HostBatchView& b, const uint8_t* read_slice, int n_slices, std::vector<int>* out,
+                           std::vector<int64_t>* slice_first) {
+    const int64_t n = b.n_pairs;
     out->resize((size_t)n);
     slice_first->assign((size_t)n_slices + 1, 0);
     std::vector<int64_t> hist((size_t)BATCHER_THREADS * (size_t)n_slices, 0);
     const int T = parallel_chunks(n, 1 << 17, [&](int t, int64_t lo, int64_t hi) {
         int64_t* hs = hist.data() + (size_t)t * n_slices;
-        for (int64_t i = lo; i < hi; i++) hs[read_slice[b.pair_read[sorted[(size_t)i]]]]++;
+        for (int64_t p = lo; p < hi; p++) hs[read_slice[b.pair_read[p]]]++;
     });
     int64_t run = 0;
     for (int s = 0; s < n_slices; s++) {
@@ -79,9 +79,39 @@ void split_by_slice(const HostBatchView& b, const std::vector<int>& sorted, cons
         for (int t = 0; t < T; t++) { int64_t& c = hist[(size_t)t * n_slices + s]; const int64_t v = c; c = run; run += v; }
     }
     (*slice_first)[(size_t)n_slices] = run;
+    int* dst = out->data();
     parallel_chunks(n, 1 << 17, [&](int t, int64_t lo, int64_t hi) {
         int64_t* pos = hist.data() + (size_t)t * n_slices;
-        for (int64_t i = lo; i < hi; i++) { const int p = sorted[(size_t)i]; (*out)[(size_t)pos[read_slice[b.pair_read[p]]]++] = p; }
+        for (int64_t p = lo; p < hi; p++) dst[pos[read_slice[b.pair_read[p]]]++] = (int)p;
+    });
+}
+
+// Stable counting sort of a list of pair indices by haplotype; the histogram spans only the haplotypes the list uses.
+void sort_ids_by_hap(const HostBatchView& b, const int* ids, int64_t n, std::vector<int>* sorted) {
+    if (sorted->size() != (size_t)n) sorted->resize((size_t)n);
+    if (n == 0) return;
+    int hmin[BATCHER_THREADS], hmax[BATCHER_THREADS];
+    const int T0 = parallel_chunks(n, 1 << 17, [&](int t, int64_t lo, int64_t hi) {
+        int mn = INT32_MAX, mx = -1;
+        for (int64_t i = lo; i < hi; i++) { const int h = b.pair_hap[ids[i]]; mn = std::min(mn, h); mx = std::max(mx, h); }
+        hmin[t] = mn; hmax[t] = mx;
+    });
+    int h0 = INT32_MAX, h1 = -1;
+    for (int t = 0; t < T0; t++) { h0 = std::min(h0, hmin[t]); h1 = std::max(h1, hmax[t]); }
+    const int64_t nh = (int64_t)h1 - h0 + 1;
+    std::vector<std::vector<int>> hist(BATCHER_THREADS);
+    const int T = parallel_chunks(n, 1 << 17, [&](int t, int64_t lo, int64_t hi) {
+        std::vector<int>& hs = hist[t];
+        hs.assign((size_t)nh, 0);
+        for (int64_t i = lo; i < hi; i++) hs[b.pair_hap[ids[i]] - h0]++;
+    });
+    int64_t run = 0;
+    for (int64_t h = 0; h < nh; h++)
+        for (int t = 0; t < T; t++) { const int c = hist[t][h]; hist[t][h] = (int)run; run += c; }
+    int* out = sorted->data();
+    parallel_chunks(n, 1 << 17, [&](int t, int64_t lo, int64_t hi) {
+        std::vector<int>& pos = hist[t];
+        for (int64_t i = lo; i < hi; i++) { const int p = ids[i]; out[pos[b.pair_hap[p] - h0]++] = p; }
     });
 }
 

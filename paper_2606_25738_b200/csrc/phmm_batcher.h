@@ -19,7 +19,7 @@
 namespace phmm {
 
 // fn(t, begin, end) over [0, n) in contiguous chunks on up to BATCHER_THREADS threads (the caller's included)
-constexpr int BATCHER_THREADS = 8;
+constexpr int BATCHER_THREADS = 16;
 template <typename F> inline int parallel_chunks(int64_t n, int64_t min_chunk, F fn) {
     int T = (int)std::min<int64_t>(BATCHER_THREADS, std::max<int64_t>(1, n / min_chunk));
     const unsigned hw = std::thread::hardware_concurrency();
@@ -54,8 +54,9 @@ struct ShortPlan {
 void plan_short(const HostBatchView& b, const uint8_t* is_short, int cols_per_lane, int task_rows, ShortPlan* out);
 // The three stages of plan_short, for batches that are processed in slices of reads (phmm_api.cu):
 void sort_pairs_by_hap(const HostBatchView& b, const uint8_t* is_short, std::vector<int>* sorted);
-void split_by_slice(const HostBatchView& b, const std::vector<int>& sorted, const uint8_t* read_slice, int n_slices,
-                    std::vector<int>* out, std::vector<int64_t>* slice_first);
+void bucket_pairs_by_slice(const HostBatchView& b, const uint8_t* read_slice, int n_slices, std::vector<int>* out,
+                           std::vector<int64_t>* slice_first);
+void sort_ids_by_hap(const HostBatchView& b, const int* ids, int64_t n, std::vector<int>* sorted);
 void plan_tasks(const HostBatchView& b, const int* sorted, int64_t n_sel, int64_t table_base, int cols_per_lane, int task_rows,
                 ShortPlan* out);
 
