@@ -46,6 +46,8 @@ WORKLOADS = {  # name -> (BASELINE.json config index, description)
     "verylong": (4, "configs[4] very-long stress: 16 pairs of 100 kbp x 105 kbp"),
     "equal": (5, "paper's scalability-sweep shape (PAPER.md:366): read length = haplotype length = --len, noisy copies"),
 }
+L2_NOTE = ("no flush: the inputs of a step exceed L2 (payload plus the row-constant table, which is rewritten and re-read "
+           "every step; 2.9 GB on the short-read batch, 1.3 GB on the long-read batch, 126 MB of L2)")
 FLOPS_PER_CELL = 10.0  # SURVEY 8(d)'s algorithmic count (4 FMA + 2 MUL per cell); DESIGN.md section 7
 FLOPS_PER_CELL_EXECUTED = {"fp32": 9.0, "fp64": 11.0}  # what the engines issue: 4 FMA + 1 MUL (fp32 T/J form), 4 FMA + 3 MUL (fp64 sub-warp kernel)
 
@@ -59,14 +61,15 @@ def _measured_peaks():
 
 
 def _profiled_traffic(name, workload, scale):
-    """DRAM bytes per launch of the dominant kernel from the committed ncu capture (profiles/traffic.json),
-    scaled linearly from the captured batch size to this run's; None if there is no capture of this workload."""
+    """DRAM bytes per launch of the dominant kernel from the committed `ncu --set full` capture of THIS kernel on THIS
+    workload at THIS scale (profiles/traffic.json; DRAM counters cannot be read outside a profiler); None when the
+    committed capture is of another workload or size -- nothing is scaled."""
     try:
         with open(os.path.join(ROOT, "profiles", "traffic.json")) as f:
             e = json.load(f).get(name)
-        if not e or e.get("workload") != workload:
+        if not e or e.get("workload") != workload or abs(float(e["scale"]) - float(scale)) > 1e-9:
             return None
-        return float(e["dram_bytes_per_launch"]) * scale / float(e["scale"])
+        return float(e["dram_bytes_per_launch"])
     except Exception:
         return None
 
@@ -170,7 +173,10 @@ def run_reference(args, rank, world):
         "impl": "reference", "metric": "PairHMM forward throughput", "value": v, "unit": "GCUPS", "n_gpus": args.gpus,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": tot_s / max(1, args.steps) * 1e3,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": WORKLOADS[args.workload][1], "precision": args.precision, "scale": args.scale},
+        "config": {"workload": WORKLOADS[args.workload][1] + (" (len %d)" % args.len if cfg == 5 else ""),
+                   "precision": "fp32 + fp64 rescue" if args.precision == "fp32" else "fp64",
+                   "scale": args.scale, "pairs": int(batch.n_pairs), "cells": int(batch.cells()), "parallelism": "replicas x%d" % world,
+                   "l2": L2_NOTE},
         "pairs_per_s": tot_pairs / tot_s,
         "cpu_baseline": {"value": v, "unit": "GCUPS", "cores": res["cores"], "kind": "oracle", "sample": sample},
         "e2e": {"value": v, "unit": "GCUPS", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
@@ -178,40 +184,15 @@ def run_reference(args, rank, world):
     }))
 
 
-def main():
-    ap = argparse.ArgumentParser()
-    ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=10)
-    ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
-    ap.add_argument("--workload", default="short", choices=sorted(WORKLOADS))
-    ap.add_argument("--precision", default="fp32", choices=["fp32", "fp64"])
-    ap.add_argument("--scale", type=float, default=1.0, help="fraction of the workload's full size")
-    ap.add_argument("--len", type=int, default=512, help="--workload equal: read length = haplotype length")
-    ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--no-e2e", action="store_true")
-    args = ap.parse_args()
-    args.warmup = max(args.warmup, 3) if args.impl == "b200" else args.warmup
-
-    rank = int(os.environ.get("RANK", "0"))
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
-    if args.impl == "reference":
-        run_reference(args, rank, world)
-        return
-
+def measure(args, workload, steps, rank, world, local, with_cpu):
+    """One workload: K pipelined calls (the headline number), 5 individually timed calls (median / best), the end-to-end
+    leg, the roofline of the dominant kernel and (rank 0, with_cpu) the oracle on a bounded sample."""
     import torch
     import torch.distributed as dist
     from paper_2606_25738_b200 import binding, replicas
 
-    if not torch.cuda.is_available():
-        raise SystemExit("bench.py: no CUDA device (there is no CPU fallback)")
-    torch.cuda.set_device(local)
     dev = "cuda:%d" % local
-    if world > 1:
-        dist.init_process_group("nccl", device_id=torch.device(dev))
-
-    batch, cfg = make_batch(args.workload, args.scale, replicas.rank_seed(0, rank), args.len)
+    batch, cfg = make_batch(workload, args.scale, replicas.rank_seed(0, rank), args.len)
     cells, n_pairs = batch.cells(), batch.n_pairs
     prec = binding.PHMM_FP32_RESCUE if args.precision == "fp32" else binding.PHMM_FP64
     ctx = binding.Context(local, profile_events=1)
@@ -235,24 +216,36 @@ def main():
         sampler.start()
         time.sleep(0.3)
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    fam = {"ms_table": 0.0, "ms_short": 0.0, "ms_rescue": 0.0, "ms_long": 0.0}
-    host_ms = 0.0
     barrier()
     e0.record()
-    for _ in range(args.steps):
+    for _ in range(steps):
         # asynchronous: the host batcher (row a11) of call s+1 runs while the GPU works on call s
         ctx.forward_batch(db, prec, out=out, flags=flags, sync=False)
     e1.record()
     barrier()
     ms = e0.elapsed_time(e1)
     s = ctx.stats()  # per-family CUDA-event durations of the last timed call
-    for k in fam:
-        fam[k] = s[k]
+    fam = {k: s[k] for k in ("ms_table", "ms_short", "ms_rescue", "ms_long")}
     host_ms = s["host_batch_ms"]
+    # ---- SURVEY 8(d) protocol: 5 calls timed one by one (host batcher inside, nothing to overlap with): median and best
+    single = []
+    for _ in range(5):
+        a0, a1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        t_host = time.perf_counter()
+        a0.record()
+        ctx.forward_batch(db, prec, out=out, flags=flags, sync=False)
+        a1.record()
+        torch.cuda.synchronize()
+        single.append((a0.elapsed_time(a1), (time.perf_counter() - t_host) * 1e3))
     clocks = sampler.stop() if sampler else None
     ms, tot_cells, tot_pairs = replicas.aggregate(ms, cells, n_pairs, dist if world > 1 else None, dev)
-    ms_step = ms / args.steps
-    gcups = replicas.whole_job_gcups(ms, tot_cells, args.steps)
+    ms_step = ms / steps
+    gcups = replicas.whole_job_gcups(ms, tot_cells, steps)
+    wall = sorted(w for _, w in single)
+    per_call = {"n": len(single), "median_ms": wall[len(wall) // 2], "best_ms": wall[0],
+                "median_gcups": cells / (wall[len(wall) // 2] * 1e-3) / 1e9, "best_gcups": cells / (wall[0] * 1e-3) / 1e9,
+                "timer": "host wall clock around one synchronised call of this rank (host batcher included, no overlap)"}
 
     # ---- end to end: host (pinned) buffers in, host results out, copies inside the timed region
     e2e = None
@@ -262,7 +255,7 @@ def main():
             ctx.forward_batch_host(hb, prec)
         barrier()
         t0 = time.perf_counter()
-        for _ in range(args.steps):
+        for _ in range(steps):
             ctx.forward_batch_host(hb, prec)
         torch.cuda.synchronize()
         dt = time.perf_counter() - t0
@@ -270,14 +263,13 @@ def main():
             t = torch.tensor([dt], dtype=torch.float64, device=dev)
             dist.all_reduce(t, op=dist.ReduceOp.MAX)
             dt = float(t.item())
-        e2e = {"value": tot_cells / (dt / args.steps) / 1e9, "unit": "GCUPS",
+        e2e = {"value": tot_cells / (dt / steps) / 1e9, "unit": "GCUPS",
                "h2d_bytes_per_step": int(hb.h2d_bytes()), "d2h_bytes_per_step": int(hb.d2h_bytes()),
-               "ms_per_step": dt / args.steps * 1e3, "timer": "host wall clock around the synchronous C-ABI call"}
-
+               "ms_per_step": dt / steps * 1e3, "slices": ctx.stats()["n_slices"],
+               "timer": "host wall clock around the synchronous C-ABI call"}
+        del hb
     if rank != 0:
-        if world > 1:
-            dist.destroy_process_group()
-        return
+        return None
 
     # ---- roofline of the dominant kernel
     peaks = _measured_peaks()
@@ -291,46 +283,101 @@ def main():
         meas = binding.measure_peak(2, local)
     peak = prop.multi_processor_count * lanes * 2 * sm_max * 1e6 / 1e12
     if st["n_long_pairs"] * 2 > st["n_pairs"]:
-        kname, kms, kcells = "k_chain (concurrent strips)", fam["ms_long"], cells * 1.0
+        kname = "k_long_f32" if args.precision == "fp32" else "k_chain<double> (concurrent strips)"
+        kms, kcells = fam["ms_long"], cells * 1.0
     elif args.precision == "fp64":
         kname, kms, kcells = "k_rescue_f64 (+ chain fallback)", fam["ms_rescue"], cells * 1.0
     else:
         kname, kms, kcells = "k_short_f32", fam["ms_short"], float(st["short_cells"])
     achieved = FLOPS_PER_CELL * kcells / (kms * 1e-3) / 1e12 if kms > 0 else 0.0
+    step_tflops = FLOPS_PER_CELL * tot_cells / world / (ms_step * 1e-3) / 1e12
     roofline = {"bound": "alu", "kernel": kname, "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
-                "frac": achieved / peak, "traffic": _profiled_traffic(kname.split(" ")[0].split("<")[0], args.workload, args.scale),
+                "frac": achieved / peak, "traffic": _profiled_traffic(kname.split(" ")[0].split("<")[0], workload, args.scale),
                 "peak_source": "nominal non-tensor %s peak = %d SMs x %d lanes x 2 x %.0f MHz (DESIGN.md); in-run FMA "
                                "microbenchmark measured %.2f TFLOP/s" % (args.precision.upper(), prop.multi_processor_count,
                                                                         lanes, sm_max, meas),
                 "flops_per_cell": FLOPS_PER_CELL, "flops_per_cell_executed": FLOPS_PER_CELL_EXECUTED[args.precision],
                 "frac_at_executed_flops": achieved / peak * FLOPS_PER_CELL_EXECUTED[args.precision] / FLOPS_PER_CELL,
+                "whole_step_frac": step_tflops / peak,
+                "whole_step_frac_at_executed_flops": step_tflops / peak * FLOPS_PER_CELL_EXECUTED[args.precision] / FLOPS_PER_CELL,
                 "kernel_ms_per_launch": kms, "kernel_gcups": kcells / (kms * 1e-3) / 1e9 if kms > 0 else 0.0,
                 "kernel_share_of_step": kms / ms_step if ms_step > 0 else None,
                 "hbm_gbs_achieved": None, "family_ms": fam, "host_batch_ms": host_ms}
-    if roofline["traffic"] and kms > 0:  # DRAM bytes of the committed ncu capture (scaled to this batch) / this run's kernel time
+    if roofline["traffic"] and kms > 0:  # DRAM bytes of the committed ncu capture of this very workload and scale / this run's kernel time
         roofline["hbm_gbs_achieved"] = roofline["traffic"] / (kms * 1e-3) / 1e9
         roofline["hbm_frac_of_measured_peak"] = roofline["hbm_gbs_achieved"] / float(peaks.get("hbm_gbs") or 6471.1)
 
     cpu = None
-    if not args.no_cpu_baseline:
+    if with_cpu:
         r = oracle_sample(batch, 15.0)
         cpu = {"value": r["gcups"], "unit": "GCUPS", "cores": r["cores"], "kind": "oracle",
-               "sample": "uniform random sample of %d pairs (%.3g cells) of the same batch, %.1f s" % (r["pairs"], r["cells"], r["seconds"])}
-
-    line = {
-        "metric": "PairHMM forward throughput", "value": gcups, "unit": "GCUPS", "n_gpus": world, "steps": args.steps,
-        "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-        "dtype": "f32" if args.precision == "fp32" else "f64", "data": "synthetic",
-        "config": {"workload": WORKLOADS[args.workload][1] + (" (len %d)" % args.len if cfg == 5 else ""),
+               "sample": "uniform random sample of %d pairs (%.3g cells) of the same batch, %.1f s; the --impl reference arm "
+                         "times other samples of the same batch (6 s each)" % (r["pairs"], r["cells"], r["seconds"])}
+    ctx.close()
+    return {
+        "value": gcups, "unit": "GCUPS", "steps": steps, "ms_per_step": ms_step,
+        "config": {"workload": WORKLOADS[workload][1] + (" (len %d)" % args.len if cfg == 5 else ""),
                    "precision": "fp32 + fp64 rescue" if args.precision == "fp32" else "fp64",
                    "scale": args.scale, "pairs": int(tot_pairs), "cells": int(tot_cells), "parallelism": "replicas x%d" % world,
-                   "l2": "inputs larger than L2 (payload + %.0f MB row-constant table rewritten and re-read every step)" % (st["table_bytes"] / 1e6)},
-        "pairs_per_s": tot_pairs / (ms_step * 1e-3),
-        "clocks": clocks, "e2e": e2e, "gpu_launches": int(st["n_kernel_launches"]) * args.steps,
+                   "l2": L2_NOTE},
+        "pairs_per_s": tot_pairs / (ms_step * 1e-3), "per_call": per_call,
+        "clocks": clocks, "e2e": e2e, "gpu_launches": int(st["n_kernel_launches"]) * steps,
         "roofline": roofline, "cpu_baseline": cpu,
-        "stats": {k: st[k] for k in ("n_short_pairs", "n_long_pairs", "n_rescued", "short_cells", "short_padded_cells", "n_short_warps")},
+        "stats": {k: st[k] for k in ("n_short_pairs", "n_long_pairs", "n_rescued", "short_cells", "short_padded_cells", "n_short_warps",
+                                     "n_slices", "table_bytes")},
     }
-    print(json.dumps(line))
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    ap.add_argument("--workload", default="short", choices=sorted(WORKLOADS))
+    ap.add_argument("--precision", default="fp32", choices=["fp32", "fp64"])
+    ap.add_argument("--scale", type=float, default=1.0, help="fraction of the workload's full size")
+    ap.add_argument("--len", type=int, default=512, help="--workload equal: read length = haplotype length")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-secondary", action="store_true",
+                    help="default run (short-read batch, full size): do not also measure the long-read target batch configs[3]")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "b200" else args.warmup
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if args.impl == "reference":
+        run_reference(args, rank, world)
+        return
+
+    import torch
+    import torch.distributed as dist
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (there is no CPU fallback)")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda:%d" % local))
+
+    head = measure(args, args.workload, args.steps, rank, world, local, with_cpu=not args.no_cpu_baseline)
+    # north_star names two target batches: the short-read batch (the headline, configs[1]) and the 10k-bp long-read
+    # batch (configs[3]); the default run measures both, the second one in `secondary` with the same keys
+    secondary = []
+    if args.workload == "short" and args.scale >= 1.0 and args.precision == "fp32" and not args.no_secondary:
+        sec = measure(args, "long", max(3, min(args.steps, 5)), rank, world, local, with_cpu=False)
+        if sec is not None:
+            secondary.append(sec)
+    if rank == 0:
+        line = {"metric": "PairHMM forward throughput", "value": head["value"], "unit": "GCUPS", "n_gpus": world,
+                "steps": args.steps, "warmup": args.warmup, "ms_per_step": head["ms_per_step"], "higher_is_better": True,
+                "scaling": "weak", "vs_baseline": None, "dtype": "f32" if args.precision == "fp32" else "f64",
+                "data": "synthetic"}
+        for k in ("config", "pairs_per_s", "per_call", "clocks", "e2e", "roofline", "cpu_baseline", "stats"):
+            line[k] = head[k]
+        line["gpu_launches"] = head["gpu_launches"] + sum(x["gpu_launches"] for x in secondary)
+        line["secondary"] = secondary
+        print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()
 

@@ -14,15 +14,15 @@
  * Conventions
  *   - "host" / "device" below says where a pointer must live.  Device buffers are allocated by
  *     the caller (e.g. through PyTorch); the library only reads inputs and writes the outputs.
- *   - Bases are bytes compared literally (Eq.3: r_i == h_j); the workloads use ASCII A,C,G,T.
- *     Only the low 2 bits after the mapping A->0 C->1 G->2 T->3 are used on the device; any other
- *     byte is mapped to a code that matches nothing in the other sequence ('N' matches nothing,
- *     DESIGN.md reading G17) -- on the read side it is code 4, on the haplotype side it is "no bit set".
- *   - Qualities are RAW Phred bytes 0..93 (NOT ASCII+33; reading G5):
+ *   - Bases are compared literally (Eq.3: r_i == h_j) over the alphabet A, C, G, T, N: an N matches an N and nothing
+ *     else (reading G17; phmm_options.n_is_wildcard makes it match everything).  Any other byte is treated
+ *     as N; phmm_options.validate rejects it.
+ *   - Qualities are RAW Phred bytes 0..93 (NOT ASCII+33 unless phmm_options.qual_offset says so; reading G5):
  *        eps = 10^(-Qbase/10), iota = 10^(-Qins/10), delta = 10^(-Qdel/10), gamma = 10^(-Qgcp/10);
  *        T_MM = 1-iota-delta, T_MI = iota, T_MD = delta, T_II = T_DD = gamma, T_IM = T_DM = 1-gamma,
  *     all taken at the read position (row) of the cell being written.  Precondition: iota+delta < 1.
- *   - All calls are thread-compatible per context (one context = one caller at a time).
+ *   - All calls are thread-compatible per context (one context = one caller at a time).  Calls on different streams
+ *     of one context are ordered by the library (they share the context's workspaces).
  *   - Every function returns PHMM_OK (0) or a negative PHMM_E_* code; nothing throws or aborts.
  *     A call that fails argument validation writes nothing.
  */
@@ -73,13 +73,28 @@ typedef struct phmm_options {
      * haplotype through one lane group); 0 = chosen per batch between 1024 and 8192 so that the
      * GPU still gets several waves of warps */
     int32_t task_rows;
-    /* upper bound, in bytes, for the row-constant table of the short path (64 bytes per read base + 256 per
-     * read); a batch needing more fails with PHMM_E_NOMEM (split it).  Default 64 GiB. */
+    /* workspace budget, in bytes, of the row-constant table (64 bytes per read base + 256 per read).  A batch that
+     * needs more is processed in slices of reads inside the call (phmm_stats.n_slices), each with a table within the
+     * budget; PHMM_E_NOMEM only if a single read does not fit.  Default 4 GiB, minimum 4 MiB. */
     int64_t max_table_bytes;
     /* non-zero: bracket every kernel family of a call with CUDA events on the caller's stream; the
      * durations appear in phmm_stats.ms_* (phmm_get_stats synchronises the last event).  Default 0. */
     int32_t profile_events;
-    int32_t reserved0;
+    /* non-zero: before anything is launched, one device pass checks the payload's preconditions -- every base is one of
+     * A C G T N, every quality byte is >= qual_offset, and iota + delta < 1 on every read position -- and the call returns
+     * PHMM_E_ARG, having written nothing, if one is violated (it synchronises the stream once).  Default 0: the payload
+     * is trusted (SURVEY.md section 8(b) "Errors"). */
+    int32_t validate;
+    /* Compatibility semantics (none of them changes a config of
+     * BASELINE.json, all default to 0 = the literal reading of Eq.3 on raw Phred bytes):
+     *   qual_offset     subtracted from every quality byte before use (33 for FASTQ / ASCII-encoded qualities, PAPER.md:76
+     *                   "Q - 33"); bytes below it count as quality 0
+     *   min_base_qual   base qualities below this value (after the offset) are raised to it (a quality floor)
+     *   n_is_wildcard   non-zero: an N in the read or in the haplotype matches every base (prior 1 - eps), instead of
+     *                   matching only another N */
+    int32_t qual_offset;
+    int32_t min_base_qual;
+    int32_t n_is_wildcard;
 } phmm_options;
 
 /* One batch, CSR layout, natural order (a read, a haplotype and four
@@ -112,7 +127,7 @@ typedef struct phmm_stats {
     int64_t table_bytes;        /* row-constant table size of the call */
     double host_batch_ms;       /* host time spent in the batcher */
     int32_t n_short_warps;      /* warp tasks of the short kernel */
-    int32_t n_slices;
+    int32_t n_slices;           /* slices of reads the call was processed in (phmm_options.max_table_bytes) */
     /* device time per kernel family, milliseconds, CUDA events on the caller's stream; filled only
      * with phmm_options.profile_events (else 0).  ms_short is the sub-warp systolic fp32 kernel, ms_table
      * the row-constant prologue, ms_rescue the fp64 (rescue / PHMM_FP64 short) chain launch, ms_long
@@ -140,9 +155,9 @@ int phmm_forward_batch(phmm_ctx* ctx, const phmm_batch* b, int precision, double
 /* Same computation with ALL buffers on the host (the d_* members of `b` are host pointers, out
  * pointers are host): the library copies the payload to the device, runs phmm_forward_batch, copies
  * the results back and synchronises.  This is the end-to-end entry ("with transfer").
- * A large pair list whose consecutive chunks (>= 400 k pairs, at most 8) use disjoint haplotypes is enqueued chunk
- * by chunk, so that the host batcher of one chunk overlaps the device work of the previous one; results and
- * flags are the same as for one call.  phmm_get_stats afterwards reports the sums over the chunks. */
+ * The reads are processed in slices (at least one per 32 MB of read payload, and as many as the table budget asks for):
+ * the copy of a slice's reads and its host plan run under the kernels of the slice before; results and flags are the
+ * same as for one call with device buffers.  phmm_get_stats afterwards reports the sums over the slices. */
 int phmm_forward_batch_host(phmm_ctx* ctx, const phmm_batch* b, int precision, double* h_out_log10,
                             uint8_t* h_out_flags);
 

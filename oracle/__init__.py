@@ -50,6 +50,8 @@ def _load():
                                           _u8p, ctypes.c_double, ctypes.c_int, ctypes.c_int, _f64p]
         lib.phmm_oracle_batch.restype = ctypes.c_int
         lib.phmm_oracle_num_threads.restype = ctypes.c_int
+        lib.phmm_oracle_set_n_wildcard.argtypes = [ctypes.c_int]
+        lib.phmm_oracle_set_n_wildcard.restype = None
         _lib = lib
     return _lib
 
@@ -68,7 +70,8 @@ def num_threads() -> int:
     return int(_load().phmm_oracle_num_threads())
 
 
-def forward_pair(read, qb, qi, qd, qg, hap, log2C: float = 0.0, rescale: bool = True, matrices: bool = False):
+def forward_pair(read, qb, qi, qd, qg, hap, log2C: float = 0.0, rescale: bool = True, matrices: bool = False,
+                 n_wildcard: bool = False):
     """log10 L of one pair.  With ``matrices=True`` also returns (M, I, D, row_exp): arrays of shape
     (l+1, k+1) holding mantissas, true value = X[i] * 2**row_exp[i]."""
     lib = _load()
@@ -81,6 +84,7 @@ def forward_pair(read, qb, qi, qd, qg, hap, log2C: float = 0.0, rescale: bool = 
     out = np.zeros(1, dtype=np.float64)
     dump = np.zeros((3, l + 1, k + 1), dtype=np.float64) if matrices else None
     dexp = np.zeros(l + 1, dtype=np.int32) if matrices else None
+    lib.phmm_oracle_set_n_wildcard(int(bool(n_wildcard)))
     rc = lib.phmm_oracle_pair(_p(read, _u8p), _p(q[0], _u8p), _p(q[1], _u8p), _p(q[2], _u8p), _p(q[3], _u8p), l,
                               _p(hap, _u8p), k, float(log2C), int(bool(rescale)), _p(out, _f64p),
                               _p(dump, _f64p) if matrices else None, _p(dexp, _i32p) if matrices else None)
@@ -91,7 +95,8 @@ def forward_pair(read, qb, qi, qd, qg, hap, log2C: float = 0.0, rescale: bool = 
     return float(out[0])
 
 
-def forward_batch(batch, log2C: float = 0.0, rescale: bool = True, n_threads: int = 0, pairs=None) -> np.ndarray:
+def forward_batch(batch, log2C: float = 0.0, rescale: bool = True, n_threads: int = 0, pairs=None,
+                  n_wildcard: bool = False) -> np.ndarray:
     """log10 L for every pair of a workloads.Batch-like object (or for the pair indices ``pairs``)."""
     lib = _load()
     pr = np.ascontiguousarray(batch.pair_read if pairs is None else batch.pair_read[pairs], dtype=np.int32)
@@ -99,6 +104,7 @@ def forward_batch(batch, log2C: float = 0.0, rescale: bool = True, n_threads: in
     out = np.zeros(len(pr), dtype=np.float64)
     arrs = [np.ascontiguousarray(a) for a in (batch.read_off, batch.hap_off, batch.read_bases, batch.qual_base,
                                               batch.qual_ins, batch.qual_del, batch.qual_gcp, batch.hap_bases)]
+    lib.phmm_oracle_set_n_wildcard(int(bool(n_wildcard)))
     rc = lib.phmm_oracle_batch(len(pr), _p(pr, _i32p), _p(ph, _i32p), _p(arrs[0], _i64p), _p(arrs[1], _i64p),
                                _p(arrs[2], _u8p), _p(arrs[3], _u8p), _p(arrs[4], _u8p), _p(arrs[5], _u8p),
                                _p(arrs[6], _u8p), _p(arrs[7], _u8p), float(log2C), int(bool(rescale)),

@@ -36,8 +36,9 @@ def row_probs(qb, qi, qd, qg, exact=False):
     return rows
 
 
-def likelihood(read, hap, qb, qi, qd, qg, exact=False):
-    """L (not its log) by summing the weight of every alignment path."""
+def likelihood(read, hap, qb, qi, qd, qg, exact=False, n_wildcard=False):
+    """L (not its log) by summing the weight of every alignment path.  n_wildcard: an ``N`` in either sequence
+    matches anything (the compatibility switch of SURVEY 8(f) item 3; off by default = literal Eq.3)."""
     l, k = len(read), len(hap)
     read = read.encode() if isinstance(read, str) else bytes(read)
     hap = hap.encode() if isinstance(hap, str) else bytes(hap)
@@ -48,7 +49,8 @@ def likelihood(read, hap, qb, qi, qd, qg, exact=False):
 
     def emit(i, j):  # P(r_i | h_j), 1-based
         pm, px = rows[i - 1][0], rows[i - 1][1]
-        return pm if read[i - 1] == hap[j - 1] else px
+        a, c = read[i - 1], hap[j - 1]
+        return pm if (a == c or (n_wildcard and (a == 78 or c == 78))) else px
 
     def walk(state, i, j, w):
         """Sum of weights of all accepted completions of a path currently at (state,i,j) with weight w."""
@@ -78,5 +80,5 @@ def likelihood(read, hap, qb, qi, qd, qg, exact=False):
     return total
 
 
-def log10_likelihood(read, hap, qb, qi, qd, qg):
-    return math.log10(float(likelihood(read, hap, qb, qi, qd, qg)))
+def log10_likelihood(read, hap, qb, qi, qd, qg, n_wildcard=False):
+    return math.log10(float(likelihood(read, hap, qb, qi, qd, qg, n_wildcard=n_wildcard)))

@@ -30,7 +30,8 @@
  *       of the cell being written (gamma = 0.1 at GCP 10, the paper's constants).
  *       Non-uniform GCP is NOT pinned by the paper ("parity unpinned" for that case only).
  *   G8  the sum of Eq.4 runs over j = 1..k.
- *   G17 P(r_i|h_j) compares bytes literally.
+ *   G17 P(r_i|h_j) compares bytes literally.  n_wildcard != 0 (off in every BASELINE.json config; the GATK-style
+ *       compatibility switch of SURVEY.md section 8(f) item 3): an 'N' in either sequence matches anything.
  *
  * Pins (tests/test_oracle_pins.py, -m "not gpu"): brute-force path enumeration, closed forms
  * (1-base read, 1-base haplotype, gapless limit), the paper's first-row formula,
@@ -54,6 +55,9 @@
  * dump (optional, may be NULL): 3*(l+1)*(k+1) doubles, the matrices M, I, D (in that order, row
  * major, row 0 and column 0 included) holding mantissas; dump_exp (l+1 ints) the power-of-two
  * exponent of each row, so that true value = dump * 2^dump_exp[i] (all 0 when rescale == 0). */
+static int n_wildcard_flag = 0; /* set through phmm_oracle_set_n_wildcard; read-only while a batch runs */
+void phmm_oracle_set_n_wildcard(int on) { n_wildcard_flag = on ? 1 : 0; }
+
 int phmm_oracle_pair(const uint8_t* read, const uint8_t* qb, const uint8_t* qi, const uint8_t* qd,
                      const uint8_t* qg, int64_t l, const uint8_t* hap, int64_t k, double log2C, int rescale,
                      double* out_log10, double* dump, int32_t* dump_exp) {
@@ -86,7 +90,8 @@ int phmm_oracle_pair(const uint8_t* read, const uint8_t* qb, const uint8_t* qi, 
 
         Mc[0] = 0.0; Ic[0] = 0.0; Dc[0] = 0.0; /* Eq.1: column 0 is zero for i >= 1 */
         for (int64_t j = 1; j <= k; j++) {
-            const double p = (r == hap[j - 1]) ? p_match : p_mis;                      /* Eq.3 */
+            const int same = (r == hap[j - 1]) || (n_wildcard_flag && (r == 'N' || hap[j - 1] == 'N'));
+            const double p = same ? p_match : p_mis;                                   /* Eq.3 */
             Mc[j] = p * (T_MM * Mp[j - 1] + T_IM * Ip[j - 1] + T_DM * Dp[j - 1]);      /* Eq.2 */
             Ic[j] = T_MI * Mp[j] + T_II * Ip[j];                                        /* Eq.2 */
             Dc[j] = T_MD * Mc[j - 1] + T_DD * Dc[j - 1];                                /* Eq.2 */

@@ -29,7 +29,8 @@ class phmm_options(ctypes.Structure):
     _fields_ = [("size", ctypes.c_uint32), ("rescue_log2_threshold", ctypes.c_int32),
                 ("long_min_hap_len", ctypes.c_int32), ("task_rows", ctypes.c_int32),
                 ("max_table_bytes", ctypes.c_int64), ("profile_events", ctypes.c_int32),
-                ("reserved0", ctypes.c_int32)]
+                ("validate", ctypes.c_int32), ("qual_offset", ctypes.c_int32), ("min_base_qual", ctypes.c_int32),
+                ("n_is_wildcard", ctypes.c_int32)]
 
 
 class phmm_batch(ctypes.Structure):

@@ -145,9 +145,15 @@ extern "C" int phmm_create(phmm_ctx** out, int device, const phmm_options* opt) 
             cudaEventCreateWithFlags(&ctx->cset[i].ev_free, cudaEventDisableTiming) != cudaSuccess ||
             cudaEventCreateWithFlags(&ctx->cset[i].ev_up, cudaEventDisableTiming) != cudaSuccess) { phmm_destroy(ctx); return PHMM_E_CUDA; }
     if (cudaStreamCreateWithFlags(&ctx->copy_stream, cudaStreamNonBlocking) != cudaSuccess) { phmm_destroy(ctx); return PHMM_E_CUDA; }
-    // 10^(-q/10) for q = 0..255, the paper's "q64" table
-    double lut[256];
-    for (int q = 0; q < 256; q++) lut[q] = pow(10.0, -(double)q / 10.0);
+    // 10^(-q/10) for every quality byte, the paper's "q64" table: [0..255] for insertion, deletion and
+    // continuation qualities, [256..511] for base qualities (with the optional floor), both after the optional offset
+    if (ctx->opt.qual_offset < 0 || ctx->opt.qual_offset > 255 || ctx->opt.min_base_qual < 0) { phmm_destroy(ctx); return PHMM_E_ARG; }
+    double lut[512];
+    for (int q = 0; q < 256; q++) {
+        const int v = std::max(0, q - ctx->opt.qual_offset);
+        lut[q] = pow(10.0, -(double)v / 10.0);
+        lut[256 + q] = pow(10.0, -(double)std::max(v, ctx->opt.min_base_qual) / 10.0);
+    }
     if (ctx->d_lut.need(sizeof(lut)) != cudaSuccess || cudaMemcpy(ctx->d_lut.p, lut, sizeof(lut), cudaMemcpyHostToDevice) != cudaSuccess) {
         phmm_destroy(ctx);
         return PHMM_E_CUDA;
@@ -291,6 +297,22 @@ struct SliceWork {  // one slice of reads [r0, r1) of a call and the pairs that 
 
 static int run_slice(phmm_ctx* ctx, const phmm_batch* b, const HostBatchView& hv, bool fp64, double* d_out, uint8_t* d_flags,
                      cudaStream_t st, const phmm_ctx::CallSet& cs, SliceWork& sw, const HostPayload* hp);
+
+// phmm_options.validate: one device pass over the payload (device pointers in `b`), then a synchronisation
+static int validate_payload(phmm_ctx* ctx, const phmm_batch* b, cudaStream_t st) {
+    DevBatch db;
+    memset(&db, 0, sizeof(db));
+    db.read_bases = b->d_read_bases; db.qual_base = b->d_qual_base; db.qual_ins = b->d_qual_ins;
+    db.qual_del = b->d_qual_del; db.qual_gcp = b->d_qual_gcp; db.hap_bases = b->d_hap_bases;
+    CK(ctx->d_acc.need(16));
+    CK(cudaMemsetAsync(ctx->d_acc.p, 0, 16, st));
+    CK(launch_validate(db, (const double*)ctx->d_lut.p, b->h_read_off[0], b->h_read_off[b->n_reads], b->h_hap_off[0],
+                       b->h_hap_off[b->n_haps], ctx->opt.qual_offset, (int*)ctx->d_acc.p, st));
+    int err = 0;
+    CK(cudaMemcpyAsync(&err, ctx->d_acc.p, sizeof(int), cudaMemcpyDeviceToHost, st));
+    CK(cudaStreamSynchronize(st));
+    return err ? PHMM_E_ARG : PHMM_OK;
+}
 
 // The whole call: validation, classification, the global haplotype-major order of the short pairs, the cut into slices of
 // reads (so that the row-constant table of a slice fits the workspace budget), then slice after slice: host plan, uploads
@@ -518,6 +540,7 @@ static int run_slice(phmm_ctx* ctx, const phmm_batch* b, const HostBatchView& hv
     db.read_off = (const int64_t*)cs.d_read_off.p; db.hap_off = (const int64_t*)cs.d_hap_off.p;
     db.n_reads = b->n_reads; db.n_haps = b->n_haps;
     db.table_base = sw.table_base;
+    db.n_wild = ctx->opt.n_is_wildcard ? 1 : 0;
     const int* d_pair_read = (const int*)cs.d_pair_read.p;
     const int* d_pair_hap = (const int*)cs.d_pair_hap.p;
     int* counters = (int*)ctx->d_counters.p;
@@ -692,6 +715,10 @@ extern "C" int phmm_forward_batch(phmm_ctx* ctx, const phmm_batch* b, int precis
     RC(validate_batch(hv));
     DeviceGuard guard(ctx->device);
     if (!guard.ok) return PHMM_E_CUDA;
+    if (ctx->opt.validate) {
+        CK(cudaStreamWaitEvent((cudaStream_t)cuda_stream, ctx->ev_last, 0));
+        RC(validate_payload(ctx, b, (cudaStream_t)cuda_stream));
+    }
     return forward_impl(ctx, b, precision, d_out, d_flags, (cudaStream_t)cuda_stream, nullptr, 1);
 }
 
@@ -734,7 +761,15 @@ extern "C" int phmm_forward_batch_host(phmm_ctx* ctx, const phmm_batch* b, int p
     // host plan run while the GPU works on slice s (the "with transfers" convention).
     const int min_slices = (int)std::max<size_t>(1, std::min<size_t>(16, 5 * R / ((size_t)32 << 20)));
     const int64_t np = b->n_pairs;
-    int rc = forward_impl(ctx, &db, precision, (double*)ctx->d_out.p, (uint8_t*)ctx->d_flags.p, st, &hp, min_slices);
+    const HostPayload* hpp = &hp;
+    if (ctx->opt.validate) {  // the whole payload first, then the check: nothing may be written for a bad batch
+        CK(cudaStreamWaitEvent(st, ctx->ev_last, 0));
+        for (int i = 0; i < 5; i++) CK(cudaMemcpyAsync(base + i * Ra, src[i], R, cudaMemcpyHostToDevice, ctx->copy_stream));
+        CK(cudaStreamSynchronize(ctx->copy_stream));
+        RC(validate_payload(ctx, &db, st));
+        hpp = nullptr;
+    }
+    int rc = forward_impl(ctx, &db, precision, (double*)ctx->d_out.p, (uint8_t*)ctx->d_flags.p, st, hpp, min_slices);
     if (rc != PHMM_OK) { cudaStreamSynchronize(st); return rc; }
     std::vector<uint8_t> tmp_flags;
     uint8_t* fl = h_flags;

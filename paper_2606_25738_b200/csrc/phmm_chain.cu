@@ -192,7 +192,7 @@ k_chain(DevBatch b, ChainLaunch p, int items_are_pairs) {
 
             L ln;
             ln.init();
-            ln.load_hap(b.hap_bases + ho, k, (st * 32 + lane) * N2);
+            ln.load_hap(b.hap_bases + ho, k, (st * 32 + lane) * N2, b.n_wild != 0);
             int ex = 0;        // true value = stored value * 2^ex, one exponent per thread
             bool zero = true;  // this thread holds nothing but zeros
             __syncwarp();

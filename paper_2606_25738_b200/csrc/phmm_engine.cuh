@@ -81,7 +81,8 @@ template <typename T, int NV, bool HS = false> struct Lane2 {
     }
 
     // hap: pointer to the haplotype bytes, k its length, j0 = 0-based first column of this thread
-    __device__ __forceinline__ void load_hap(const uint8_t* __restrict__ hap, int k, int j0) {
+    // wild (match words only; the fp16 codes of HS cannot express it): a haplotype N matches every read base
+    __device__ __forceinline__ void load_hap(const uint8_t* __restrict__ hap, int k, int j0, bool wild = false) {
         if constexpr (HS) {
 #pragma unroll
             for (int x = 0; x < NV; x++) {
@@ -99,12 +100,12 @@ template <typename T, int NV, bool HS = false> struct Lane2 {
                 if (x < nvx) {
                     const int c = base_code(hap[j0 + x]);
 #pragma unroll
-                    for (int q = 0; q < 5; q++) hm[q] |= (c == q ? 1u : 0u) << x;
+                    for (int q = 0; q < 5; q++) hm[q] |= ((c == q || (wild && c == 4)) ? 1u : 0u) << x;
                 }
                 if (x < nvy) {
                     const int c = base_code(hap[j0 + NV + x]);
 #pragma unroll
-                    for (int q = 0; q < 5; q++) hm[q] |= (c == q ? 1u : 0u) << (16 + x);
+                    for (int q = 0; q < 5; q++) hm[q] |= ((c == q || (wild && c == 4)) ? 1u : 0u) << (16 + x);
                 }
             }
             uint32_t v = 0;  // what "matches" the sum entry: columns more than one behind the haplotype's last

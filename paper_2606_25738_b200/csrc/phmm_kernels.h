@@ -31,6 +31,7 @@ struct DevBatch {  // device mirrors of the batch
     const uint8_t *read_bases, *qual_base, *qual_ins, *qual_del, *qual_gcp, *hap_bases;
     const int64_t *read_off, *hap_off;  // device copies of the host offset arrays
     int64_t n_reads, n_haps;
+    int n_wild;          // phmm_options.n_is_wildcard: an N (read or haplotype) matches every base
     int64_t table_base;  // absolute table position (table_run_start) of the zero run of the table in use: a slice of reads has its own
 };
 
@@ -157,6 +158,8 @@ int rescue_ctas_per_sm();
 
 cudaError_t launch_lut_table(const DevBatch& b, const double* lut, float* table, int64_t r0, int64_t r1, int max_read_len, cudaStream_t st);
 cudaError_t launch_short_f32(const DevBatch& b, const ShortLaunch& p, cudaStream_t st);
+// debug pass (phmm_options.validate): *d_err |= 1 bad base, 2 quality below the offset, 4 iota + delta >= 1
+cudaError_t launch_validate(const DevBatch& b, const double* lut, int64_t read_lo, int64_t read_hi, int64_t hap_lo, int64_t hap_hi, int qual_offset, int* d_err, cudaStream_t st);
 // rescue_from_list: items are taken from p.items[...] as plain pair indices in `rescue_list` form
 cudaError_t launch_chain(const DevBatch& b, const ChainLaunch& p, bool fp64, bool items_are_pairs, int grid_ctas,
                          cudaStream_t st);

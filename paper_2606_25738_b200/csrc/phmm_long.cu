@@ -89,9 +89,9 @@ struct LongSmem {
     float2 fin[32];           // per lane: its share of Eq.4 and the exponent it is stored at
 };
 
-template <int NV>
+template <int NV, bool HS>  // HS = false only under phmm_options.n_is_wildcard (phmm_short.cu)
 __global__ void __launch_bounds__(LONG_WPC * 32, LONG_MIN_CTAS) k_long_f32(DevBatch b, LongLaunch p) {
-    typedef Lane2<float, NV, true> L;
+    typedef Lane2<float, NV, HS> L;
     constexpr int N2 = 2 * NV;
     constexpr int STRIP = 32 * N2;
     __shared__ __align__(128) LongSmem sm_all[LONG_WPC];
@@ -124,7 +124,7 @@ __global__ void __launch_bounds__(LONG_WPC * 32, LONG_MIN_CTAS) k_long_f32(DevBa
 
         L ln;
         ln.init();
-        ln.load_hap(b.hap_bases + ho, k, (strip * 32 + lane) * N2);
+        ln.load_hap(b.hap_bases + ho, k, (strip * 32 + lane) * N2, b.n_wild != 0);
         int ex = 0;            // true value = stored value * 2^ex
         float f_in = 1.f;      // 2^(ex of the left neighbour - ex)
         int seen = 0;          // entries the producer strip is known to have published
@@ -351,13 +351,14 @@ __global__ void __launch_bounds__(LONG_WPC * 32, LONG_MIN_CTAS) k_long_f32(DevBa
 
 cudaError_t launch_long_f32(const DevBatch& b, const LongLaunch& p, int grid_ctas, cudaStream_t st) {
     if (grid_ctas <= 0) return cudaSuccess;
-    k_long_f32<SHORT_NV><<<grid_ctas, LONG_WPC * 32, 0, st>>>(b, p);
+    if (b.n_wild) k_long_f32<SHORT_NV, false><<<grid_ctas, LONG_WPC * 32, 0, st>>>(b, p);
+    else k_long_f32<SHORT_NV, true><<<grid_ctas, LONG_WPC * 32, 0, st>>>(b, p);
     return cudaGetLastError();
 }
 
 int long_ctas_per_sm() {
     int n = 0;
-    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, k_long_f32<SHORT_NV>, LONG_WPC * 32, 0);
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, k_long_f32<SHORT_NV, true>, LONG_WPC * 32, 0);
     return n > 0 ? n : 1;
 }
 int long_warps_per_cta() { return LONG_WPC; }

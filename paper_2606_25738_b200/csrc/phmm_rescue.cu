@@ -104,9 +104,9 @@ struct RescueArgs {
 
 __global__ void __launch_bounds__(RESCUE_WARPS * 32, RESCUE_MIN_CTAS) k_rescue_f64(DevBatch b, RescueArgs p) {
     constexpr int NV = RESCUE_NV;
-    __shared__ double s_lut[256];
+    __shared__ double s_lut[512];  // [0..255] gap qualities, [256..511] base qualities (phmm_rowconst.cuh)
     __shared__ int s_plan[68];
-    for (int i = threadIdx.x; i < 256; i += blockDim.x) s_lut[i] = p.lut[i];
+    for (int i = threadIdx.x; i < 512; i += blockDim.x) s_lut[i] = p.lut[i];
     for (int i = threadIdx.x; i < 68; i += blockDim.x) s_plan[i] = p.plan[i];
     __syncthreads();
     const int lane = threadIdx.x & 31;
@@ -143,7 +143,7 @@ __global__ void __launch_bounds__(RESCUE_WARPS * 32, RESCUE_MIN_CTAS) k_rescue_f
         for (int x = 0; x < nv; x++) {
             const int c = base_code(b.hap_bases[ho + j0 + x]);
 #pragma unroll
-            for (int q = 0; q < 5; q++) hm[q] |= (c == q ? 1u : 0u) << x;
+            for (int q = 0; q < 5; q++) hm[q] |= ((c == q || (b.n_wild && c == 4)) ? 1u : 0u) << x;
         }
         const double Cok = ldexp(1.0, RESCUE_LOG2C) / (double)k;
 
@@ -162,10 +162,11 @@ __global__ void __launch_bounds__(RESCUE_WARPS * 32, RESCUE_MIN_CTAS) k_rescue_f
             if (on) {
                 gam = gam_own;
                 if (e >= 1) {
-                    const double eps = s_lut[b.qual_base[ro + e - 1]];
+                    const double eps = s_lut[256 + b.qual_base[ro + e - 1]];
                     const int code = base_code(b.read_bases[ro + e - 1]);
                     px = eps * (1.0 / 3.0);  // within 1 ulp of Eq.3's eps/3; a double division per step would cost ~10 % here
                     pm = 1.0 - eps;
+                    if (b.n_wild && code == 4) px = pm;  // n_is_wildcard: a read N matches every column
                     const uint32_t m01 = (code & 1) ? hm[1] : hm[0], m23 = (code & 1) ? hm[3] : hm[2];
                     mw = (code & 4) ? hm[4] : (code & 2) ? m23 : m01;
                 }
@@ -274,7 +275,7 @@ __global__ void __launch_bounds__(RESCUE_WARPS * 32, RESCUE_MIN_CTAS) k_rescue_f
         for (int x = 0; x < nv; x++) {
             const int c = base_code(b.hap_bases[ho + j0 + x]);
 #pragma unroll
-            for (int q = 0; q < 5; q++) hm[q] |= (c == q ? 1u : 0u) << x;
+            for (int q = 0; q < 5; q++) hm[q] |= ((c == q || (b.n_wild && c == 4)) ? 1u : 0u) << x;
         }
 #pragma unroll
         for (int x = 0; x < NV; x++) hm[5] |= (j0 + x > k ? 1u : 0u) << x;

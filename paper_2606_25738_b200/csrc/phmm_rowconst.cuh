@@ -13,7 +13,8 @@
 // leaves T[x+1] = M_{l,x} + I_{l,x};  e = l+1 is the SUM entry (gamma := 1, pm := 0, px := 1, base code 0, all else 0):
 // U = T on every column with a non-zero code, so the chain s = s + U leaves Eq.4's sum in the group's last lane;
 // e = l+2 is the all-zero flush entry, which clears the J = U the sum entry left behind.
-// Constants are formed in double from the 10^(-q/10) table and rounded once to the working type
+// Constants are formed in double from the 10^(-q/10) tables (lut[0..255]: insertion, deletion and continuation
+// qualities; lut[256..511]: base qualities, with phmm_options.min_base_qual applied; both after qual_offset) and rounded once to the working type
 // ("q32"/"q64" tables; Listing 2 :293-295 for which qualities enter which transition).
 #pragma once
 #include "phmm_common.cuh"
@@ -34,7 +35,7 @@ __device__ __forceinline__ RowC row_constants(const DevBatch& b, const double* _
         c.gam = 1.0; c.C = 1.0 - lut[b.qual_gcp[off]]; c.meta = META_FIRST;
     } else if (e >= 1 && e <= l) {
         const int i = e;  // read row, 1-based
-        const double eps = lut[b.qual_base[off + i - 1]];
+        const double eps = lut[256 + b.qual_base[off + i - 1]];  // (the base-quality table carries the quality floor)
         const int code = base_code(b.read_bases[off + i - 1]);
         c.meta = (uint32_t)code | META_ROW | (i == l ? META_LAST : 0u);
         c.gam = lut[b.qual_gcp[off + i - 1]];
@@ -54,6 +55,7 @@ __device__ __forceinline__ RowC row_constants(const DevBatch& b, const double* _
         }
         c.pm = (1.0 - eps) * gin;  // (an N row matches N columns only: literal Eq.3, reading G17)
         c.px = eps / 3.0 * gin;
+        if (b.n_wild && code == 4) c.px = c.pm;  // phmm_options.n_is_wildcard: a read N matches every column
     }
     return c;
 }

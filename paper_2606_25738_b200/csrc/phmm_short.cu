@@ -77,9 +77,11 @@ struct Cursor {
     int q;               // reads of the task already handed to (npos, nend)
 };
 
-template <int NV>
+// HS = false (match words instead of fp16 column codes) only under phmm_options.n_is_wildcard, where a haplotype N has to
+// match every read base -- something one fp16 equality cannot say
+template <int NV, bool HS>
 __global__ void __launch_bounds__(SHORT_WARPS_PER_CTA * 32, SHORT_MIN_CTAS) k_short_f32(DevBatch b, ShortLaunch p) {
-    typedef Lane2<float, NV, true> L;  // HSETP2 predicates (2.78 vs 2.60 TCUPS with bit tests), Eq.4 through the s chain
+    typedef Lane2<float, NV, HS> L;  // HSETP2 predicates (2.78 vs 2.60 TCUPS with bit tests), Eq.4 through the s chain
     constexpr int N2 = 2 * NV;
     const int warp = blockIdx.x * SHORT_WARPS_PER_CTA + (threadIdx.x >> 5);
     if (warp >= p.n_warps) return;
@@ -126,7 +128,7 @@ __global__ void __launch_bounds__(SHORT_WARPS_PER_CTA * 32, SHORT_MIN_CTAS) k_sh
 
     L ln;
     ln.init();
-    ln.load_hap(b.hap_bases + (ti < 0 ? 0 : b.hap_off[m_hap]), m_k, lg * N2);
+    ln.load_hap(b.hap_bases + (ti < 0 ? 0 : b.hap_off[m_hap]), m_k, lg * N2, b.n_wild != 0);
     const float Cok = (float)(ldexp(1.0, 120) / (double)(m_k > 0 ? m_k : 1));  // Eq.1: C/k with C = 2^120
 
     const float4* tab = reinterpret_cast<const float4*>(p.table);
@@ -224,7 +226,31 @@ __global__ void __launch_bounds__(SHORT_WARPS_PER_CTA * 32, SHORT_MIN_CTAS) k_sh
 cudaError_t launch_short_f32(const DevBatch& b, const ShortLaunch& p, cudaStream_t st) {
     if (p.n_warps == 0) return cudaSuccess;
     const int grid = (p.n_warps + SHORT_WARPS_PER_CTA - 1) / SHORT_WARPS_PER_CTA;
-    k_short_f32<SHORT_NV><<<grid, SHORT_WARPS_PER_CTA * 32, 0, st>>>(b, p);
+    if (b.n_wild) k_short_f32<SHORT_NV, false><<<grid, SHORT_WARPS_PER_CTA * 32, 0, st>>>(b, p);
+    else k_short_f32<SHORT_NV, true><<<grid, SHORT_WARPS_PER_CTA * 32, 0, st>>>(b, p);
+    return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------ debug pass: preconditions of the payload
+__global__ void k_validate(DevBatch b, const double* __restrict__ lut, int64_t read_lo, int64_t read_hi, int64_t hap_lo, int64_t hap_hi,
+                           int qual_offset, int* err) {
+    int bad = 0;
+    const int64_t stride = (int64_t)gridDim.x * blockDim.x, i0 = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    auto base_ok = [](uint8_t c) { return c == 'A' || c == 'C' || c == 'G' || c == 'T' || c == 'N'; };
+    for (int64_t i = read_lo + i0; i < read_hi; i += stride) {
+        if (!base_ok(b.read_bases[i])) bad |= 1;
+        const int qb = b.qual_base[i], qi = b.qual_ins[i], qd = b.qual_del[i], qg = b.qual_gcp[i];
+        if (qb < qual_offset || qi < qual_offset || qd < qual_offset || qg < qual_offset) bad |= 2;
+        if (!(lut[qi] + lut[qd] < 1.0)) bad |= 4;  // T_MM = 1 - iota - delta must stay positive (reading G18)
+    }
+    for (int64_t i = hap_lo + i0; i < hap_hi; i += stride)
+        if (!base_ok(b.hap_bases[i])) bad |= 1;
+    if (bad) atomicOr(err, bad);
+}
+
+cudaError_t launch_validate(const DevBatch& b, const double* lut, int64_t read_lo, int64_t read_hi, int64_t hap_lo, int64_t hap_hi,
+                            int qual_offset, int* d_err, cudaStream_t st) {
+    k_validate<<<592, 256, 0, st>>>(b, lut, read_lo, read_hi, hap_lo, hap_hi, qual_offset, d_err);
     return cudaGetLastError();
 }
 

@@ -366,6 +366,101 @@ def test_n_bases_literal_equality(B, ctx):
     assert abs(ox[0] - ref[0]) <= TOL64 and abs(ox[1] - ref[0]) <= TOL64
 
 
+def _options_batch(rng, with_n):
+    """Pairs through every kernel family: short related / unrelated (fp32 + rescue), haplotype > 1024 (long path)."""
+    cases = []
+    for k, l in ((60, 30), (300, 120), (700, 250), (1500, 400), (2500, 700)):
+        hap = list(_rand_seq(rng, k))
+        if with_n:
+            for i in rng.choice(k, max(1, k // 25), replace=False):
+                hap[i] = "N"
+        hap = "".join(hap)
+        for rel in (True, True, False):
+            s0 = int(rng.integers(0, k - l))
+            rd = list(hap[s0:s0 + l]) if rel else list(_rand_seq(rng, l))
+            for i in rng.choice(l, max(1, l // 20), replace=False):
+                rd[i] = "N" if with_n else "ACGT"[int(rng.integers(0, 4))]
+            cases.append(("".join(rd), hap, list(rng.integers(2, 41, l)), list(rng.integers(12, 50, l)), list(rng.integers(12, 50, l)),
+                          list(rng.integers(8, 30, l))))
+    return cases
+
+
+def test_option_n_is_wildcard(B):
+    """phmm_options.n_is_wildcard: an N on either side matches every base -- the same switch in the oracle
+    (pinned by the path enumeration, tests/test_oracle_pins.py); all kernel families, both precisions."""
+    rng = np.random.default_rng(41)
+    b = W.from_strings(_options_batch(rng, True))
+    ref_w = oracle.forward_batch(b, n_wildcard=True)
+    ref_l = oracle.forward_batch(b)
+    assert np.max(ref_w - ref_l) > 1.0  # the switch matters on these inputs
+    c = B.Context(0, n_is_wildcard=1)
+    try:
+        out, fl = run(B, c, b, B.PHMM_FP32_RESCUE)
+        assert np.max(np.abs(out - ref_w)) <= TOL32
+        out64, _ = run(B, c, b, B.PHMM_FP64)
+        assert np.max(np.abs(out64 - ref_w)) <= TOL64
+    finally:
+        c.close()
+
+
+def test_options_qual_offset_and_floor(B):
+    """phmm_options.qual_offset (ASCII+33 qualities) and min_base_qual (a floor on the base quality): the
+    library on encoded bytes == the oracle on the decoded / floored Phred values."""
+    rng = np.random.default_rng(42)
+    cases = _options_batch(rng, False)
+    plain = W.from_strings(cases)
+    floor = 10
+    dec = W.from_strings([(r, h, np.maximum(np.asarray(qb), floor), qi, qd, qg) for r, h, qb, qi, qd, qg in cases])
+    enc = W.from_strings([(r, h, np.asarray(qb) + 33, np.asarray(qi) + 33, np.asarray(qd) + 33, np.asarray(qg) + 33)
+                          for r, h, qb, qi, qd, qg in cases])
+    ref = oracle.forward_batch(dec)
+    assert np.max(np.abs(ref - oracle.forward_batch(plain))) > 1e-3  # the floor matters on these inputs
+    c = B.Context(0, qual_offset=33, min_base_qual=floor)
+    try:
+        out, fl = run(B, c, enc, B.PHMM_FP32_RESCUE)
+        assert np.max(np.abs(out - ref)) <= TOL32
+        out64, _ = run(B, c, enc, B.PHMM_FP64)
+        assert np.max(np.abs(out64 - ref)) <= TOL64
+    finally:
+        c.close()
+
+
+def test_option_validate_rejects_bad_payloads(B):
+    """phmm_options.validate: a byte outside ACGTN, a quality below the offset, or iota + delta >= 1 make the call return
+    PHMM_E_ARG before anything is launched: outputs untouched.  A clean batch passes and gives the usual result."""
+    import torch
+    rng = np.random.default_rng(43)
+    good = W.from_strings(_options_batch(rng, True))
+    c = B.Context(0, validate=1)
+    try:
+        out, fl, ref = check(B, c, good, B.PHMM_FP32_RESCUE)
+        oh, fh = c.forward_batch_host(good, B.PHMM_FP32_RESCUE)
+        assert np.array_equal(oh, out)
+        bad_base = W.from_strings([("ACGT", "ACGTAC"), ("ACXT", "ACGTAC")])
+        bad_hap = W.from_strings([("ACGT", "AC*TAC")])
+        bad_gap = W.from_strings([("ACGT", "ACGTAC", 30, 2, 2, 10)])  # iota + delta = 1.26
+        for bad in (bad_base, bad_hap, bad_gap):
+            sentinel = torch.full((bad.n_pairs,), 7.0, dtype=torch.float64, device="cuda:0")
+            with pytest.raises(B.PhmmError) as ei:
+                c.forward_batch(B.DeviceBatch(bad), B.PHMM_FP32_RESCUE, out=sentinel)
+            assert ei.value.code == B.PHMM_E_ARG
+            torch.cuda.synchronize()
+            assert torch.all(sentinel == 7.0)
+            with pytest.raises(B.PhmmError) as ei:
+                c.forward_batch_host(bad, B.PHMM_FP64)
+            assert ei.value.code == B.PHMM_E_ARG
+    finally:
+        c.close()
+    c2 = B.Context(0, validate=1, qual_offset=33)
+    try:
+        low = W.from_strings([("ACGT", "ACGTAC", 20, 45, 45, 10)])  # raw bytes below the offset of 33
+        with pytest.raises(B.PhmmError) as ei:
+            c2.forward_batch(B.DeviceBatch(low), B.PHMM_FP32_RESCUE)
+        assert ei.value.code == B.PHMM_E_ARG
+    finally:
+        c2.close()
+
+
 def test_few_reads_on_a_fresh_context_with_dirty_memory(B):
     """The zero run at the start of the row-constant table (what idle lanes walk before their stream starts) must be
     cleared whatever the batch size: 1-4 reads against haplotypes of more than 32 bases on a NEW context whose device

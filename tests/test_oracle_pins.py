@@ -42,6 +42,36 @@ def test_bruteforce_all_small_shapes():
     assert worst < 1e-12, worst
 
 
+def test_bruteforce_n_bases_literal_and_wildcard():
+    """Reading G17: Eq.3 compares bytes, so an N matches an N only; with the compatibility switch n_wildcard (SURVEY 8(f)
+    item 3, off in every config) an N in either sequence matches anything.  Both against the path enumeration, which
+    implements the two rules in its own emit()."""
+    rng = np.random.default_rng(17)
+    worst = 0.0
+    differ = 0
+    for l in range(1, 5):
+        for k in range(1, 7):
+            for rep in range(4):
+                read, hap, qb, qi, qd, qg = _rand_case(rng, l, k, uniform_gcp=(rep % 2 == 0))
+                read, hap = list(read), list(hap)
+                read[int(rng.integers(0, l))] = "N"
+                if rep >= 2:
+                    hap[int(rng.integers(0, k))] = "N"
+                read, hap = "".join(read), "".join(hap)
+                vals = []
+                for wild in (False, True):
+                    got = oracle.forward_pair(read, qb, qi, qd, qg, hap, n_wildcard=wild)
+                    want = bruteforce.log10_likelihood(read, hap, qb, qi, qd, qg, n_wildcard=wild)
+                    worst = max(worst, abs(got - want))
+                    vals.append(got)
+                assert vals[1] >= vals[0] - 1e-12  # a wildcard can only add matches
+                differ += vals[1] > vals[0] + 1e-9
+    assert worst < 1e-12, worst
+    assert differ > 50
+    assert oracle.forward_pair("N", 30, 45, 45, 10, "N") == oracle.forward_pair("A", 30, 45, 45, 10, "A")  # literal N == N
+    assert oracle.forward_pair("N", 30, 45, 45, 10, "A") < oracle.forward_pair("N", 30, 45, 45, 10, "A", n_wildcard=True)
+
+
 def test_golden_exact_values():
     """tests/golden/tiny_exact.json: exact rational path sums (written by make_golden.py from oracle/bruteforce)."""
     path = os.path.join(os.path.dirname(__file__), "golden", "tiny_exact.json")
