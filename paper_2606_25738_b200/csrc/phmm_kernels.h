@@ -6,7 +6,10 @@
 
 namespace phmm {
 
-constexpr int SHORT_NV = 16;              // columns per virtual lane, fp32 short kernel
+#ifndef SHORT_NV_
+#define SHORT_NV_ 16  // (8 for the columns-per-thread sweep of profiles/r2_gn_sweep.md)
+#endif
+constexpr int SHORT_NV = SHORT_NV_;        // columns per virtual lane, fp32 short and long kernels
 constexpr int SHORT_N2 = 2 * SHORT_NV;    // columns per CUDA lane
 constexpr int SHORT_MAX_K = 32 * SHORT_N2;  // 1024: widest haplotype one warp covers
 constexpr int CHAIN_NV_F32 = 16;

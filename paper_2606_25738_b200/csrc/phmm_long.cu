@@ -84,6 +84,7 @@ __device__ __forceinline__ float scale2(float v, int d) {
 // float4 of an entry) at c * 2048, the odd entries 1024 bytes behind the even ones, entry pos at ((pos >> 1) & 63) * 16.
 struct LongSmem {
     float4 ring[4 * 128];
+    float4 rraw[LONG_EVERY];  // the boundary records of the NEXT event, copied in (cp.async) during the steps before it
     float2 rin[LONG_EVERY];   // boundary values lane 0 consumes in the next 16 steps, already at its exponent
     float2 rout[LONG_EVERY];  // what lane 31 handed out in the last 16 steps (flushed to the records at the next event)
     float2 fin[32];           // per lane: its share of Eq.4 and the exponent it is stored at
@@ -128,6 +129,7 @@ __global__ void __launch_bounds__(LONG_WPC * 32, LONG_MIN_CTAS) k_long_f32(DevBa
         int ex = 0;            // true value = stored value * 2^ex
         float f_in = 1.f;      // 2^(ex of the left neighbour - ex)
         int seen = 0;          // entries the producer strip is known to have published
+        int pre = -1;          // first entry of the boundary records that are on their way into sm.rraw (-1: none)
         sm.fin[lane] = make_float2(0.f, 0.f);
 
         // ---- fetch.  The table blocks live in the ring, filled by cp.async one block (32 steps) ahead of lane 0: the step
@@ -194,7 +196,22 @@ __global__ void __launch_bounds__(LONG_WPC * 32, LONG_MIN_CTAS) k_long_f32(DevBa
                     while (q < need) { __nanosleep(100); q = ld_relaxed_gpu(inprog); }
                     seen = q;
                 }
-                if (lane < LONG_EVERY && s + lane < n_ent) rec = ld_strong_f4(p.records + it.buf0 + (int64_t)(strip - 1) * n_ent + s + lane);
+                const float4* src = p.records + it.buf0 + (int64_t)(strip - 1) * n_ent;
+                if (pre == s) {  // copied in during the last 16 steps
+                    asm volatile("cp.async.wait_group 0;" ::: "memory");
+                    if (lane < LONG_EVERY && s + lane < n_ent) rec = sm.rraw[lane];
+                } else if (lane < LONG_EVERY && s + lane < n_ent) {
+                    rec = ld_strong_f4(src + s + lane);
+                }
+                // the records of the next event, if the producer has them already (it usually has): no L2 round trip then
+                const int s2 = s + LONG_EVERY;
+                pre = -1;
+                if (s2 < n_ent && seen >= min(s2 + LONG_EVERY, n_ent)) {
+                    if (lane < LONG_EVERY && s2 + lane < n_ent)
+                        asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"((uint32_t)__cvta_generic_to_shared(&sm.rraw[lane])), "l"(src + s2 + lane) : "memory");
+                    asm volatile("cp.async.commit_group;" ::: "memory");
+                    pre = s2;
+                }
             }
             // 2. own proposal (none for a lane that holds nothing)
             float m = fmax3(ln.outS.x, ln.outS.y, fmaxf(ln.outT.x, ln.outT.y));
@@ -292,10 +309,13 @@ __global__ void __launch_bounds__(LONG_WPC * 32, LONG_MIN_CTAS) k_long_f32(DevBa
         // lane 31's .y half finishes entry run_len - 1 >= n_ent - 1 at step run_len + 62; a multiple of 16 steps
         const int steps = (run_len + 64 + 15) & ~15;
         for (int s = 0; s < steps; s += 2) {
-            if ((s & (LONG_EVERY - 1)) == 0) event(s, false);
-            if (((run0 + s + 2) & 31) == 0) {  // lane 0's next fetch enters a new block (now complete): the one after it starts its way in
-                fill_wait();
-                fill(((run0 + s + 2) >> 5) + 1);
+            const bool ev = (s & (LONG_EVERY - 1)) == 0, fl = ((run0 + s + 2) & 31) == 0;
+            if (ev | fl) {  // (one branch per two steps)
+                if (ev) event(s, false);
+                if (fl) {  // lane 0's next fetch enters a new block (now complete): the one after it starts its way in
+                    fill_wait();
+                    fill(((run0 + s + 2) >> 5) + 1);
+                }
             }
             const uint32_t slot = rin_s + ((s & (LONG_EVERY - 2)) << 3);
             fetch_odd(eB);

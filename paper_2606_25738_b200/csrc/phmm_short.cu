@@ -13,6 +13,9 @@
 #ifndef SHORT_L2_PREFETCH
 #define SHORT_L2_PREFETCH 1  // table loads carry the L2 256-byte prefetch hint: +0.6 %
 #endif
+#ifndef SHORT_L2_LINE_PREFETCH
+#define SHORT_L2_LINE_PREFETCH 0  // entries ahead (0 = off)
+#endif
 #ifndef SHORT_MIN_CTAS
 #define SHORT_MIN_CTAS 3  // resident CTAs per SM the register allocation is held to (3 x 128 threads -> <= 168 registers); 4 x 128 registers spills: 3.17 vs 3.36 TCUPS
 #endif
@@ -167,6 +170,16 @@ __global__ void __launch_bounds__(SHORT_WARPS_PER_CTA * 32, SHORT_MIN_CTAS) k_sh
     auto fetch_even = [&](RawEntry& r, uint32_t dep) {
         if (c.pos == c.end) { c.pos = c.npos; c.end = c.nend; load_next(); }
         e_even = tab + ((((int64_t)(c.pos >> 5)) << 7) + (int64_t)(((c.pos >> 1) & 15) + (dep >> 31)));  // table_slot of an even position
+#if SHORT_L2_LINE_PREFETCH
+        // the group's first lane asks L2 for one 128-byte table line PF entries ahead per two steps: the 8 lines (4 chunk
+        // planes x 2 parities) of a 16-entry half block over 16 entries.  Past the end of a run this runs into the next
+        // read's entries, which the task usually streams next (reads of a haplotype are adjacent in the pair list).
+        if (is_first) {
+            const int t = c.pos + SHORT_L2_LINE_PREFETCH, q = (c.pos >> 1) & 7;
+            const float4* pf = tab + ((((int64_t)(t >> 5)) << 7) + (int64_t)((q >> 1) * TABLE_CHUNK_STRIDE + (q & 1) * 16 + ((t >> 4) & 1) * 8));
+            asm volatile("prefetch.global.L2 [%0];" ::"l"(pf));
+        }
+#endif
         c.pos += 2;
         load_entry(r, e_even);
     };

@@ -216,6 +216,19 @@ def test_equal_length_sweep_shape(B, ctx):
         check(B, ctx, b, B.PHMM_FP64, ref=ref)
 
 
+def test_equal_length_sweep_shape_long(B, ctx):
+    """The upper end of the paper's scalability sweep (PAPER.md:378-392 runs to 131072 bp): one pair each of 16384 and
+    65536 bp (16 and 64 strips chained through boundary records), both precisions, against the oracle."""
+    for L in (16384, 65536):
+        b = W.generate(5, seed=40 + L, n=1, len_lo=L)
+        ref = oracle.forward_batch(b)
+        out, fl = run(B, ctx, b, B.PHMM_FP32_RESCUE)
+        assert fl[0] == B.PHMM_FLAG_LONG
+        assert abs(out[0] - ref[0]) <= TOL32, (L, out[0], ref[0])
+        out64, _ = run(B, ctx, b, B.PHMM_FP64)
+        assert abs(out64[0] - ref[0]) <= TOL64, (L, out64[0], ref[0])
+
+
 def test_async_calls_back_to_back_bitwise(B, ctx):
     """The call only enqueues: different batches issued back to back on one stream (plan uploads of call s+1 run
     on the context's copy stream under the kernels of call s, two plan sets alternate) must give exactly what each
