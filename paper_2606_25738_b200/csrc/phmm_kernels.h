@@ -14,7 +14,10 @@ constexpr int SHORT_N2 = 2 * SHORT_NV;    // columns per CUDA lane
 constexpr int SHORT_MAX_K = 32 * SHORT_N2;  // 1024: widest haplotype one warp covers
 constexpr int CHAIN_NV_F32 = 16;
 constexpr int CHAIN_NV_F64 = 8;
-constexpr int SHORT_WARPS_PER_CTA = 4;
+#ifndef SHORT_WPC_
+#define SHORT_WPC_ 4
+#endif
+constexpr int SHORT_WARPS_PER_CTA = SHORT_WPC_;
 constexpr int TABLE_ZERO_RUN = 256;       // all-zero entries at the start of the row-constant table (idle lanes read them)
 constexpr int TABLE_EXTRA_ROWS = 3;       // short path: run-in entry in front of, sum and flush entries behind every read's rows (phmm_rowconst.cuh)
 // Table positions of the short path.  Every read's run starts at an EVEN entry and has an even length (padded with one
