@@ -14,7 +14,7 @@ value      GCUPS = cells / time / 1e9 (TCUPS x 1000), payload resi
 e2e        same metric through phmm_forward_batch_host: all buffers in pinned HOST memory, the
            host->device copies of the payload and the device->host copy of the results inside the
            timed region ("with transfers").
-roofline   dominant kernel (short: k_short_f32, long: k_chain, fp64: k_rescue_f64) against the FP32 (FP64)
+roofline   dominant kernel (short: k_short_f32, long: k_long_f32, fp64: k_rescue_f64t / k_chain<double>) against the FP32 (FP64)
            non-tensor peak; flops = 10 per cell; duration from the library's CUDA events.
 cpu_baseline  the oracle (oracle/, as it stands) on the host cores on a bounded sample of the same batch.
 
@@ -49,7 +49,7 @@ WORKLOADS = {  # name -> (BASELINE.json config index, description)
 L2_NOTE = ("no flush: the inputs of a step exceed L2 (payload plus the row-constant table, which is rewritten and re-read "
            "every step; 2.9 GB on the short-read batch, 1.3 GB on the long-read batch, 126 MB of L2)")
 FLOPS_PER_CELL = 10.0  # SURVEY 8(d)'s algorithmic count (4 FMA + 2 MUL per cell); DESIGN.md section 7
-FLOPS_PER_CELL_EXECUTED = {"fp32": 9.0, "fp64": 11.0}  # what the engines issue: 4 FMA + 1 MUL (fp32 T/J form), 4 FMA + 3 MUL (fp64 sub-warp kernel)
+FLOPS_PER_CELL_EXECUTED = {"fp32": 9.0, "fp64": 9.0}  # what the engines issue: 4 FMA + 1 MUL (the T/J form, in both precisions)
 
 
 def _measured_peaks():
@@ -286,7 +286,7 @@ def measure(args, workload, steps, rank, world, local, with_cpu):
         kname = "k_long_f32" if args.precision == "fp32" else "k_chain<double> (concurrent strips)"
         kms, kcells = fam["ms_long"], cells * 1.0
     elif args.precision == "fp64":
-        kname, kms, kcells = "k_rescue_f64 (+ chain fallback)", fam["ms_rescue"], cells * 1.0
+        kname, kms, kcells = "k_rescue_f64t<double> (+ chain fallback)", fam["ms_rescue"], cells * 1.0
     else:
         kname, kms, kcells = "k_short_f32", fam["ms_short"], float(st["short_cells"])
     achieved = FLOPS_PER_CELL * kcells / (kms * 1e-3) / 1e12 if kms > 0 else 0.0

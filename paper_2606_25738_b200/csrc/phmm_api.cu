@@ -327,7 +327,7 @@ static int forward_impl(phmm_ctx* ctx, const phmm_batch* b, int precision, doubl
     // ---- slices of reads: equal shares of the table, each within the budget (fp64 uses no table: one slice unless asked)
     const int64_t total_entries = table_run_start(b->h_read_off[nr], nr) - TABLE_ZERO_RUN;
     const int64_t budget_entries = std::max<int64_t>(ctx->opt.max_table_bytes / 64 - 1024, 1 << 16);
-    int n_slices = fp64 ? 1 : (int)std::min<int64_t>(250, (total_entries + budget_entries - 1) / budget_entries);
+    int n_slices = (int)std::min<int64_t>(250, (total_entries + budget_entries - 1) / budget_entries);  // (PHMM_FP64 has a table too: the sub-warp kernel's)
     n_slices = (int)std::max<int64_t>(1, std::min<int64_t>(std::max(n_slices, min_slices), nr));
     std::vector<int64_t> bound((size_t)n_slices + 1, 0);
     bound[(size_t)n_slices] = nr;
@@ -347,8 +347,8 @@ static int forward_impl(phmm_ctx* ctx, const phmm_batch* b, int precision, doubl
         w.slice = s; w.n_slices = n_slices; w.r0 = bound[(size_t)s]; w.r1 = bound[(size_t)s + 1];
         w.table_base = table_run_start(b->h_read_off[w.r0], w.r0) - TABLE_ZERO_RUN;
         w.table_entries = table_run_start(b->h_read_off[w.r1], w.r1) - w.table_base + 192;  // (slack: prefetches run past a run)
-        if (!fp64 && w.table_entries > INT32_MAX) return PHMM_E_TOOLONG;
-        if (!fp64 && w.table_entries * 64 > ctx->opt.max_table_bytes && n_slices >= std::min<int64_t>(250, nr)) return PHMM_E_NOMEM;
+        if (w.table_entries > INT32_MAX) return PHMM_E_TOOLONG;
+        if (w.table_entries * 64 > ctx->opt.max_table_bytes && n_slices >= std::min<int64_t>(250, nr)) return PHMM_E_NOMEM;
     }
 
     // ---- the pairs of each slice (stable: ascending pair index within a slice)
@@ -557,6 +557,15 @@ static int run_slice(phmm_ctx* ctx, const phmm_batch* b, const HostBatchView& hv
         PROF(0, 1);
         launches++;
     }
+    if (fp64 && !sw.sub_pairs.empty()) {  // PHMM_FP64: the same table in double, for the sub-warp kernel
+        const size_t table_bytes = (size_t)sw.table_entries * 64;
+        CK(ctx->d_table.need(table_bytes));
+        ctx->stats.table_bytes = std::max<int64_t>(ctx->stats.table_bytes, (int64_t)table_bytes);
+        PROF(0, 0);
+        CK(launch_table_f64(db, (const double*)ctx->d_lut.p, (double*)ctx->d_table.p, sw.r0, sw.r1, max_seq_l, st));
+        PROF(0, 1);
+        launches++;
+    }
     // ---- short path: systolic kernel, then (below) fp64 rescue of what underflowed
     if (n_warps > 0) {
         ShortLaunch sl;
@@ -641,7 +650,8 @@ static int run_slice(phmm_ctx* ctx, const phmm_batch* b, const HostBatchView& hv
         memset(&rl, 0, sizeof(rl));
         rl.queue.queue = (int4*)ctx->d_rq_queue.p;
         rl.queue.cnt = (int*)ctx->d_rq.p;
-        rl.table = fp64 ? nullptr : (const float*)ctx->d_table.p;
+        rl.table = ctx->d_table.p;
+        rl.table_f64 = fp64 ? 1 : 0;
         rl.max_queue = (int)(fp64 ? (int64_t)sw.sub_pairs.size() : sw.n_short);
         rl.enqueue_pairs = fp64 ? (const int*)ps.d_rq_enq.p : nullptr;
         rl.n_enqueue = fp64 ? (int)sw.sub_pairs.size() : 0;

@@ -147,9 +147,9 @@ struct RescueLaunch {
     int n_enqueue;
     int* plan;                 // RESCUE_PLAN_INTS ints of scratch
     int* sorted;               // max_queue ints of scratch
-    const float* table;        // fp32 mode: the row-constant table of the short path (the recomputation runs in double on
-                               // the fp32-rounded constants: it needs the range, not the precision); nullptr: constants are
-                               // formed in double from the quality bytes (PHMM_FP64)
+    const void* table;         // PHMM_FP32_RESCUE: the fp32 row-constant table of the short path (the recomputation runs in
+                               // double on the fp32-rounded constants: it needs the range, not the precision);
+    int table_f64;             // PHMM_FP64: the table of launch_table_f64 (constants in double)
     const int* pair_read;
     const int* pair_hap;
     const double* lut;
@@ -161,6 +161,8 @@ struct RescueLaunch {
 };
 cudaError_t launch_rescue_f64(const DevBatch& b, const RescueLaunch& r, int grid_ctas, cudaStream_t st);
 int rescue_ctas_per_sm();
+// PHMM_FP64: the row-constant table in double for the sub-warp kernel (64 bytes per entry, field-major blocks of 32 entries)
+cudaError_t launch_table_f64(const DevBatch& b, const double* lut, double* table, int64_t r0, int64_t r1, int max_read_len, cudaStream_t st);
 
 cudaError_t launch_lut_table(const DevBatch& b, const double* lut, float* table, int64_t r0, int64_t r1, int max_read_len, cudaStream_t st);
 cudaError_t launch_short_f32(const DevBatch& b, const ShortLaunch& p, cudaStream_t st);
