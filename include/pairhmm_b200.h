@@ -184,6 +184,15 @@ int phmm_measure_peak(int device, int kind, int reps, double* out_tflops);
 int phmm_plan_host(const phmm_batch* b, int long_min_hap_len, int task_rows, int64_t* plan_counts, int32_t* warp_first,
                    int64_t cap_warps, int32_t* tasks, int64_t cap_tasks, int32_t* sorted_pair, int64_t cap_pairs);
 
+/* Host batcher only (no device is touched): how phmm_forward_batch would cut the reads of `b` into slices for a table budget
+ * of max_table_bytes (0 = default 4 GiB) and at least min_slices slices.  Only the host arrays of `b` are read.
+ *   n_slices     number of slices (written)
+ *   read_first   n_slices + 1 read indices: slice s covers the reads [read_first[s], read_first[s+1])   (may be NULL)
+ *   pair_count   pairs of each slice (a pair belongs to the slice of its read)                           (may be NULL)
+ *   cap_slices   capacity of pair_count (read_first needs cap_slices + 1); PHMM_E_NOMEM if too small */
+int phmm_plan_slices_host(const phmm_batch* b, int64_t max_table_bytes, int min_slices, int64_t* n_slices,
+                          int64_t* read_first, int64_t* pair_count, int64_t cap_slices);
+
 #ifdef __cplusplus
 }
 #endif

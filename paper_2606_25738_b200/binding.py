@@ -22,7 +22,7 @@ PHMM_FP32_RESCUE, PHMM_FP64 = 0, 1
 PHMM_FLAG_RESCUED, PHMM_FLAG_LONG = 1, 2
 
 EXPORTS = ["phmm_create", "phmm_destroy", "phmm_forward_batch", "phmm_forward_batch_host", "phmm_get_stats",
-           "phmm_strerror", "phmm_last_cuda_error", "phmm_measure_peak", "phmm_plan_host"]
+           "phmm_strerror", "phmm_last_cuda_error", "phmm_measure_peak", "phmm_plan_host", "phmm_plan_slices_host"]
 
 
 class phmm_options(ctypes.Structure):
@@ -96,6 +96,9 @@ def lib() -> ctypes.CDLL:
         L.phmm_plan_host.argtypes = [ctypes.POINTER(phmm_batch), ctypes.c_int, ctypes.c_int, ctypes.c_void_p, ctypes.c_void_p,
                                      ctypes.c_int64, ctypes.c_void_p, ctypes.c_int64, ctypes.c_void_p, ctypes.c_int64]
         L.phmm_measure_peak.restype = ctypes.c_int
+        L.phmm_plan_slices_host.restype = ctypes.c_int
+        L.phmm_plan_slices_host.argtypes = [ctypes.POINTER(phmm_batch), ctypes.c_int64, ctypes.c_int, ctypes.c_void_p, ctypes.c_void_p,
+                                            ctypes.c_void_p, ctypes.c_int64]
         _lib = L
     return _lib
 
@@ -164,6 +167,25 @@ def plan_host(batch, long_min_hap_len: int = 0, task_rows: int = 0):
     if rc != PHMM_OK:
         raise PhmmError(rc)
     return {"n_warps": nw, "cols_per_lane": int(counts[3]), "warp_first": wf, "tasks": tk[:nt], "sorted_pair": sp[:ns]}
+
+
+def plan_slices_host(batch, max_table_bytes: int = 0, min_slices: int = 1):
+    """phmm_plan_slices_host: (read_first[n_slices+1], pair_count[n_slices]) -- the slices of reads phmm_forward_batch would
+    process the batch in (no device needed)."""
+    ro = np.ascontiguousarray(batch.read_off, dtype=np.int64); ho = np.ascontiguousarray(batch.hap_off, dtype=np.int64)
+    pr = np.ascontiguousarray(batch.pair_read, dtype=np.int32); ph = np.ascontiguousarray(batch.pair_hap, dtype=np.int32)
+    cb = phmm_batch(len(ro) - 1, len(ho) - 1, len(pr), _hp(ro), _hp(ho), 0, 0, 0, 0, 0, 0, _hp(pr), _hp(ph))
+    n = np.zeros(1, dtype=np.int64)
+    L = lib()
+    rc = L.phmm_plan_slices_host(ctypes.byref(cb), max_table_bytes, min_slices, n.ctypes.data, None, None, 0)
+    if rc != PHMM_OK:
+        raise PhmmError(rc)
+    ns = int(n[0])
+    first = np.zeros(ns + 1, dtype=np.int64); cnt = np.zeros(max(ns, 1), dtype=np.int64)
+    rc = L.phmm_plan_slices_host(ctypes.byref(cb), max_table_bytes, min_slices, n.ctypes.data, first.ctypes.data, cnt.ctypes.data, ns)
+    if rc != PHMM_OK:
+        raise PhmmError(rc)
+    return first, cnt[:ns]
 
 
 class HostBatch:

@@ -246,6 +246,30 @@ extern "C" int phmm_plan_host(const phmm_batch* b, int long_min_hap_len, int tas
     return PHMM_OK;
 }
 
+extern "C" int phmm_plan_slices_host(const phmm_batch* b, int64_t max_table_bytes, int min_slices, int64_t* n_slices,
+                                     int64_t* read_first, int64_t* pair_count, int64_t cap_slices) {
+    if (!b || !n_slices || b->n_pairs < 0 || b->n_reads < 0 || b->n_haps < 0) return PHMM_E_ARG;
+    HostBatchView hv = {b->n_reads, b->n_haps, b->n_pairs, b->h_read_off, b->h_hap_off, b->h_pair_read, b->h_pair_hap};
+    if (b->n_pairs > 0) RC(validate_batch(hv));
+    if (max_table_bytes <= 0) max_table_bytes = (int64_t)4 << 30;
+    std::vector<int64_t> bound;
+    const int ns = b->n_reads > 0 ? slice_reads(hv, max_table_bytes, min_slices, &bound) : 0;
+    *n_slices = ns;
+    if (read_first || pair_count) {
+        if (cap_slices < ns) return PHMM_E_NOMEM;
+        if (read_first) for (int s = 0; s <= ns; s++) read_first[s] = bound[(size_t)s];
+        if (pair_count) {
+            for (int s = 0; s < ns; s++) pair_count[s] = 0;
+            for (int64_t p = 0; p < b->n_pairs; p++) {
+                const int64_t r = b->h_pair_read[p];
+                const int s = (int)(std::upper_bound(bound.begin(), bound.end(), r) - bound.begin()) - 1;
+                pair_count[s]++;
+            }
+        }
+    }
+    return PHMM_OK;
+}
+
 // ---------------------------------------------------------------- staging helper
 namespace {
 struct Stager {  // packs several host arrays into the pinned buffer and copies them with one memcpy each
@@ -324,19 +348,9 @@ static int forward_impl(phmm_ctx* ctx, const phmm_batch* b, int precision, doubl
     const bool fp64 = precision == PHMM_FP64;
     const int64_t np = b->n_pairs, nr = b->n_reads;
 
-    // ---- slices of reads: equal shares of the table, each within the budget (fp64 uses no table: one slice unless asked)
-    const int64_t total_entries = table_run_start(b->h_read_off[nr], nr) - TABLE_ZERO_RUN;
-    const int64_t budget_entries = std::max<int64_t>(ctx->opt.max_table_bytes / 64 - 1024, 1 << 16);
-    int n_slices = (int)std::min<int64_t>(250, (total_entries + budget_entries - 1) / budget_entries);  // (PHMM_FP64 has a table too: the sub-warp kernel's)
-    n_slices = (int)std::max<int64_t>(1, std::min<int64_t>(std::max(n_slices, min_slices), nr));
-    std::vector<int64_t> bound((size_t)n_slices + 1, 0);
-    bound[(size_t)n_slices] = nr;
-    for (int s = 1; s < n_slices; s++) {  // first read whose run starts at or behind the s-th share
-        const int64_t want = TABLE_ZERO_RUN + total_entries * s / n_slices;
-        int64_t lo = bound[(size_t)s - 1], hi = nr;
-        while (lo < hi) { const int64_t mid = (lo + hi) / 2; if (table_run_start(b->h_read_off[mid], mid) < want) lo = mid + 1; else hi = mid; }
-        bound[(size_t)s] = lo;
-    }
+    // ---- slices of reads: equal shares of the table, each within the budget
+    std::vector<int64_t> bound;
+    const int n_slices = slice_reads(hv, ctx->opt.max_table_bytes, min_slices, &bound);
     if (n_slices > 1) {
         ctx->read_slice.resize((size_t)nr);
         for (int s = 0; s < n_slices; s++) memset(ctx->read_slice.data() + bound[(size_t)s], s, (size_t)(bound[(size_t)s + 1] - bound[(size_t)s]));

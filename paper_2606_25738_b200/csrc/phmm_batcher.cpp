@@ -62,6 +62,25 @@ void sort_pairs_by_hap(const HostBatchView& b, const uint8_t* is_short, std::vec
     });
 }
 
+// Slices of consecutive reads: equal shares of the row-constant table (64 bytes per entry), as many as it takes for a
+// share to stay within max_table_bytes (at least min_slices, at most 250 and one per read).  bound: n_slices + 1 read indices.
+int slice_reads(const HostBatchView& b, int64_t max_table_bytes, int min_slices, std::vector<int64_t>* bound) {
+    const int64_t nr = b.n_reads;
+    const int64_t total_entries = table_run_start(b.read_off[nr], nr) - TABLE_ZERO_RUN;
+    const int64_t budget_entries = std::max<int64_t>(max_table_bytes / 64 - 1024, 1 << 16);
+    int n_slices = (int)std::min<int64_t>(250, (total_entries + budget_entries - 1) / budget_entries);
+    n_slices = (int)std::max<int64_t>(1, std::min<int64_t>(std::max(n_slices, min_slices), nr));
+    bound->assign((size_t)n_slices + 1, 0);
+    (*bound)[(size_t)n_slices] = nr;
+    for (int s = 1; s < n_slices; s++) {  // first read whose run starts at or behind the s-th share
+        const int64_t want = TABLE_ZERO_RUN + total_entries * s / n_slices;
+        int64_t lo = (*bound)[(size_t)s - 1], hi = nr;
+        while (lo < hi) { const int64_t mid = (lo + hi) / 2; if (table_run_start(b.read_off[mid], mid) < want) lo = mid + 1; else hi = mid; }
+        (*bound)[(size_t)s] = lo;
+    }
+    return n_slices;
+}
+
 // Stable counting sort of all pair indices by the slice their read belongs to: slice_first[s] = first position of slice s.
 void bucket_pairs_by_slice(const HostBatchView& b, const uint8_t* read_slice, int n_slices, std::vector<int>* out,
                            std::vector<int64_t>* slice_first) {

@@ -54,6 +54,7 @@ struct ShortPlan {
 void plan_short(const HostBatchView& b, const uint8_t* is_short, int cols_per_lane, int task_rows, ShortPlan* out);
 // The three stages of plan_short, for batches that are processed in slices of reads (phmm_api.cu):
 void sort_pairs_by_hap(const HostBatchView& b, const uint8_t* is_short, std::vector<int>* sorted);
+int slice_reads(const HostBatchView& b, int64_t max_table_bytes, int min_slices, std::vector<int64_t>* bound);
 void bucket_pairs_by_slice(const HostBatchView& b, const uint8_t* read_slice, int n_slices, std::vector<int>* out,
                            std::vector<int64_t>* slice_first);
 void sort_ids_by_hap(const HostBatchView& b, const int* ids, int64_t n, std::vector<int>* sorted);

@@ -93,3 +93,23 @@ def test_replica_aggregation_world_size_2_gloo():
 
 def test_replica_aggregation_single_process():
     assert replicas.aggregate(4.0, 8.0, 2.0) == (4.0, 8.0, 2.0)
+
+
+def test_slices_of_reads_respect_the_table_budget():
+    """phmm_plan_slices_host: the cut of a batch into slices of consecutive reads: the slices cover
+    all reads in order, every slice's table (64 bytes per entry: l + 3 rounded up to even per read, 4 slots of slack) stays
+    within the budget up to one read, every pair lands in the slice of its read."""
+    b = W.generate(2, n=60000)
+    rl = b.read_len()
+    for budget, min_slices in ((8 << 20, 1), (32 << 20, 1), (4 << 30, 1), (4 << 30, 6)):
+        first, cnt = B.plan_slices_host(b, budget, min_slices)
+        ns = len(cnt)
+        assert first[0] == 0 and first[-1] == b.n_reads and np.all(np.diff(first) >= 0)
+        assert ns >= min_slices and cnt.sum() == b.n_pairs
+        sl = np.searchsorted(first, b.pair_read, side="right") - 1
+        assert np.array_equal(np.bincount(sl, minlength=ns), cnt)
+        entries = np.add.reduceat(rl + 5, first[:-1])[:ns] if ns > 1 else np.array([np.sum(rl + 5)])  # (at most l + 5 table slots per read)
+        if budget < (4 << 30):
+            assert ns > 1 and np.all(entries * 64 <= budget + 64 * (rl.max() + 5))
+        else:
+            assert ns == max(1, min_slices)
