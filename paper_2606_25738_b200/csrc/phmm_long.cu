@@ -43,9 +43,10 @@ namespace phmm {
 #define LONG_MIN_CTAS 3
 #endif
 constexpr int LONG_WPC = 4;       // warps per CTA
-constexpr int LONG_TGT = 0;       // a lane's maximum is brought back to 2^TGT at every event (0: the shift 2^(TGT - ilogb) is always one factor)
-constexpr int LONG_KTOT = 90;     // a lane's exponent is at most this much below that of any lane to its left
+constexpr int LONG_TGT = 40;      // a lane's maximum is brought back to 2^TGT at every event: 166 bits of range below it
+constexpr int LONG_KTOT = 80;     // a lane's exponent is at most this much below that of any lane to its left
 constexpr int LONG_EVERY = 16;    // steps between two events
+constexpr int LONG_DROP = 126;    // a lane's own maximum may fall by 2^LONG_DROP between two events before the pair is sent to fp64
 constexpr int LONG_FLOOR = -(1 << 28);  // "no proposal" (a lane that holds nothing but zeros)
 
 __device__ __forceinline__ int ld_relaxed_gpu(const int* p) {
@@ -88,6 +89,8 @@ struct LongSmem {
     float2 rin[LONG_EVERY];   // boundary values lane 0 consumes in the next 16 steps, already at its exponent
     float2 rout[LONG_EVERY];  // what lane 31 handed out in the last 16 steps (flushed to the records at the next event)
     float2 fin[32];           // per lane: its share of Eq.4 and the exponent it is stored at
+    uint8_t own[32];          // per lane: see the event
+    int lossy;
 };
 
 template <int NV, bool HS>  // HS = false only under phmm_options.n_is_wildcard (phmm_short.cu)
@@ -130,6 +133,10 @@ __global__ void __launch_bounds__(LONG_WPC * 32, LONG_MIN_CTAS) k_long_f32(DevBa
         float f_in = 1.f;      // 2^(ex of the left neighbour - ex)
         int seen = 0;          // entries the producer strip is known to have published
         int pre = -1;          // first entry of the boundary records that are on their way into sm.rraw (-1: none)
+        // sm.own[lane]: at the last event this lane's exponent was set by its own maximum (stored maximum = 2^TGT);
+        // sm.lossy: some lane's maximum then fell by more than 2^LONG_DROP within one interval (see the event)
+        sm.own[lane] = 0;
+        if (lane == 0) sm.lossy = 0;
         sm.fin[lane] = make_float2(0.f, 0.f);
 
         // ---- fetch.  The table blocks live in the ring, filled by cp.async one block (32 steps) ahead of lane 0: the step
@@ -217,7 +224,17 @@ __global__ void __launch_bounds__(LONG_WPC * 32, LONG_MIN_CTAS) k_long_f32(DevBa
             float m = fmax3(ln.outS.x, ln.outS.y, fmaxf(ln.outT.x, ln.outT.y));
 #pragma unroll
             for (int x = 0; x < NV; x++) m = fmax3(m, fmaxf(ln.Tt[x].x, ln.Tt[x].y), fmaxf(ln.J[x].x, ln.J[x].y));
-            int c = m > 0.f ? ex + Fx<float>::ilogb(m) - LONG_TGT : LONG_FLOOR;
+            int c = m > 0.f ? ex + max(Fx<float>::ilogb(m) - LONG_TGT, -127) : LONG_FLOOR;  // (the shift 2^(ex - ex') stays one factor)
+            // Soundness of the 16-step interval: a lane whose own maximum stood at 2^TGT one event ago and has dropped by more
+            // than LONG_DROP bits since (it takes gap-continuation qualities above 20, i.e. more than ~7 bits lost per row on every
+            // path) may have flushed values that were NOT negligible (less than 166 - LONG_DROP bits below that maximum): the pair is
+            // recomputed by the fp64 chain kernel.  Only while the lane is inside the read's rows and holds real columns.
+            {
+                const int e = s - 2 * lane;
+                const int lane_hi = (min(k - strip * STRIP, STRIP) - 1) / N2;  // lanes that hold real columns
+                if (sm.own[lane] && lane <= lane_hi && e - LONG_EVERY >= 1 && e + 1 <= l && !(m > 0.f && Fx<float>::ilogb(m) >= LONG_TGT - LONG_DROP))
+                    sm.lossy = 1;
+            }
             int bmax = LONG_FLOOR;
             if (in_now) {
                 const float mi = fmaxf(rec.x, rec.y);
@@ -240,7 +257,8 @@ __global__ void __launch_bounds__(LONG_WPC * 32, LONG_MIN_CTAS) k_long_f32(DevBa
             if (lane == 0) pm = bsrc;
             if (pm > LONG_FLOOR) c = max(c, pm - LONG_KTOT);
             const int exn = c < LONG_FLOOR / 2 ? ex : c;  // nothing held, nothing to the left: keep the exponent
-            // 4. rescale the state: d <= TGT - ilogb(m) <= 127 when something is held, any d when nothing is
+            sm.own[lane] = m > 0.f && exn == ex + Fx<float>::ilogb(m) - LONG_TGT;  // (a clamped proposal does not count)
+            // 4. rescale the state: d <= 127 when something is held (the proposal is clamped), any d when nothing is
             const float f = pow2f(m > 0.f ? ex - exn : 0);  // 0 for d < -126: what is held is negligible against what arrives
             const float2 F = make_float2(f, f);
 #pragma unroll
@@ -327,7 +345,8 @@ __global__ void __launch_bounds__(LONG_WPC * 32, LONG_MIN_CTAS) k_long_f32(DevBa
 
         // ---- Eq.4: combine the lanes' shares, then the strips' (each strip waits for the total of the strips to its left)
         const float2 fin = sm.fin[lane];
-        const float fin_m = fin.x;
+        __syncwarp();
+        const float fin_m = sm.lossy ? __int_as_float(0x7fc00000) : fin.x;  // (NaN poisons the total)
         const int fin_e = __float_as_int(fin.y);
         int em = fin_m > 0.f ? fin_e + Fx<float>::ilogb(fin_m) : LONG_FLOOR;  // exponent of the largest share
 #pragma unroll

@@ -229,6 +229,52 @@ def test_equal_length_sweep_shape_long(B, ctx):
         assert abs(out64[0] - ref[0]) <= TOL64, (L, out64[0], ref[0])
 
 
+def test_long_kernel_stress_mixed_structure(B, ctx):
+    """The fp32 long kernel's exponent scheme on inputs built to move the mass around: haplotypes of
+    1.1-5 kbp, reads of 50-3000 bp that are related, unrelated, or related in one part and unrelated in the other, with
+    deletions of up to 55 and insertions of up to 40 bases, per-base gap-continuation qualities between 5 and 30 (rows on
+    which the running sum hardly decays next to rows on which it vanishes within a lane), base qualities 5-40."""
+    rng = np.random.default_rng(77)
+    cases = []
+    for it in range(120):
+        k = int(rng.integers(1100, 5000))
+        hap = _rand_seq(rng, k)
+        l = int(rng.integers(50, min(3000, k - 100)))
+        kind = it % 4
+        s0 = int(rng.integers(0, k - l - 60))
+        rd = list(hap[s0:s0 + l + 60])
+        if kind == 1:
+            rd = list(_rand_seq(rng, l))                                   # unrelated
+        elif kind == 2:
+            cut = int(rng.integers(l // 4, 3 * l // 4))
+            rd = rd[:cut] + list(_rand_seq(rng, l - cut))                  # related head, unrelated tail
+        elif kind == 3:
+            cut = int(rng.integers(l // 4, 3 * l // 4))
+            d = int(rng.integers(5, 56))
+            rd = rd[:cut] + rd[cut + d:]                                   # a deletion of d bases in the read
+            if rng.random() < 0.5:
+                c2 = int(rng.integers(10, max(11, cut - 5)))
+                rd = rd[:c2] + list(_rand_seq(rng, int(rng.integers(3, 41)))) + rd[c2:]  # and an insertion
+        rd = rd[:l]
+        for i in rng.choice(len(rd), max(1, len(rd) // 30), replace=False):
+            rd[i] = "ACGT"[int(rng.integers(0, 4))]
+        n = len(rd)
+        gcp = rng.integers(5, 31, n) if it % 3 else np.full(n, 10)
+        cases.append(("".join(rd), hap, list(rng.integers(5, 41, n)), list(rng.integers(15, 50, n)), list(rng.integers(15, 50, n)), list(gcp)))
+    b = W.from_strings(cases)
+    ref = oracle.forward_batch(b)
+    out, fl = run(B, ctx, b, B.PHMM_FP32_RESCUE)
+    assert np.all(np.isfinite(out))
+    err = np.abs(out - ref)
+    bad = np.where(~(err <= TOL32))[0]
+    assert len(bad) == 0, "max err %g at %s (got %s want %s, flags %s)" % (err.max(), bad[:6], out[bad[:6]], ref[bad[:6]], fl[bad[:6]])
+    assert np.all(fl & B.PHMM_FLAG_LONG)
+    n_fb = int((fl & B.PHMM_FLAG_RESCUED).sum())
+    print("long-kernel stress: max |dlog10| %.2e, %d of %d pairs fell back to the fp64 chain kernel" % (err.max(), n_fb, b.n_pairs))
+    out64, _ = run(B, ctx, b, B.PHMM_FP64)
+    assert np.max(np.abs(out64 - ref)) <= TOL64
+
+
 def test_async_calls_back_to_back_bitwise(B, ctx):
     """The call only enqueues: different batches issued back to back on one stream (plan uploads of call s+1 run
     on the context's copy stream under the kernels of call s, two plan sets alternate) must give exactly what each
