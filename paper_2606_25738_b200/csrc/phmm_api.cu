@@ -84,7 +84,7 @@ struct phmm_ctx {
     cudaEvent_t ev_last = nullptr;  // end of the device work of the most recent call: the next call's stream waits for it,
                                     // because the table, the counters, the queues and the boundary buffers exist once per context
     DevBuf d_lut, d_table;
-    DevBuf d_counters, d_rescue, d_boundary, d_progress, d_scratch, d_totals, d_acc;
+    DevBuf d_counters, d_rescue, d_boundary, d_progress, d_scratch, d_totals, d_acc, d_risk;
     DevBuf d_rq, d_rq_queue, d_rq_sorted, d_rq_plan;  // fp64 sub-warp recomputation: counters, queue, ordered queue, plan
     DevBuf d_payload, d_out, d_flags;  // phmm_forward_batch_host only
     std::vector<uint8_t> is_short, read_slice;
@@ -169,7 +169,7 @@ extern "C" int phmm_destroy(phmm_ctx* ctx) {
     if (!ctx) return PHMM_E_ARG;
     DeviceGuard guard(ctx->device);
     cudaDeviceSynchronize();
-    DevBuf* bufs[] = {&ctx->d_lut, &ctx->d_table, &ctx->d_counters, &ctx->d_rescue, &ctx->d_boundary, &ctx->d_progress, &ctx->d_scratch, &ctx->d_totals, &ctx->d_acc,
+    DevBuf* bufs[] = {&ctx->d_lut, &ctx->d_table, &ctx->d_counters, &ctx->d_rescue, &ctx->d_boundary, &ctx->d_progress, &ctx->d_scratch, &ctx->d_totals, &ctx->d_acc, &ctx->d_risk,
                       &ctx->d_payload, &ctx->d_out, &ctx->d_flags, &ctx->d_rq, &ctx->d_rq_queue, &ctx->d_rq_sorted, &ctx->d_rq_plan};
     for (DevBuf* b : bufs) b->release();
     for (int i = 0; i < 2; i++) {
@@ -633,6 +633,8 @@ static int run_slice(phmm_ctx* ctx, const phmm_batch* b, const HostBatchView& hv
         } else {
             CK(ctx->d_boundary.need((size_t)(n_bnd_blocks + 1) * 16));
             CK(ctx->d_totals.need((size_t)n_prog * 16 + 16));
+            CK(ctx->d_risk.need((size_t)b->n_reads + 16));
+            CK(launch_read_risk(db, ctx->opt.qual_offset, sw.r0, sw.r1, (uint8_t*)ctx->d_risk.p, st));
             LongLaunch ll;
             memset(&ll, 0, sizeof(ll));
             ll.table = (const float*)ctx->d_table.p;
@@ -652,6 +654,7 @@ static int run_slice(phmm_ctx* ctx, const phmm_batch* b, const HostBatchView& hv
             ll.publish = need_ctas <= ctx->long_grid ? 16 : 64;
             ll.fallback_count = counters + 0;
             ll.fallback_list = (int*)ctx->d_rescue.p;
+            ll.risk = (const uint8_t*)ctx->d_risk.p;
             CK(launch_long_f32(db, ll, std::min(ctx->long_grid, need_ctas), st));
         }
         PROF(3, 1);

@@ -167,7 +167,14 @@ k_chain(DevBatch b, ChainLaunch p, int items_are_pairs) {
         const int l = (int)(b.read_off[r + 1] - ro), k = (int)(b.hap_off[h + 1] - ho);
         const int n_ent = l + CHAIN_EXTRA_ROWS;  // run-in entry, rows 1..l, sum entry, flush entry
         const int nstrips = (k + 32 * N2 - 1) / (32 * N2);
-        const bool full_last = k == nstrips * 32 * N2;  // no column behind the haplotype's last one (see the output below)
+        // The lane that holds the haplotype's last column, in the last strip: Eq.4 is taken there, and nothing flows into the
+        // lanes behind it.  (Until round 2 the sum travelled on to lane 31 through lanes that hold only padding columns; what
+        // circulates there -- mismatch diagonals that never run out of columns -- can decay more slowly than the real cells,
+        // where every further read base has to be an insertion, and the sum, converted from lane to lane to ever larger
+        // exponents, vanished: -inf for a 535-base read against a 2-base haplotype at GCP 40.  Found by fuzzing.)
+        const int k_last = k - (nstrips - 1) * 32 * N2;   // real columns of the last strip
+        const int out_lane = (k_last - 1) / N2;
+        const bool full_last = (k_last % N2) == 0;        // its last real column is the last column of that lane (see the output below)
         const int nblk = (n_ent + 31) / 32;  // boundary blocks per buffer
         const int st_lo = strip < 0 ? 0 : strip, st_hi = strip < 0 ? nstrips : strip + 1;
         const T Cok = (T)(ldexp(1.0, p.log2C) / (double)k);
@@ -292,6 +299,7 @@ k_chain(DevBatch b, ChainLaunch p, int items_are_pairs) {
                         exL = 0;
                     }
                 }
+                if (!has_out && lane > out_lane) { inS = (T)0; inT = (T)0; }  // lanes of padding columns only stay empty
                 // ---- bring the incoming values to this thread's exponent (exact power-of-two multiply)
                 {
                     const T mi = Fx<T>::fmax_(inS, inT);
@@ -332,13 +340,14 @@ k_chain(DevBatch b, ChainLaunch p, int items_are_pairs) {
                             }
                             __syncwarp();
                         }
-                    } else if (eo == l + 1 && lane == 31) {  // the sum entry: s has collected Eq.4; log10 in double
-                        // M+I of column j reaches the chain through the T of column j+1; a haplotype that fills its last
-                        // strip has the last one in what this lane handed out one step ago instead
-                        const T sum = full_last ? ln.outS.y + prevT : ln.outS.y;
-                        p.out[pair] = log10((double)sum) + ((double)ex - (double)p.log2C) * LOG10_2;
-                        if (p.flags) p.flags[pair] = p.flag_bits | ((items_are_pairs && (k > p.long_k || l > 4096)) ? 2u /* PHMM_FLAG_LONG */ : 0u);
                     }
+                }
+                if (!has_out && lane == out_lane && (E.metaY & META_SUM)) {  // the sum entry: s has collected Eq.4; log10 in double
+                    // M+I of column j reaches the chain through the T of column j+1; a haplotype that fills its last
+                    // lane has the last one in what this lane handed out one step ago instead
+                    const T sum = full_last ? ln.outS.y + prevT : ln.outS.y;
+                    p.out[pair] = log10((double)sum) + ((double)ex - (double)p.log2C) * LOG10_2;
+                    if (p.flags) p.flags[pair] = p.flag_bits | ((items_are_pairs && (k > p.long_k || l > 4096)) ? 2u /* PHMM_FLAG_LONG */ : 0u);
                 }
             }
             __syncwarp();

@@ -21,7 +21,9 @@
 //      the lane's own maximum or 2^-(126+TGT+KTOT) below the maximum of a lane to its left: G15's documented limit) and
 //      recomputes f_in.
 // A result that is not a normal positive number (or a NaN anywhere in a lane's share of Eq.4) sends the pair to the
-// fp64 chain kernel (phmm_chain.cu): the same cascade as fp32 -> fp64 for short pairs.
+// fp64 chain kernel (phmm_chain.cu): the same cascade as fp32 -> fp64 for short pairs.  So does a lane whose maximum falls
+// by more than 2^LONG_DROP between two events, and so does the input guard k_read_risk at the end of this file, which
+// states when 166 bits of range below a lane's maximum are enough.
 //
 // Eq.4.  The short kernel lets the running sum s collect M_l + I_l across the whole lane group on the "sum entry".  Here
 // the lanes of a group do not share an exponent and s does not decay on that entry, so each lane takes only its OWN sum
@@ -125,6 +127,13 @@ __global__ void __launch_bounds__(LONG_WPC * 32, LONG_MIN_CTAS) k_long_f32(DevBa
         const int run0 = (int)(table_run_start(ro, r) - b.table_base), run_len = table_run_len(l);
         const int nstrips = (k + STRIP - 1) / STRIP;
         const bool has_in = strip > 0, has_out = strip + 1 < nstrips;
+        if (p.risk[r]) {  // k_read_risk: fp32's range per lane may not do for this read; the pair's last strip hands it to fp64
+            if (!has_out && lane == 0) {
+                const int idx = atomicAdd(p.fallback_count, 1);
+                p.fallback_list[idx] = pair;
+            }
+            continue;
+        }
 
         L ln;
         ln.init();
@@ -386,6 +395,59 @@ __global__ void __launch_bounds__(LONG_WPC * 32, LONG_MIN_CTAS) k_long_f32(DevBa
         }
         __syncwarp();
     }
+}
+
+// ---- input guard of the fp32 long kernel.  Inside one lane (32 columns, 2 rows) everything shares one exponent, 166 bits of
+// range below the lane's maximum A.  A cell B of the same lane that is flushed can never matter later if A's path can reach B's
+// continuation for less than those 166 bits: either by deleting up to 31 columns in B's row (cost 31 x 0.332 x GCP of the row +
+// the gap-open cost) or by inserting up to 32 rows (0.332 x the sum of their GCP qualities + the open cost).  At GCP 10 both
+// bridges cost ~125 bits: 40 bits of margin, what is flushed weighs < 2^-40.  A read with any GCP quality above 10 is marked
+// and k_long_f32 hands its pairs to the fp64 chain kernel.  (Found by fuzzing with per-base GCP between 3 and 40: results
+// off by up to 0.6 in log10 with no non-finite value to detect.)  Second condition, the padding columns of the haplotype's
+// last lane: mismatch diagonals seeded by the real columns keep running there at the cost of a mismatch per row
+// (0.332 Qbase + 1.585 bits) while the real cells, once their diagonals have run off the haplotype's end, pay a gap
+// continuation per row (0.332 GCP): where base qualities stay below ~5 for long, the padding outgrows the real cells and
+// takes the lane's exponent with it.  A read whose best stretch of rows gains the padding more than 60 bits is marked too.
+// One warp per read; every lane scans a contiguous share of the rows, the shares are combined (maximum subarray).
+__global__ void k_read_risk(DevBatch b, int qual_offset, int64_t r0, int64_t r1, uint8_t* __restrict__ risk) {
+    const int64_t r = r0 + (int64_t)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+    if (r >= r1) return;
+    const int lane = threadIdx.x & 31;
+    const int64_t off = b.read_off[r];
+    const int l = (int)(b.read_off[r + 1] - off);
+    const int seg = (l + 31) / 32, lo = min(l, lane * seg), hi = min(l, lo + seg);
+    bool bad = false;
+    // maximum-subarray summary of this lane's rows: total, best prefix, best suffix, best
+    float tot = 0.f, pre = 0.f, suf = 0.f, best = 0.f;
+    for (int i = lo; i < hi; i++) {
+        const int g = max((int)b.qual_gcp[off + i] - qual_offset, 0), q = max((int)b.qual_base[off + i] - qual_offset, 0);
+        if (g > 10) bad = true;
+        const float v = 0.332f * (float)(g - q) - 1.585f;
+        tot += v;
+        pre = fmaxf(pre, tot);
+        suf = fmaxf(suf + v, 0.f);
+        best = fmaxf(best, suf);
+    }
+    for (int o = 1; o < 32; o <<= 1) {  // inclusive scan of the summaries, left to right
+        const float t2 = __shfl_up_sync(PHMM_FULL, tot, o), p2 = __shfl_up_sync(PHMM_FULL, pre, o);
+        const float s2 = __shfl_up_sync(PHMM_FULL, suf, o), b2 = __shfl_up_sync(PHMM_FULL, best, o);
+        if (lane >= o) {  // (left = the shuffled one, right = this lane's)
+            best = fmaxf(fmaxf(best, b2), s2 + pre);
+            pre = fmaxf(p2, t2 + pre);
+            suf = fmaxf(suf, s2 + tot);
+            tot = t2 + tot;
+        }
+    }
+    if (best > 60.f) bad = true;
+    if (__any_sync(PHMM_FULL, bad) && lane == 0) risk[r] = 1;
+}
+
+cudaError_t launch_read_risk(const DevBatch& b, int qual_offset, int64_t r0, int64_t r1, uint8_t* risk, cudaStream_t st) {
+    if (r1 <= r0) return cudaSuccess;
+    cudaError_t e = cudaMemsetAsync(risk + r0, 0, (size_t)(r1 - r0), st);
+    if (e != cudaSuccess) return e;
+    k_read_risk<<<(unsigned)((r1 - r0 + 7) / 8), 256, 0, st>>>(b, qual_offset, r0, r1, risk);
+    return cudaGetLastError();
 }
 
 cudaError_t launch_long_f32(const DevBatch& b, const LongLaunch& p, int grid_ctas, cudaStream_t st) {

@@ -53,9 +53,10 @@ def check(B, ctx, batch, prec, ref=None, pairs=None):
     return out, fl, ref
 
 
-def check_flags(B, batch, fl, ref, pairs=None):
+def check_flags(B, batch, fl, ref, pairs=None, long_may_fall_back=False):
     """Rescue flags must equal the oracle's prediction except within +-1e-3 of the threshold (G16).
-    Only short-path pairs can be rescued; long-path pairs carry PHMM_FLAG_LONG instead."""
+    That criterion is the short path's; long-path pairs carry PHMM_FLAG_LONG, and PHMM_FLAG_RESCUED on top only where the
+    fp32 long kernel handed the pair to fp64 (never on the GCP-10 data of the configs)."""
     f = fl if pairs is None else fl[pairs]
     is_long = (f & B.PHMM_FLAG_LONG) != 0
     want = ref < RESCUE_LOG10
@@ -63,7 +64,7 @@ def check_flags(B, batch, fl, ref, pairs=None):
     sel = ~is_long & ~border
     got = (f & B.PHMM_FLAG_RESCUED) != 0
     assert np.array_equal(got[sel], want[sel]), "rescue flag mismatch at %s" % np.where(got[sel] != want[sel])[0][:8]
-    assert not np.any(got & is_long)
+    assert long_may_fall_back or not np.any(got & is_long)
     return int(border.sum())
 
 
@@ -329,6 +330,88 @@ def test_host_entry_matches_device_entry(B, ctx):
     assert hb.h2d_bytes() > 5 * len(b.read_bases) and hb.d2h_bytes() == 9 * b.n_pairs
 
 
+# ------------------------------------------------------------------ randomized batches (the fuzzer that found round 2's bugs)
+def _fz_rs(rng, n): return "".join(rng.choice(list("ACGT"), n))
+def _fz_make(rng, npairs, kmax, lmax):
+    haps=[]; reads=[]; pr=[]; ph=[]
+    nh = max(1, npairs // int(rng.integers(1, 12)))
+    for h in range(nh):
+        k = int(rng.integers(1, kmax)) if rng.random() < 0.9 else int(rng.choice([1,2,31,32,33,63,64,65,1023,1024,1025,2048]))
+        s = list(_fz_rs(rng, k))
+        if rng.random() < 0.2:
+            for i in rng.choice(k, max(1, k // 40), replace=False): s[i] = 'N'
+        haps.append("".join(s))
+    for p in range(npairs):
+        h = int(rng.integers(0, nh)); hap = haps[h]; k = len(hap)
+        l = int(rng.integers(1, lmax))
+        mode = rng.random()
+        if mode < 0.55 and k > 2:
+            s0 = int(rng.integers(0, max(1, k - 1)))
+            rd = list((hap[s0:s0 + l] + _fz_rs(rng, l))[:l])
+            for i in rng.choice(l, max(0, l // 25), replace=False): rd[i] = "ACGTN"[int(rng.integers(0, 5))]
+            if l > 20 and rng.random() < 0.3:
+                c = int(rng.integers(5, l - 5)); d = int(rng.integers(1, 30)); rd = (rd[:c] + rd[c + d:] + list(_fz_rs(rng, d)))[:l]
+        else:
+            rd = list(_fz_rs(rng, l))
+        qmode = rng.random()
+        if qmode < 0.4:
+            q = (rng.integers(2, 42, l), rng.integers(10, 61, l), rng.integers(10, 61, l), np.full(l, 10))
+        elif qmode < 0.55:
+            q = (rng.integers(2, 8, l), rng.integers(10, 61, l), rng.integers(10, 61, l), rng.integers(3, 11, l))
+        elif qmode < 0.8:
+            q = (rng.integers(2, 42, l), rng.integers(10, 61, l), rng.integers(10, 61, l), rng.integers(3, 41, l))
+        else:
+            q = (np.full(l, 30), np.full(l, 45), np.full(l, 45), np.full(l, 10))
+        reads.append(("".join(rd),) + q); pr.append(len(reads) - 1); ph.append(h)
+        if rng.random() < 0.3 and nh > 1:
+            pr.append(len(reads) - 1); ph.append(int(rng.integers(0, nh)))
+    cat = lambda i: np.concatenate([np.asarray(r[i], dtype=np.uint8) if i else np.frombuffer(r[0].encode(), dtype=np.uint8) for r in reads])
+    b = W.Batch(np.concatenate([[0], np.cumsum([len(r[0]) for r in reads])]).astype(np.int64),
+                np.concatenate([[0], np.cumsum([len(h) for h in haps])]).astype(np.int64),
+                cat(0), cat(1), cat(2), cat(3), cat(4), np.frombuffer("".join(haps).encode(), dtype=np.uint8),
+                np.asarray(pr, dtype=np.int32), np.asarray(ph, dtype=np.int32))
+    return b.select_pairs(rng.permutation(b.n_pairs))
+
+
+def test_randomized_batches_against_oracle(B, ctx):
+    """Seeded random batches of every shape the entry points accept -- haplotypes of 1..6000 bases (tile-boundary lengths
+    over-represented), reads of 1..3000, related / unrelated / with gaps, N bases, constant and per-base qualities with GCP
+    between 3 and 40 -- through both precisions, one and many slices, and the host entry, element-wise against the oracle.
+    Where PHMM_FP64 and the C oracle disagree the log-space companion (oracle/logspace.py) arbitrates: with GCP qualities
+    near 40 single rows lose more than the 2^-1074 the oracle keeps below a row's maximum (its documented limit).
+    This loop, run for minutes, found: -inf from the fp64 chain kernel for long reads against very short haplotypes at
+    GCP 40 (padding lanes), and silent errors of up to 0.6 in the fp32 long kernel for GCP above 10 (now guarded)."""
+    from oracle import logspace
+    cs = B.Context(0, max_table_bytes=4 << 20)
+    n_arb = n_long = n_fb = 0
+    try:
+        for it in range(36):
+            rng = np.random.default_rng(7000 + it)
+            kind = it % 3
+            b = _fz_make(rng, [400, 60, 12][kind], [400, 1500, 6000][kind], [300, 700, 3000][kind])
+            ref = oracle.forward_batch(b)
+            db = B.DeviceBatch(b)
+            o64, _ = ctx.forward_batch(db, B.PHMM_FP64)
+            o64 = o64.cpu().numpy()
+            for i in np.where(~(np.abs(o64 - ref) <= TOL64))[0]:
+                pp = b.pair(i)
+                ref[i] = logspace.log10_likelihood(pp[0], pp[5], pp[1], pp[2], pp[3], pp[4])
+                n_arb += 1
+            assert np.all(np.abs(o64 - ref) <= TOL64), "seed %d fp64" % (7000 + it)
+            for c in (ctx, cs):
+                o, f = c.forward_batch(db, B.PHMM_FP32_RESCUE)
+                o, f = o.cpu().numpy(), f.cpu().numpy()
+                e = np.abs(o - ref)
+                assert np.all(e <= TOL32), "seed %d fp32: pair %d got %r want %r flag %d" % (7000 + it, int(np.nanargmax(e)), o[int(np.nanargmax(e))], ref[int(np.nanargmax(e))], f[int(np.nanargmax(e))])
+                n_long += int(((f & 2) == 2).sum()); n_fb += int(((f & 3) == 3).sum())
+            oh, fh = ctx.forward_batch_host(b, B.PHMM_FP32_RESCUE)
+            assert np.all(np.abs(oh - ref) <= TOL32), "seed %d host entry" % (7000 + it)
+    finally:
+        cs.close()
+    print("randomized: %d long pairs, %d of them handed to fp64, %d arbitrations by the log-space companion" % (n_long, n_fb, n_arb))
+    assert n_long > 200 and n_fb < n_long
+
+
 # ------------------------------------------------------------------ edge cases
 def _rand_seq(rng, n):
     return "".join(rng.choice(list("ACGT"), n))
@@ -378,7 +461,8 @@ def test_nonuniform_gcp_and_streams(B, ctx):
                 cat(0), cat(1), cat(2), cat(3), cat(4), np.frombuffer("".join(haps).encode(), dtype=np.uint8),
                 np.asarray(pr, dtype=np.int32), np.asarray(ph, dtype=np.int32))
     out, fl, ref = check(B, ctx, b, B.PHMM_FP32_RESCUE)
-    check_flags(B, b, fl, ref)
+    check_flags(B, b, fl, ref, long_may_fall_back=True)  # (GCP above 10 on the 1500-base haplotype: the input guard sends those to fp64)
+    assert np.all(fl[28:] & B.PHMM_FLAG_LONG)
     check(B, ctx, b, B.PHMM_FP64, ref=ref)
 
 
