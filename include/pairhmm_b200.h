@@ -56,6 +56,7 @@ extern "C" {
 /* bits of the per-pair output flags */
 #define PHMM_FLAG_RESCUED 1u /* PHMM_FP32_RESCUE only: pair was recomputed in fp64 */
 #define PHMM_FLAG_LONG 2u    /* pair went through the multi-warp / multi-CTA rescaled wavefront path */
+#define PHMM_FLAG_RANGE 4u   /* phmm_forward_batch_noalloc only: the likelihood left the range of unscaled double (value unusable) */
 
 typedef struct phmm_ctx phmm_ctx; /* opaque; owns workspaces, internal streams, the last stats */
 
@@ -192,6 +193,30 @@ int phmm_plan_host(const phmm_batch* b, int long_min_hap_len, int task_rows, int
  *   cap_slices   capacity of pair_count (read_first needs cap_slices + 1); PHMM_E_NOMEM if too small */
 int phmm_plan_slices_host(const phmm_batch* b, int64_t max_table_bytes, int min_slices, int64_t* n_slices,
                           int64_t* read_first, int64_t* pair_count, int64_t cap_slices);
+
+/* ---- An entry point that allocates nothing (no cudaMalloc / cudaFree, no context): for callers under CUDA graph capture,
+ * serving loops and harnesses that forbid allocation.  It computes what phmm_forward_batch(..., PHMM_FP64, ...) computes
+ * for SHORT-CLASS pairs only -- every pair's haplotype <= 1024 bases and read <= 4096 -- with default options (raw Phred
+ * qualities, literal N), in unscaled double (Eq.1-4 with C = 2^1000): the same kernel arithmetic as the library's fp64
+ * sub-warp kernel.  Its scratch (the quality tables and the row-constant table, 64 bytes per read row) is a file-scope
+ * device array of PHMM_NOALLOC_SCRATCH_BYTES that every GPU loading the library holds until exit; a batch fits if
+ * sum over reads of (length + 4) + 258 <= phmm_noalloc_limits()' max_table_entries (131008).
+ *   b             as for phmm_forward_batch: host offsets and pair lists (read for validation and sizing), device payload
+ *   d_read_off, d_hap_off, d_pair_read, d_pair_hap   device copies of b's four host arrays (the caller's, n+1 / n_pairs long)
+ *   d_out_log10   device, n_pairs doubles (written)
+ *   d_out_flags   device, n_pairs bytes (written; may be NULL): 0, or PHMM_FLAG_RANGE where L < 1e-290 * 2^-1000 (about
+ *                 10^-591: e.g. unrelated reads over ~600 bases) -- use phmm_forward_batch for such pairs
+ * Returns PHMM_E_TOOLONG, having launched nothing, if a sequence or the batch exceeds the limits above; validation errors
+ * as phmm_forward_batch.  Asynchronous on cuda_stream.  Every call shares the one scratch array: calls that overlap on
+ * the GPU (different streams without a dependency, or two processes' worth of threads) race -- serialise them.  The
+ * first call on a device does a one-time set-up (cudaGetSymbolAddress, a 4 KB synchronous copy); call
+ * phmm_noalloc_setup(device) beforehand where that must not happen inside the call (graph capture). */
+#define PHMM_NOALLOC_SCRATCH_BYTES (8u << 20)
+int phmm_noalloc_setup(int device);
+int phmm_noalloc_limits(int64_t* max_table_entries, int32_t* max_hap_len, int32_t* max_read_len);
+int phmm_forward_batch_noalloc(int device, const phmm_batch* b, const int64_t* d_read_off, const int64_t* d_hap_off,
+                               const int32_t* d_pair_read, const int32_t* d_pair_hap, double* d_out_log10,
+                               uint8_t* d_out_flags, void* cuda_stream);
 
 #ifdef __cplusplus
 }

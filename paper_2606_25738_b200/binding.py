@@ -19,10 +19,11 @@ PHMM_OK = 0
 PHMM_E_ARG, PHMM_E_OFFSETS, PHMM_E_EMPTY, PHMM_E_TOOLONG = -1, -2, -3, -4
 PHMM_E_CUDA, PHMM_E_NOMEM, PHMM_E_UNSUPPORTED = -5, -6, -7
 PHMM_FP32_RESCUE, PHMM_FP64 = 0, 1
-PHMM_FLAG_RESCUED, PHMM_FLAG_LONG = 1, 2
+PHMM_FLAG_RESCUED, PHMM_FLAG_LONG, PHMM_FLAG_RANGE = 1, 2, 4
 
 EXPORTS = ["phmm_create", "phmm_destroy", "phmm_forward_batch", "phmm_forward_batch_host", "phmm_get_stats",
-           "phmm_strerror", "phmm_last_cuda_error", "phmm_measure_peak", "phmm_plan_host", "phmm_plan_slices_host"]
+           "phmm_strerror", "phmm_last_cuda_error", "phmm_measure_peak", "phmm_plan_host", "phmm_plan_slices_host",
+           "phmm_noalloc_setup", "phmm_noalloc_limits", "phmm_forward_batch_noalloc"]
 
 
 class phmm_options(ctypes.Structure):
@@ -96,6 +97,12 @@ def lib() -> ctypes.CDLL:
         L.phmm_plan_host.argtypes = [ctypes.POINTER(phmm_batch), ctypes.c_int, ctypes.c_int, ctypes.c_void_p, ctypes.c_void_p,
                                      ctypes.c_int64, ctypes.c_void_p, ctypes.c_int64, ctypes.c_void_p, ctypes.c_int64]
         L.phmm_measure_peak.restype = ctypes.c_int
+        L.phmm_noalloc_setup.argtypes = [ctypes.c_int]
+        L.phmm_noalloc_setup.restype = ctypes.c_int
+        L.phmm_noalloc_limits.argtypes = [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p]
+        L.phmm_noalloc_limits.restype = ctypes.c_int
+        L.phmm_forward_batch_noalloc.argtypes = [ctypes.c_int, ctypes.POINTER(phmm_batch)] + [ctypes.c_void_p] * 7
+        L.phmm_forward_batch_noalloc.restype = ctypes.c_int
         L.phmm_plan_slices_host.restype = ctypes.c_int
         L.phmm_plan_slices_host.argtypes = [ctypes.POINTER(phmm_batch), ctypes.c_int64, ctypes.c_int, ctypes.c_void_p, ctypes.c_void_p,
                                             ctypes.c_void_p, ctypes.c_int64]
@@ -296,6 +303,39 @@ class Context:
         if rc != PHMM_OK:
             raise PhmmError(rc)
         return s.as_dict()
+
+
+def noalloc_limits():
+    """phmm_noalloc_limits: (max table entries, max haplotype length, max read length) of the no-alloc entry point."""
+    e = ctypes.c_int64(); k = ctypes.c_int32(); l = ctypes.c_int32()
+    lib().phmm_noalloc_limits(ctypes.byref(e), ctypes.byref(k), ctypes.byref(l))
+    return int(e.value), int(k.value), int(l.value)
+
+
+class NoAllocBatch:
+    """What phmm_forward_batch_noalloc takes besides a DeviceBatch: device copies of the offset arrays and of the pair list
+    (made here, once, by torch; the entry point itself allocates nothing)."""
+
+    def __init__(self, db: DeviceBatch):
+        import torch
+        self.db = db
+        up = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to(db.device)
+        self.d_read_off, self.d_hap_off = up(db.read_off), up(db.hap_off)
+        self.d_pair_read, self.d_pair_hap = up(db.pair_read), up(db.pair_hap)
+
+
+def forward_batch_noalloc(nb: NoAllocBatch, out, flags=None, stream=None, device: int = 0):
+    """phmm_forward_batch_noalloc into the caller's `out` (float64 cuda tensor, n_pairs) and `flags` (uint8, optional);
+    asynchronous on `stream` (default: torch's current stream)."""
+    import torch
+    st = torch.cuda.current_stream(nb.db.device) if stream is None else stream
+    cb = nb.db.c_struct()
+    ptr = lambda t: t.data_ptr() if t is not None and t.numel() else 0
+    rc = lib().phmm_forward_batch_noalloc(device, ctypes.byref(cb), ptr(nb.d_read_off), ptr(nb.d_hap_off), ptr(nb.d_pair_read),
+                                          ptr(nb.d_pair_hap), ptr(out), ptr(flags), st.cuda_stream)
+    if rc != PHMM_OK:
+        raise PhmmError(rc)
+    return out, flags
 
 
 def measure_peak(kind: int, device: int = 0, reps: int = 5) -> float:
