@@ -282,7 +282,13 @@ struct Stager {  // packs several host arrays into the pinned buffer and copies 
         CK(dst.need(bytes));
         const size_t at = (used + 255) & ~(size_t)255;
         if (at + bytes > stage->cap) return PHMM_E_NOMEM;
-        memcpy((char*)stage->p + at, src, bytes);
+        if (bytes >= ((size_t)8 << 20)) {  // (plans of millions of tasks: 100 MB and more)
+            char* d = (char*)stage->p + at;
+            const char* s0 = (const char*)src;
+            parallel_chunks((int64_t)bytes, 1 << 20, [&](int, int64_t lo, int64_t hi) { memcpy(d + lo, s0 + lo, (size_t)(hi - lo)); });
+        } else {
+            memcpy((char*)stage->p + at, src, bytes);
+        }
         used = at + bytes;
         CK(cudaMemcpyAsync(dst.p, (char*)stage->p + at, bytes, cudaMemcpyHostToDevice, st));
         return PHMM_OK;

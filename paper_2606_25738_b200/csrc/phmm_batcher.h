@@ -48,12 +48,22 @@ struct ShortPlan {
     int64_t cells = 0;              // real cells of the short pairs
     int64_t padded_cells = 0;       // lane-cells swept: sum over warps of steps * 32 lanes * columns-per-lane
     int max_read_len = 0;
+    // scratch of plan_tasks, kept between calls so that a steady stream of equal-sized batches touches no fresh memory
+    struct PackPart {
+        std::vector<ShortTask> tasks;   // in packing order
+        std::vector<int> warp_end;      // one past the last task of each warp
+        std::vector<int> warps_after;   // [c]: warps closed once the classes >= c are done
+        std::vector<int> tb, ids, bstart, avail;
+        int64_t padded = 0;
+    };
+    std::vector<ShortTask> tmp_tasks;
+    std::vector<ShortTask> tmp_cut[BATCHER_THREADS];
+    PackPart tmp_pack[BATCHER_THREADS];
 };
 
 // is_short[p] != 0 selects the pairs to plan.  cols_per_lane = 2*NV of the kernel.
 void plan_short(const HostBatchView& b, const uint8_t* is_short, int cols_per_lane, int task_rows, ShortPlan* out);
 // The three stages of plan_short, for batches that are processed in slices of reads (phmm_api.cu):
-void sort_pairs_by_hap(const HostBatchView& b, const uint8_t* is_short, std::vector<int>* sorted);
 int slice_reads(const HostBatchView& b, int64_t max_table_bytes, int min_slices, std::vector<int64_t>* bound);
 void bucket_pairs_by_slice(const HostBatchView& b, const uint8_t* read_slice, int n_slices, std::vector<int>* out,
                            std::vector<int64_t>* slice_first);

@@ -47,6 +47,38 @@ def test_plan_mixed_unsorted_stream_and_long_pairs_left_out():
     assert len(p["sorted_pair"]) < b.n_pairs  # some haplotypes exceed 1024 and go to the chain path
 
 
+def test_plan_many_haplotypes_shuffled_and_grouped():
+    """The three ways the batcher sorts pairs by haplotype (csrc/phmm_batcher.cpp, sort_ids_by_hap): a list that is grouped
+    already (copied), many more haplotypes than pairs per thread (radix sort), else per-thread histograms; and the packing of
+    many equal one-pair tasks (whole warps at once, several threads, merged class by class): same invariants for all."""
+    rng = np.random.default_rng(3)
+    n_h, n_r = 300_000, 1000
+    hap_len = rng.integers(20, 90, n_h)
+    read_len = rng.integers(10, 60, n_r)
+    ho = np.concatenate([[0], np.cumsum(hap_len)]).astype(np.int64)
+    ro = np.concatenate([[0], np.cumsum(read_len)]).astype(np.int64)
+    z = np.zeros(int(ro[-1]), dtype=np.uint8)
+    pair_hap = rng.choice(n_h, 40_000, replace=False).astype(np.int32)
+    pair_hap = np.concatenate([pair_hap, pair_hap[:5000]])          # some haplotypes twice
+    pair_read = rng.integers(0, n_r, len(pair_hap)).astype(np.int32)
+    b = W.Batch(ro, ho, z, z, z, z, z, np.zeros(int(ho[-1]), dtype=np.uint8), pair_read, pair_hap)
+    p = B.plan_host(b)                                                # shuffled, 300 000 haplotypes for 45 000 pairs: radix
+    _check_plan(b, p)
+    order = np.argsort(pair_hap, kind="stable")
+    g = b.select_pairs(order)                                         # grouped already
+    pg = B.plan_host(g)
+    _check_plan(g, pg)
+    assert np.array_equal(order[pg["sorted_pair"]], p["sorted_pair"])  # the same stable order either way
+    # equal tasks: every pair its own haplotype of 32 bases -> one class, one lane count, whole warps of 32 tasks
+    n = 70_000
+    e = W.Batch(np.arange(n + 1, dtype=np.int64) * 32, np.arange(n + 1, dtype=np.int64) * 32, np.zeros(n * 32, np.uint8),
+                np.zeros(n * 32, np.uint8), np.zeros(n * 32, np.uint8), np.zeros(n * 32, np.uint8), np.zeros(n * 32, np.uint8),
+                np.zeros(n * 32, np.uint8), np.arange(n, dtype=np.int32), np.arange(n, dtype=np.int32))
+    pe = B.plan_host(e)
+    _check_plan(e, pe)
+    assert pe["n_warps"] <= -(-n // 32) + 16
+
+
 def test_plan_custom_cut_and_small_tasks():
     b = W.generate(1, n=2)
     p = B.plan_host(b, long_min_hap_len=300, task_rows=500)
