@@ -162,6 +162,8 @@ int phmm_forward_batch(phmm_ctx* ctx, const phmm_batch* b, int precision, double
 int phmm_forward_batch_host(phmm_ctx* ctx, const phmm_batch* b, int precision, double* h_out_log10,
                             uint8_t* h_out_flags);
 
+/* Statistics of the most recent call on the context.  Waits for that call's device work to complete (the rescue count and
+ * the per-family times are only known then), on whatever stream the call was issued. */
 int phmm_get_stats(phmm_ctx* ctx, phmm_stats* out);
 const char* phmm_strerror(int code);
 /* cudaError_t value of the last failing CUDA call on this context (0 if none). */

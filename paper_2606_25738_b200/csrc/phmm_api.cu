@@ -196,8 +196,9 @@ extern "C" int phmm_destroy(phmm_ctx* ctx) {
 
 extern "C" int phmm_get_stats(phmm_ctx* ctx, phmm_stats* out) {
     if (!ctx || !out) return PHMM_E_ARG;
-    if (!ctx->stats_final && ctx->d_acc.p && ctx->stats.n_pairs > 0) {  // the rescue count lives on the device until the caller has synchronised
+    if (!ctx->stats_final && ctx->d_acc.p && ctx->stats.n_pairs > 0) {  // the rescue count lives on the device until the call has completed
         DeviceGuard guard(ctx->device);
+        if (ctx->ev_last) cudaEventSynchronize(ctx->ev_last);  // (the end of the call's device work, whatever stream it ran on)
         long long acc[2] = {0, 0};
         if (cudaMemcpy(acc, ctx->d_acc.p, sizeof(acc), cudaMemcpyDeviceToHost) == cudaSuccess) ctx->stats.n_rescued = (int64_t)acc[0];
     }
@@ -641,6 +642,7 @@ static int run_slice(phmm_ctx* ctx, const phmm_batch* b, const HostBatchView& hv
             CK(ctx->d_totals.need((size_t)n_prog * 16 + 16));
             CK(ctx->d_risk.need((size_t)b->n_reads + 16));
             CK(launch_read_risk(db, ctx->opt.qual_offset, sw.r0, sw.r1, (uint8_t*)ctx->d_risk.p, st));
+            launches++;
             LongLaunch ll;
             memset(&ll, 0, sizeof(ll));
             ll.table = (const float*)ctx->d_table.p;
@@ -728,6 +730,7 @@ static int run_slice(phmm_ctx* ctx, const phmm_batch* b, const HostBatchView& hv
     if (!fp64 && (n_warps > 0 || long32)) {  // pairs recomputed in fp64 so far (phmm_get_stats)
         k_accumulate_rescued<<<1, 1, 0, st>>>((long long*)ctx->d_acc.p, counters, (const int*)ctx->d_rq.p);
         CK(cudaGetLastError());
+        launches++;
     }
     ctx->stats.n_kernel_launches += launches;
     return PHMM_OK;
