@@ -167,8 +167,8 @@ k_chain(DevBatch b, ChainLaunch p, int items_are_pairs) {
         const int l = (int)(b.read_off[r + 1] - ro), k = (int)(b.hap_off[h + 1] - ho);
         const int n_ent = l + CHAIN_EXTRA_ROWS;  // run-in entry, rows 1..l, sum entry, flush entry
         const int nstrips = (k + 32 * N2 - 1) / (32 * N2);
-        // The lane that holds the haplotype's last column, in the last strip: Eq.4 is taken there, and nothing flows into the
-        // lanes behind it.  (Until round 2 the sum travelled on to lane 31 through lanes that hold only padding columns; what
+        // The lane that holds the haplotype's last column, in the last strip: Eq.4 is taken there; the lanes behind it hold only
+        // padding columns and feed nothing.  (Until round 2 the sum travelled on to lane 31 through lanes that hold only padding columns; what
         // circulates there -- mismatch diagonals that never run out of columns -- can decay more slowly than the real cells,
         // where every further read base has to be an insertion, and the sum, converted from lane to lane to ever larger
         // exponents, vanished: -inf for a 535-base read against a 2-base haplotype at GCP 40.  Found by fuzzing.)
@@ -196,6 +196,8 @@ k_chain(DevBatch b, ChainLaunch p, int items_are_pairs) {
                 outprog = p.progress + prog0 + st;
             }
             const bool has_in = st > 0, has_out = st + 1 < nstrips;
+            // the step at which the .y half of the haplotype's last lane processes the sum entry (entry l + 1): e = s - 2 lane - 1
+            const int out_step = (!has_out && lane == out_lane) ? l + 2 + 2 * lane : -1;
 
             L ln;
             ln.init();
@@ -299,7 +301,6 @@ k_chain(DevBatch b, ChainLaunch p, int items_are_pairs) {
                         exL = 0;
                     }
                 }
-                if (!has_out && lane > out_lane) { inS = (T)0; inT = (T)0; }  // lanes of padding columns only stay empty
                 // ---- bring the incoming values to this thread's exponent (exact power-of-two multiply)
                 {
                     const T mi = Fx<T>::fmax_(inS, inT);
@@ -342,7 +343,7 @@ k_chain(DevBatch b, ChainLaunch p, int items_are_pairs) {
                         }
                     }
                 }
-                if (!has_out && lane == out_lane && (E.metaY & META_SUM)) {  // the sum entry: s has collected Eq.4; log10 in double
+                if (s == out_step) {  // this lane's .y half has just done the sum entry: s has collected Eq.4; log10 in double
                     // M+I of column j reaches the chain through the T of column j+1; a haplotype that fills its last
                     // lane has the last one in what this lane handed out one step ago instead
                     const T sum = full_last ? ln.outS.y + prevT : ln.outS.y;

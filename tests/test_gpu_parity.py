@@ -568,6 +568,25 @@ def test_options_qual_offset_and_floor(B):
         c.close()
 
 
+def test_pair_dump_through_the_library(B, ctx, tmp_path):
+    """A pair dump in the text format of paper_2606_25738_b200/pairs_text.py (ASCII+33 qualities) through the library both
+    ways -- decoded by the adaptor, or taken as it is by a context with qual_offset = 33 -- against the oracle."""
+    from paper_2606_25738_b200 import pairs_text
+    src = W.generate(2, n=300)
+    path = str(tmp_path / "dump.txt")
+    pairs_text.write_pairs(path, src)
+    b = pairs_text.read_pairs(path)
+    ref = oracle.forward_batch(src)
+    out, fl = run(B, ctx, b, B.PHMM_FP32_RESCUE)
+    assert np.max(np.abs(out - ref)) <= TOL32
+    c = B.Context(0, qual_offset=33, validate=1)
+    try:
+        out2, fl2 = run(B, c, pairs_text.read_pairs(path, decode=False), B.PHMM_FP32_RESCUE)
+        assert np.array_equal(out2, out) and np.array_equal(fl2, fl)
+    finally:
+        c.close()
+
+
 def test_option_validate_rejects_bad_payloads(B):
     """phmm_options.validate: a byte outside ACGTN, a quality below the offset, or iota + delta >= 1 make the call return
     PHMM_E_ARG before anything is launched: outputs untouched.  A clean batch passes and gives the usual result."""

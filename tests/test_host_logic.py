@@ -145,3 +145,25 @@ def test_slices_of_reads_respect_the_table_budget():
             assert ns > 1 and np.all(entries * 64 <= budget + 64 * (rl.max() + 5))
         else:
             assert ns == max(1, min_slices)
+
+
+def test_pair_dump_text_adaptor_round_trip(tmp_path):
+    """paper_2606_25738_b200/pairs_text.py: write a seeded batch as a six-column pair dump with ASCII+33
+    qualities, read it back: the same pairs (sequences and qualities, pair by pair), shared reads / haplotypes stored once;
+    decode=False keeps the encoded bytes; malformed lines are refused."""
+    from paper_2606_25738_b200 import pairs_text
+    b = W.generate(1, n=1)  # 128 reads x 8 haplotypes, 1024 pairs
+    path = str(tmp_path / "pairs.txt")
+    pairs_text.write_pairs(path, b)
+    r = pairs_text.read_pairs(path)
+    assert r.n_pairs == b.n_pairs and r.n_reads <= b.n_reads and r.n_haps <= b.n_haps
+    for p in (0, 1, 7, 500, b.n_pairs - 1):
+        for x, y in zip(b.pair(p), r.pair(p)):
+            assert np.array_equal(x, y)
+    assert r.cells() == b.cells()
+    e = pairs_text.read_pairs(path, decode=False)
+    assert np.array_equal(e.qual_base, r.qual_base + 33) and np.array_equal(e.qual_gcp, r.qual_gcp + 33)
+    with open(path, "ab") as f:
+        f.write(b"# a comment\n\nACGT ACG III III III\n")
+    with pytest.raises(ValueError):
+        pairs_text.read_pairs(path)
