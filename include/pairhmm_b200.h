@@ -68,7 +68,9 @@ typedef struct phmm_options {
      * < 2^rescue_log2_threshold.  Default -90  (<=> L < 2^-210 ~ 10^-63.2). */
     int32_t rescue_log2_threshold;
     /* haplotypes longer than this many bases (or reads longer than 4096) use the long, rescaled multi-strip path;
-     * default and maximum 1024 (= 32 lanes x 32 columns, what one warp of the short kernel covers) */
+     * default and maximum 1024 (= 32 lanes x 32 columns, what one warp of the short kernel covers).  In PHMM_FP32_RESCUE
+     * pairs with a haplotype over 7/8 of it and a read of 768 bases or more take that path too (as one strip): such reads
+     * increasingly underflow the unrescaled fp32 kernel.  Either way the pair carries PHMM_FLAG_LONG. */
     int32_t long_min_hap_len;
     /* target number of read rows per short-path task (a task streams several reads of one
      * haplotype through one lane group); 0 = chosen per batch between 1024 and 8192 so that the
@@ -176,8 +178,8 @@ int phmm_last_cuda_error(phmm_ctx* ctx);
 int phmm_measure_peak(int device, int kind, int reps, double* out_tflops);
 
 /* Host batcher only (no device is touched): the work plan the short path
- * would use for the pairs of `b` with haplotype length <= long_min_hap_len (0 = default 1024) and read
- * length <= 4096.  Only the host arrays of `b` are read (offsets, pair list).  Outputs, all host, caller-owned:
+ * would use for the short-class pairs of `b` in PHMM_FP32_RESCUE: haplotype length <= long_min_hap_len (0 = default 1024), read
+ * length <= 4096, and not both haplotype > 7/8 of the cut and read >= 768 (phmm_options.long_min_hap_len).  Only the host arrays of `b` are read (offsets, pair list).  Outputs, all host, caller-owned:
  *   plan_counts[4]   = { n_warps, n_tasks, n_sorted_pairs, columns per lane }
  *   warp_first       n_warps + 1 ints: first task of each warp              (capacity cap_warps + 1)
  *   tasks            4 ints per task: haplotype, first sorted pair, number of pairs, read rows (capacity 4 * cap_tasks)

@@ -229,7 +229,7 @@ extern "C" int phmm_plan_host(const phmm_batch* b, int long_min_hap_len, int tas
     for (int64_t p = 0; p < b->n_pairs; p++) {
         const int r = b->h_pair_read[p], h = b->h_pair_hap[p];
         const int64_t l = b->h_read_off[r + 1] - b->h_read_off[r], k = b->h_hap_off[h + 1] - b->h_hap_off[h];
-        is_short[(size_t)p] = !(k > long_min_hap_len || l > 4096);
+        is_short[(size_t)p] = !long_class(k, l, long_min_hap_len, long_min_hap_len * 7 / 8);  // (the PHMM_FP32_RESCUE classification)
     }
     ShortPlan pl;
     plan_short(hv, is_short.data(), SHORT_N2, task_rows, &pl);
@@ -430,6 +430,7 @@ static int run_slice(phmm_ctx* ctx, const phmm_batch* b, const HostBatchView& hv
         struct Part { std::vector<int> seq, strip, sub, sh; int64_t cells = 0, lane_rows = 0; int max_l = 0, max_l_long = 0; };
         Part part[BATCHER_THREADS];
         const int long_k = ctx->opt.long_min_hap_len;
+        const int tall_k = fp64 ? 0 : long_k * 7 / 8;  // (phmm_kernels.h, long_class)
         const int* ids = sw.ids;
         const int T = parallel_chunks(np_slice, 1 << 16, [&](int t, int64_t lo, int64_t hi) {
             Part& q = part[t];
@@ -438,7 +439,7 @@ static int run_slice(phmm_ctx* ctx, const phmm_batch* b, const HostBatchView& hv
                 const int r = b->h_pair_read[p], h = b->h_pair_hap[p];
                 const int64_t l = b->h_read_off[r + 1] - b->h_read_off[r], k = b->h_hap_off[h + 1] - b->h_hap_off[h];
                 q.cells += l * k;
-                if (k > long_k || l > 4096) { q.strip.push_back(p); if (l > q.max_l_long) q.max_l_long = (int)l; }
+                if (long_class(k, l, long_k, tall_k)) { q.strip.push_back(p); if (l > q.max_l_long) q.max_l_long = (int)l; }
                 else {
                     if (fp64 && k <= RESCUE_MAX_K && l <= RESCUE_MAX_L) q.sub.push_back(p);
                     else if (fp64) q.seq.push_back(p);
@@ -721,6 +722,7 @@ static int run_slice(phmm_ctx* ctx, const phmm_batch* b, const HostBatchView& hv
         cl.flags = d_flags;
         cl.flag_bits = fp64 ? 0 : PHMM_FLAG_RESCUED;
         cl.long_k = ctx->opt.long_min_hap_len;
+        cl.tall_k = fp64 ? 0 : ctx->opt.long_min_hap_len * 7 / 8;
         cl.log2C = 0;
         if (!sub) PROF(2, 0);
         CK(launch_chain(db, cl, true, true, grid, st));

@@ -348,7 +348,7 @@ k_chain(DevBatch b, ChainLaunch p, int items_are_pairs) {
                     // lane has the last one in what this lane handed out one step ago instead
                     const T sum = full_last ? ln.outS.y + prevT : ln.outS.y;
                     p.out[pair] = log10((double)sum) + ((double)ex - (double)p.log2C) * LOG10_2;
-                    if (p.flags) p.flags[pair] = p.flag_bits | ((items_are_pairs && (k > p.long_k || l > 4096)) ? 2u /* PHMM_FLAG_LONG */ : 0u);
+                    if (p.flags) p.flags[pair] = p.flag_bits | ((items_are_pairs && long_class(k, l, p.long_k, p.tall_k)) ? 2u /* PHMM_FLAG_LONG */ : 0u);
                 }
             }
             __syncwarp();

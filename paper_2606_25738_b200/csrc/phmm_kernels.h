@@ -33,6 +33,15 @@ inline __host__ __device__ int table_run_len(int l) { return (l + TABLE_EXTRA_RO
 static_assert(TABLE_ZERO_RUN % 2 == 0, "idle lanes walk the zero run two entries per loop iteration");
 constexpr int CHAIN_EXTRA_ROWS = 3;       // chain kernel: the same stream
 
+// PHMM_FP32_RESCUE: short-class pairs whose haplotype nearly fills a strip of the long kernel (> 7/8 of the short/long cut) and
+// whose read has this many rows or more go through the long kernel as one-strip items: a related read loses 0.2-0.8 bits per
+// row, so from here on a growing share would underflow the unrescaled fp32 kernel and be recomputed in fp64 (27 % of the
+// 1024 x 1024 pairs of the paper's sweep shape), while a full strip of the long kernel runs at its full rate and never underflows.
+constexpr int TALL_MIN_ROWS = 768;
+inline __host__ __device__ bool long_class(int64_t k, int64_t l, int long_k, int tall_k) {
+    return k > long_k || l > 4096 || (tall_k > 0 && k > tall_k && l >= TALL_MIN_ROWS);
+}
+
 struct DevBatch {  // device mirrors of the batch
     const uint8_t *read_bases, *qual_base, *qual_ins, *qual_del, *qual_gcp, *hap_bases;
     const int64_t *read_off, *hap_off;  // device copies of the host offset arrays
@@ -116,6 +125,7 @@ struct ChainLaunch {
     uint8_t flag_bits;         // written to flags[pair]
     int log2C;                 // scale constant C = 2^log2C of Eq.1 (0 for the rescaled kernels)
     int long_k;                // items_are_pairs: pairs with a haplotype longer than this (or a read over 4096) also get PHMM_FLAG_LONG
+    int tall_k;                // ... and so do pairs with a haplotype longer than this and a read of TALL_MIN_ROWS or more (0: rule off)
 };
 
 struct LongLaunch {  // fp32 long path (phmm_long.cu): strips of 32 lanes x 32 columns, table-driven like the short kernel

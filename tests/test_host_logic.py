@@ -15,7 +15,7 @@ def _check_plan(b, plan, long_min=1024):
     rl, hl = b.read_len(), b.hap_len()
     N2 = plan["cols_per_lane"]
     k = hl[b.pair_hap]; l = rl[b.pair_read]
-    is_short = (k <= long_min) & (l <= 4096)
+    is_short = (k <= long_min) & (l <= 4096) & ~((k > long_min * 7 // 8) & (l >= 768))
     # every short pair exactly once, no long pair
     assert sorted(plan["sorted_pair"].tolist()) == np.where(is_short)[0].tolist()
     wf, tk, sp = plan["warp_first"], plan["tasks"], plan["sorted_pair"]
