@@ -377,27 +377,38 @@ def test_randomized_batches_against_oracle(B, ctx):
     """Seeded random batches of every shape the entry points accept -- haplotypes of 1..6000 bases (tile-boundary lengths
     over-represented), reads of 1..3000, related / unrelated / with gaps, N bases, constant and per-base qualities with GCP
     between 3 and 40 -- through both precisions, one and many slices, and the host entry, element-wise against the oracle.
-    Where PHMM_FP64 and the C oracle disagree the log-space companion (oracle/logspace.py) arbitrates: with GCP qualities
-    near 40 single rows lose more than the 2^-1074 the oracle keeps below a row's maximum (its documented limit).
+    For reads of 300 rows or more (100 with a GCP quality above 20) the log-space companion (oracle/logspace.py) is
+    computed too and replaces the C oracle's value where they differ: the C oracle flushes cells 2^-1074 below a row's
+    maximum (its documented limit), and on such reads a flushed cell can become the dominant one later.  That is decided from
+    the two CPU implementations alone.
     This loop, run for minutes, found: -inf from the fp64 chain kernel for long reads against very short haplotypes at
     GCP 40 (padding lanes), and silent errors of up to 0.6 in the fp32 long kernel for GCP above 10 (now guarded)."""
     from oracle import logspace
     cs = B.Context(0, max_table_bytes=4 << 20)
     n_arb = n_long = n_fb = 0
     try:
-        for it in range(36):
+        for it in range(24):
             rng = np.random.default_rng(7000 + it)
             kind = it % 3
             b = _fz_make(rng, [400, 60, 12][kind], [400, 1500, 6000][kind], [300, 700, 3000][kind])
             ref = oracle.forward_batch(b)
+            # the C oracle keeps 1074 bits below a row's maximum (its documented limit).  A cell that far down can still matter later:
+            # a read whose matching stretch runs off the haplotype's end pays a gap continuation per row from there on (3.3 bits at
+            # GCP 10, 13 at GCP 40), the unrelated background about 2.5 -- after some hundred rows the background wins.  For
+            # reads long enough for that the log-space companion is computed as well and takes over where the two differ
+            # (decided on the CPU, before anything runs on the GPU)
+            gmax = np.maximum.reduceat(b.qual_gcp, b.read_off[:-1])
+            lp = b.read_len()[b.pair_read]
+            for i in np.where((lp >= 300) | ((gmax[b.pair_read] > 20) & (lp >= 100)))[0]:  # (1074 bits take > 80 rows at GCP 40, > 320 at GCP 10)
+                pp = b.pair(i)
+                ls = logspace.log10_likelihood(pp[0], pp[5], pp[1], pp[2], pp[3], pp[4])
+                if abs(ls - ref[i]) > 1e-10:
+                    ref[i] = ls
+                    n_arb += 1
             db = B.DeviceBatch(b)
             o64, _ = ctx.forward_batch(db, B.PHMM_FP64)
             o64 = o64.cpu().numpy()
-            for i in np.where(~(np.abs(o64 - ref) <= TOL64))[0]:
-                pp = b.pair(i)
-                ref[i] = logspace.log10_likelihood(pp[0], pp[5], pp[1], pp[2], pp[3], pp[4])
-                n_arb += 1
-            assert np.all(np.abs(o64 - ref) <= TOL64), "seed %d fp64" % (7000 + it)
+            assert np.all(np.abs(o64 - ref) <= TOL64), "seed %d fp64: max err %g" % (7000 + it, np.nanmax(np.abs(o64 - ref)))
             for c in (ctx, cs):
                 o, f = c.forward_batch(db, B.PHMM_FP32_RESCUE)
                 o, f = o.cpu().numpy(), f.cpu().numpy()
@@ -409,7 +420,7 @@ def test_randomized_batches_against_oracle(B, ctx):
     finally:
         cs.close()
     print("randomized: %d long pairs, %d of them handed to fp64, %d arbitrations by the log-space companion" % (n_long, n_fb, n_arb))
-    assert n_long > 200 and n_fb < n_long
+    assert n_long > 150 and n_fb < n_long
 
 
 # ------------------------------------------------------------------ edge cases
