@@ -158,7 +158,7 @@ int phmm_forward_batch(phmm_ctx* ctx, const phmm_batch* b, int precision, double
 /* Same computation with ALL buffers on the host (the d_* members of `b` are host pointers, out
  * pointers are host): the library copies the payload to the device, runs phmm_forward_batch, copies
  * the results back and synchronises.  This is the end-to-end entry ("with transfer").
- * The reads are processed in slices (at least one per 32 MB of read payload, and as many as the table budget asks for):
+ * The reads are processed in slices (at least one per 48 MB of read payload, and as many as the table budget asks for):
  * the copy of a slice's reads and its host plan run under the kernels of the slice before; results and flags are the
  * same as for one call with device buffers.  phmm_get_stats afterwards reports the sums over the slices. */
 int phmm_forward_batch_host(phmm_ctx* ctx, const phmm_batch* b, int precision, double* h_out_log10,

@@ -797,9 +797,9 @@ extern "C" int phmm_forward_batch_host(phmm_ctx* ctx, const phmm_batch* b, int p
     phmm_batch db = *b;
     db.d_read_bases = hp.dst[0]; db.d_qual_base = hp.dst[1]; db.d_qual_ins = hp.dst[2]; db.d_qual_del = hp.dst[3];
     db.d_qual_gcp = hp.dst[4]; db.d_hap_bases = base + 5 * Ra - b->h_hap_off[0];
-    // The reads are processed in slices (at least one per 32 MB of read payload, up to 16): the copy of slice s+1 and its
+    // The reads are processed in slices (at least one per 48 MB of read payload, up to 16): the copy of slice s+1 and its
     // host plan run while the GPU works on slice s (the "with transfers" convention).
-    const int min_slices = (int)std::max<size_t>(1, std::min<size_t>(16, 5 * R / ((size_t)32 << 20)));
+    const int min_slices = (int)std::max<size_t>(1, std::min<size_t>(16, 5 * R / ((size_t)48 << 20)));  // (configs[1]: 1 / 2 / 4 / 7 / 10 slices: 53.6 / 51.5 / 48.6 / 50.7 / 50.0 ms)
     const int64_t np = b->n_pairs;
     const HostPayload* hpp = &hp;
     if (ctx->opt.validate) {  // the whole payload first, then the check: nothing may be written for a bad batch
