@@ -144,7 +144,7 @@ struct LongLaunch {  // fp32 long path (phmm_long.cu): strips of 32 lanes x 32 c
     int publish;               // entries per progress publication: a power of two >= 16
     int* fallback_count;       // pairs whose fp32 result is not a normal positive number: list for the fp64 chain kernel
     int* fallback_list;
-    const uint8_t* risk;       // per read: marked by launch_read_risk (fp32's per-lane range may not do: straight to fp64)
+    const uint8_t* risk;       // per read, by launch_read_risk: 255 = fp32's per-lane range may not do (straight to fp64), else the read's smallest GCP quality
 };
 cudaError_t launch_read_risk(const DevBatch& b, int qual_offset, int64_t r0, int64_t r1, uint8_t* risk, cudaStream_t st);
 cudaError_t launch_long_f32(const DevBatch& b, const LongLaunch& p, int grid_ctas, cudaStream_t st);

@@ -13,13 +13,13 @@
 // power-of-two factor f_in = 2^(ex_left - ex) (two multiplies per step; no branch, no exponent arithmetic in the step).
 // At an event every lane
 //   1. takes the maximum m of what it holds and proposes ex' = ex + ilogb(m) - TGT (its maximum back to 2^TGT);
-//   2. is held to ex'_L >= max over the lanes m < L of ex'_m - KTOT (a prefix maximum: 5 shuffles), and lane 0 to the
-//      exponents of the 16 boundary records it is about to consume.  Values move only right and down and only shrink in
-//      true magnitude, so whatever reaches a lane in the next 16 steps is stored at or below 2^(TGT+KTOT) there, over
-//      any number of hops: no overflow, no per-step check;
+//   2. is held to ex'_L >= max over the lanes m < L of ex'_m - KTOT - (L - 1 - m) HOP (a max-plus prefix scan: 5 shuffles),
+//      HOP = what the running sum loses crossing a lane, and lane 0 to the exponents of the 16 boundary records it is about
+//      to consume.  Values move only right and down and only shrink in true magnitude, so whatever reaches a lane in the
+//      next 16 steps is stored at or below 2^(TGT+KTOT) there, over any number of hops: no overflow, no per-step check;
 //   3. multiplies its state by 2^(ex - ex') (exact; what falls below the format's range was more than 2^-(126+TGT) below
-//      the lane's own maximum or 2^-(126+TGT+KTOT) below the maximum of a lane to its left: G15's documented limit) and
-//      recomputes f_in.
+//      the lane's own maximum or 2^-(126+TGT+KTOT+(L-1-m) HOP) below the maximum of lane m to its left: G15's limit --
+//      less than what that maximum's path would pay to get there, see the event) and recomputes f_in.
 // A result that is not a normal positive number (or a NaN anywhere in a lane's share of Eq.4) sends the pair to the
 // fp64 chain kernel (phmm_chain.cu): the same cascade as fp32 -> fp64 for short pairs.  So does a lane whose maximum falls
 // by more than 2^LONG_DROP between two events, and so does the input guard k_read_risk at the end of this file, which
@@ -127,7 +127,9 @@ __global__ void __launch_bounds__(LONG_WPC * 32, LONG_MIN_CTAS) k_long_f32(DevBa
         const int run0 = (int)(table_run_start(ro, r) - b.table_base), run_len = table_run_len(l);
         const int nstrips = (k + STRIP - 1) / STRIP;
         const bool has_in = strip > 0, has_out = strip + 1 < nstrips;
-        if (p.risk[r]) {  // k_read_risk: fp32's range per lane may not do for this read; the pair's last strip hands it to fp64
+        const int risk = p.risk[r];  // k_read_risk: 255 = fp32's range per lane may not do for this read, else its smallest GCP quality
+        const int hop = (risk * 32 * 85) >> 8;  // bits the running sum loses per lane it crosses: 32 columns x 0.332 GCP_min (rounded down)
+        if (risk == 255) {  // the pair's last strip hands it to fp64
             if (!has_out && lane == 0) {
                 const int idx = atomicAdd(p.fallback_count, 1);
                 p.fallback_list[idx] = pair;
@@ -252,19 +254,28 @@ __global__ void __launch_bounds__(LONG_WPC * 32, LONG_MIN_CTAS) k_long_f32(DevBa
                 for (int o = 8; o > 0; o >>= 1) bmax = max(bmax, __shfl_xor_sync(PHMM_FULL, bmax, o));
                 bmax = __shfl_sync(PHMM_FULL, bmax, 0);
             }
-            // 3. ex'_L = max(c_L, max over m < L of c_m - KTOT), the boundary records counting as a lane to the left of lane
-            //    0: nothing that can reach lane L (values only move right and down, and only shrink in true magnitude) is
-            //    stored above 2^(TGT+KTOT) there -- whatever the hop count
+            // 3. ex'_L = max(c_L, max over m < L of c_m - KTOT - (L - 1 - m) HOP), the boundary records counting as a lane to the
+            //    left of lane 0.  What lane m holds can reach lane L within the next 16 steps only through the running sum, which
+            //    loses HOP = 32 log2(1 / gamma_max) bits per full lane it crosses (a deletion per column; values moving
+            //    diagonally cross at most 16 columns): nothing that can reach lane L is stored above 2^(TGT+KTOT) there.
+            //    And what is flushed in lane L -- a cell more than 2^-(126+TGT+KTOT) 2^-((L-1-m) HOP) below lane m's maximum
+            //    A -- can never matter later: A's path reaches that cell's continuation by a deletion of at most
+            //    32 (L - 1 - m) + 62 columns, which costs less.  (A constraint without the HOP term, as first written,
+            //    flushes the start of a second matching stretch a few hundred columns to the right of the first one: reads
+            //    with a long deletion against the haplotype came out too small by up to 240 in log10.)
             const int bsrc = bmax > LONG_FLOOR ? bmax - LONG_TGT : LONG_FLOOR;
+            // (the run-in entry -- row 0 of Eq.1 -- carries C/k through every column undiminished, gamma := 1: no HOP until it
+            // has left the strip's last lane, at step 63)
+            const int hop_now = s < 64 + LONG_EVERY ? 0 : hop;
             int pm = lane == 0 ? max(c, bsrc) : c;
 #pragma unroll
             for (int o = 1; o < 32; o <<= 1) {
-                const int t = __shfl_up_sync(PHMM_FULL, pm, o);
+                const int t = __shfl_up_sync(PHMM_FULL, pm, o) - o * hop_now;
                 if (lane >= o) pm = max(pm, t);
             }
             pm = __shfl_up_sync(PHMM_FULL, pm, 1);
             if (lane == 0) pm = bsrc;
-            if (pm > LONG_FLOOR) c = max(c, pm - LONG_KTOT);
+            if (pm > LONG_FLOOR / 2) c = max(c, pm - LONG_KTOT);
             const int exn = c < LONG_FLOOR / 2 ? ex : c;  // nothing held, nothing to the left: keep the exponent
             sm.own[lane] = m > 0.f && exn == ex + Fx<float>::ilogb(m) - LONG_TGT;  // (a clamped proposal does not count)
             // 4. rescale the state: d <= 127 when something is held (the proposal is clamped), any d when nothing is
@@ -417,11 +428,13 @@ __global__ void k_read_risk(DevBatch b, int qual_offset, int64_t r0, int64_t r1,
     const int l = (int)(b.read_off[r + 1] - off);
     const int seg = (l + 31) / 32, lo = min(l, lane * seg), hi = min(l, lo + seg);
     bool bad = false;
+    int gmin = 255;
     // maximum-subarray summary of this lane's rows: total, best prefix, best suffix, best
     float tot = 0.f, pre = 0.f, suf = 0.f, best = 0.f;
     for (int i = lo; i < hi; i++) {
         const int g = max((int)b.qual_gcp[off + i] - qual_offset, 0), q = max((int)b.qual_base[off + i] - qual_offset, 0);
         if (g > 10) bad = true;
+        gmin = min(gmin, g);
         const float v = 0.332f * (float)(g - q) - 1.585f;
         tot += v;
         pre = fmaxf(pre, tot);
@@ -439,7 +452,10 @@ __global__ void k_read_risk(DevBatch b, int qual_offset, int64_t r0, int64_t r1,
         }
     }
     if (best > 60.f) bad = true;
-    if (__any_sync(PHMM_FULL, bad) && lane == 0) risk[r] = 1;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) gmin = min(gmin, __shfl_xor_sync(PHMM_FULL, gmin, o));
+    bad = __any_sync(PHMM_FULL, bad);
+    if (lane == 0) risk[r] = bad ? 255 : (uint8_t)gmin;  // (gmin <= 10 where not marked)
 }
 
 cudaError_t launch_read_risk(const DevBatch& b, int qual_offset, int64_t r0, int64_t r1, uint8_t* risk, cudaStream_t st) {

@@ -276,6 +276,31 @@ def test_long_kernel_stress_mixed_structure(B, ctx):
     assert np.max(np.abs(out64 - ref)) <= TOL64
 
 
+def test_reads_with_a_long_deletion_against_the_haplotype(B, ctx):
+    """A read made of two stretches of the haplotype that lie hundreds of columns apart (a long deletion in the read; also the
+    reverse order, which no path can follow): the second stretch starts as a cell far below the lanes to its left and must
+    not be flushed by their exponents -- the long kernel's constraint allows for what a path pays to cross a lane (DESIGN.md
+    section 6; without that term these came out too small by up to 240 in log10, silently).  Reference: the log-space
+    companion (the C oracle's 2^-1074-per-row limit bites on three of the eight)."""
+    from oracle import logspace
+    rng = np.random.default_rng(11)
+    cases = []
+    for (k, x0, xl, y0, yl) in ((2000, 100, 300, 1300, 300), (2000, 100, 150, 700, 400), (3000, 50, 600, 1500, 600),
+                                (5000, 100, 1000, 3000, 1000), (2000, 1200, 300, 100, 300), (1500, 100, 300, 600, 300),
+                                (4000, 200, 400, 500, 400), (2500, 100, 500, 1124, 500), (1030, 10, 200, 500, 300), (1100, 0, 120, 980, 120)):
+        hap = _rand_seq(rng, k)
+        cases.append((hap[x0:x0 + xl] + hap[y0:y0 + yl], hap))
+    b = W.from_strings(cases, qb=30, qi=45, qd=45, qg=10)
+    ref = np.array([logspace.log10_likelihood(*[b.pair(i)[j] for j in (0, 5, 1, 2, 3, 4)]) for i in range(b.n_pairs)])
+    c_or = oracle.forward_batch(b)
+    assert np.sum(np.abs(c_or - ref) > 1e-6) >= 2 and np.all(c_or <= ref + 1e-9)  # the C oracle loses mass on some of these, never gains
+    out, fl = run(B, ctx, b, B.PHMM_FP32_RESCUE)
+    assert np.max(np.abs(out - ref)) <= TOL32, (out, ref)
+    assert np.all(fl == B.PHMM_FLAG_LONG)  # computed by the fp32 long kernel itself, no fp64 fallback
+    out64, _ = run(B, ctx, b, B.PHMM_FP64)
+    assert np.max(np.abs(out64 - ref)) <= TOL64
+
+
 def test_async_calls_back_to_back_bitwise(B, ctx):
     """The call only enqueues: different batches issued back to back on one stream (plan uploads of call s+1 run
     on the context's copy stream under the kernels of call s, two plan sets alternate) must give exactly what each
@@ -345,7 +370,11 @@ def _fz_make(rng, npairs, kmax, lmax):
         h = int(rng.integers(0, nh)); hap = haps[h]; k = len(hap)
         l = int(rng.integers(1, lmax))
         mode = rng.random()
-        if mode < 0.55 and k > 2:
+        if mode < 0.12 and k > 200 and l > 60:  # two stretches of the haplotype, possibly far apart, in either order
+            cut = int(rng.integers(20, l - 20))
+            a0, b0 = int(rng.integers(0, k - 20)), int(rng.integers(0, k - 20))
+            rd = list((hap[a0:a0 + cut] + _fz_rs(rng, cut))[:cut] + (hap[b0:b0 + l - cut] + _fz_rs(rng, l))[:l - cut])
+        elif mode < 0.55 and k > 2:
             s0 = int(rng.integers(0, max(1, k - 1)))
             rd = list((hap[s0:s0 + l] + _fz_rs(rng, l))[:l])
             for i in rng.choice(l, max(0, l // 25), replace=False): rd[i] = "ACGTN"[int(rng.integers(0, 5))]
