@@ -81,6 +81,7 @@ struct phmm_ctx {
     } set[2];
     int call_idx = 0, slice_idx = 0;
     cudaStream_t copy_stream = nullptr;
+    cudaEvent_t ev_pay = nullptr;   // copy stream: a slice's read arrays (and everything uploaded before them) are on the device
     cudaEvent_t ev_last = nullptr;  // end of the device work of the most recent call: the next call's stream waits for it,
                                     // because the table, the counters, the queues and the boundary buffers exist once per context
     DevBuf d_lut, d_table;
@@ -139,6 +140,7 @@ extern "C" int phmm_create(phmm_ctx** out, int device, const phmm_options* opt) 
     if (ctx->opt.max_table_bytes <= 0) ctx->opt.max_table_bytes = (int64_t)4 << 30;
     memset(&ctx->stats, 0, sizeof(ctx->stats));
     if (cudaEventCreateWithFlags(&ctx->ev_last, cudaEventDisableTiming) != cudaSuccess) { phmm_destroy(ctx); return PHMM_E_CUDA; }
+    if (cudaEventCreateWithFlags(&ctx->ev_pay, cudaEventDisableTiming) != cudaSuccess) { phmm_destroy(ctx); return PHMM_E_CUDA; }
     for (int i = 0; i < 2; i++)
         if (cudaEventCreateWithFlags(&ctx->set[i].ev_free, cudaEventDisableTiming) != cudaSuccess ||
             cudaEventCreateWithFlags(&ctx->set[i].ev_up, cudaEventDisableTiming) != cudaSuccess ||
@@ -188,6 +190,7 @@ extern "C" int phmm_destroy(phmm_ctx* ctx) {
     }
     if (ctx->copy_stream) cudaStreamDestroy(ctx->copy_stream);
     if (ctx->ev_last) cudaEventDestroy(ctx->ev_last);
+    if (ctx->ev_pay) cudaEventDestroy(ctx->ev_pay);
     for (cudaEvent_t e : ctx->ev_prof)
         if (e) cudaEventDestroy(e);
     delete ctx;
@@ -423,8 +426,37 @@ static int forward_impl(phmm_ctx* ctx, const phmm_batch* b, int precision, doubl
 
 static int run_slice(phmm_ctx* ctx, const phmm_batch* b, const HostBatchView& hv, bool fp64, double* d_out, uint8_t* d_flags,
                      cudaStream_t st, const phmm_ctx::CallSet& cs, SliceWork& sw, const HostPayload* hp) {
-    const auto t0 = std::chrono::steady_clock::now();
     const int64_t np_slice = sw.n_ids;
+    DevBatch db;
+    db.read_bases = b->d_read_bases; db.qual_base = b->d_qual_base; db.qual_ins = b->d_qual_ins;
+    db.qual_del = b->d_qual_del; db.qual_gcp = b->d_qual_gcp; db.hap_bases = b->d_hap_bases;
+    db.read_off = (const int64_t*)cs.d_read_off.p; db.hap_off = (const int64_t*)cs.d_hap_off.p;
+    db.n_reads = b->n_reads; db.n_haps = b->n_haps;
+    db.table_base = sw.table_base;
+    db.n_wild = ctx->opt.n_is_wildcard ? 1 : 0;
+    int launches = 0;
+    // ---- fp32: the slice's share of the read arrays (host entry: pinned or pageable host memory) and its row-constant table
+    // (short and long pairs use the same one) go first: they need nothing of the plan, so the copy and the table kernel run
+    // while the host plans the slice (configs[1] through the host entry: within the run-to-run noise of the box, about +1 %)
+    if (hp) {
+        const int64_t o0 = b->h_read_off[sw.r0], o1 = b->h_read_off[sw.r1];
+        for (int i = 0; i < 5 && o1 > o0; i++)
+            CK(cudaMemcpyAsync(hp->dst[i] + o0, hp->src[i] + o0, (size_t)(o1 - o0), cudaMemcpyHostToDevice, ctx->copy_stream));
+    }
+    if (!fp64) {
+        int max_len = 0;
+        for (int64_t r = sw.r0; r < sw.r1; r++) max_len = std::max(max_len, (int)(b->h_read_off[r + 1] - b->h_read_off[r]));
+        CK(cudaEventRecord(ctx->ev_pay, ctx->copy_stream));  // (behind the call's offset arrays, uploaded on the same stream)
+        CK(cudaStreamWaitEvent(st, ctx->ev_pay, 0));
+        const size_t table_bytes = (size_t)sw.table_entries * 64;
+        CK(ctx->d_table.need(table_bytes));
+        ctx->stats.table_bytes = std::max<int64_t>(ctx->stats.table_bytes, (int64_t)table_bytes);
+        PROF(0, 0);
+        CK(launch_lut_table(db, (const double*)ctx->d_lut.p, (float*)ctx->d_table.p, sw.r0, sw.r1, max_len, st));
+        PROF(0, 1);
+        launches++;
+    }
+    const auto t0 = std::chrono::steady_clock::now();
     // ---- classify: short (sub-warp systolic fp32 kernel) / fp64 sub-warp / chain-sequential (one warp per pair) / strips
     {
         struct Part { std::vector<int> seq, strip, sub, sh; int64_t cells = 0, lane_rows = 0; int max_l = 0, max_l_long = 0; };
@@ -523,11 +555,6 @@ static int run_slice(phmm_ctx* ctx, const phmm_batch* b, const HostBatchView& hv
                          items.size() * sizeof(ChainItem) + n_seq * 4 + sw.sub_pairs.size() * 4 + 20 * 256;
     CK(ps.h_stage.need(stage_bytes));
     Stager sg{ctx, &ps.h_stage, ctx->copy_stream};
-    if (hp) {  // host entry: this slice's share of the read arrays (pinned or pageable host memory), ahead of its kernels
-        const int64_t o0 = b->h_read_off[sw.r0], o1 = b->h_read_off[sw.r1];
-        for (int i = 0; i < 5 && o1 > o0; i++)
-            CK(cudaMemcpyAsync(hp->dst[i] + o0, hp->src[i] + o0, (size_t)(o1 - o0), cudaMemcpyHostToDevice, ctx->copy_stream));
-    }
     RC(sg.upload(ps.d_tasks, pl.tasks.data(), pl.tasks.size() * sizeof(ShortTask)));
     RC(sg.upload(ps.d_warp_first, pl.warp_first.data(), pl.warp_first.size() * 4));
     RC(sg.upload(ps.d_srt_ent, pl.srt_ent.data(), pl.srt_ent.size() * 4));
@@ -556,29 +583,10 @@ static int run_slice(phmm_ctx* ctx, const phmm_batch* b, const HostBatchView& hv
     CK(ctx->d_rq_sorted.need((size_t)np_slice * 4 + 4));
     CK(cudaMemsetAsync(ctx->d_rq.p, 0, RQ_INTS * 4, st));
 
-    DevBatch db;
-    db.read_bases = b->d_read_bases; db.qual_base = b->d_qual_base; db.qual_ins = b->d_qual_ins;
-    db.qual_del = b->d_qual_del; db.qual_gcp = b->d_qual_gcp; db.hap_bases = b->d_hap_bases;
-    db.read_off = (const int64_t*)cs.d_read_off.p; db.hap_off = (const int64_t*)cs.d_hap_off.p;
-    db.n_reads = b->n_reads; db.n_haps = b->n_haps;
-    db.table_base = sw.table_base;
-    db.n_wild = ctx->opt.n_is_wildcard ? 1 : 0;
     const int* d_pair_read = (const int*)cs.d_pair_read.p;
     const int* d_pair_hap = (const int*)cs.d_pair_hap.p;
     int* counters = (int*)ctx->d_counters.p;
-    int launches = 0;
-
-    // ---- fp32: row-constant table of the slice's reads (short and long pairs use the same one)
     const bool long32 = !fp64 && !items.empty();
-    if (n_warps > 0 || long32) {
-        const size_t table_bytes = (size_t)sw.table_entries * 64;
-        CK(ctx->d_table.need(table_bytes));
-        ctx->stats.table_bytes = std::max<int64_t>(ctx->stats.table_bytes, (int64_t)table_bytes);
-        PROF(0, 0);
-        CK(launch_lut_table(db, (const double*)ctx->d_lut.p, (float*)ctx->d_table.p, sw.r0, sw.r1, std::max(max_seq_l, max_long_l), st));
-        PROF(0, 1);
-        launches++;
-    }
     if (fp64 && !sw.sub_pairs.empty()) {  // PHMM_FP64: the same table in double, for the sub-warp kernel
         const size_t table_bytes = (size_t)sw.table_entries * 64;
         CK(ctx->d_table.need(table_bytes));

@@ -356,7 +356,16 @@ k_chain(DevBatch b, ChainLaunch p, int items_are_pairs) {
     }
 }
 
-constexpr int WPC_F64 = 2, MINB_F64 = 2;
+// One-warp CTAs, twelve per SM (164 registers, no spills): the kernel waits on fp64 dependencies, and 12 warps per SM against
+// the 8 of two-warp CTAs at 192 registers are +22 % (0.85 -> 1.04 TCUPS, configs[3] x 0.25 in PHMM_FP64).  24 or 32 columns
+// per lane at 8 warps per SM measure the same; 20 columns at 12 warps spill and lose 3 %.
+#ifndef CHAIN_WPC_F64
+#define CHAIN_WPC_F64 1
+#endif
+#ifndef CHAIN_MINB_F64
+#define CHAIN_MINB_F64 12
+#endif
+constexpr int WPC_F64 = CHAIN_WPC_F64, MINB_F64 = CHAIN_MINB_F64;
 
 cudaError_t launch_chain(const DevBatch& b, const ChainLaunch& p, bool fp64, bool items_are_pairs, int grid_ctas, cudaStream_t st) {
     if (grid_ctas <= 0) return cudaSuccess;

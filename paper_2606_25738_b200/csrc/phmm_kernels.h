@@ -13,7 +13,10 @@ constexpr int SHORT_NV = SHORT_NV_;        // columns per virtual lane, fp32 sho
 constexpr int SHORT_N2 = 2 * SHORT_NV;    // columns per CUDA lane
 constexpr int SHORT_MAX_K = 32 * SHORT_N2;  // 1024: widest haplotype one warp covers
 constexpr int CHAIN_NV_F32 = 16;
-constexpr int CHAIN_NV_F64 = 8;
+#ifndef CHAIN_NV_F64_
+#define CHAIN_NV_F64_ 8
+#endif
+constexpr int CHAIN_NV_F64 = CHAIN_NV_F64_;
 #ifndef SHORT_WPC_
 #define SHORT_WPC_ 4
 #endif
