@@ -11,9 +11,10 @@ the metric is quoted on (2,000 regions x 128 reads x 8 haplotypes = 2.05 M pairs
 
 value      GCUPS = cells / time / 1e9 (TCUPS x 1000), payload resident in HBM, timed
            with CUDA events on the launching stream around exactly K calls, max over ranks.
-e2e        same metric through phmm_forward_batch_host: all buffers in pinned HOST memory, the
-           host->device copies of the payload and the device->host copy of the results inside the
-           timed region ("with transfers").
+e2e        same metric through the host entries: all buffers in pinned HOST memory, the host->device copies of the
+           payload and the device->host copy of the results of every step inside the timed region (PAPER.md:346
+           "with transfers").  value = the streaming entry (phmm_forward_batch_host_async, two calls in flight);
+           sync_value = phmm_forward_batch_host, one synchronous call after the other.
 roofline   dominant kernel (short: k_short_f32, long: k_long_f32, fp64: k_rescue_f64t / k_chain<double>) against the FP32 (FP64)
            non-tensor peak; flops = 10 per cell; duration from the library's CUDA events.
 cpu_baseline  the oracle (oracle/, as it stands) on the host cores on a bounded sample of the same batch.
@@ -250,23 +251,47 @@ def measure(args, workload, steps, rank, world, local, with_cpu):
     # ---- end to end: host (pinned) buffers in, host results out, copies inside the timed region
     e2e = None
     if not args.no_e2e:
-        hb = binding.HostBatch(batch)
+        hb = [binding.HostBatch(batch), binding.HostBatch(batch)]  # two sets of pinned buffers: a stream of batches
+
+        def wall_max(dt):
+            if world > 1:
+                t = torch.tensor([dt], dtype=torch.float64, device=dev)
+                dist.all_reduce(t, op=dist.ReduceOp.MAX)
+                dt = float(t.item())
+            return dt
+
         for _ in range(2):
-            ctx.forward_batch_host(hb, prec)
+            ctx.forward_batch_host(hb[0], prec)
+        # (1) one synchronous call after the other: nothing of step s+1 starts before the results of step s are on the host
         barrier()
         t0 = time.perf_counter()
         for _ in range(steps):
-            ctx.forward_batch_host(hb, prec)
+            ctx.forward_batch_host(hb[0], prec)
         torch.cuda.synchronize()
-        dt = time.perf_counter() - t0
-        if world > 1:
-            t = torch.tensor([dt], dtype=torch.float64, device=dev)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            dt = float(t.item())
+        dt_sync = wall_max(time.perf_counter() - t0)
+        n_slices_sync = ctx.stats()["n_slices"]
+        # (2) the streaming entry, two calls in flight: the copies in and the host plan of step s+1 run under the kernels of
+        # step s; every step still copies its inputs in and its results out inside the timed region
+        for i in range(2):
+            ctx.wait_host(ctx.forward_batch_host_async(hb[i], prec))
+        barrier()
+        t0 = time.perf_counter()
+        prev = None
+        for i in range(steps):
+            t = ctx.forward_batch_host_async(hb[i & 1], prec)
+            if prev is not None:
+                ctx.wait_host(prev)
+            prev = t
+        ctx.wait_host(prev)
+        dt = wall_max(time.perf_counter() - t0)
         e2e = {"value": tot_cells / (dt / steps) / 1e9, "unit": "GCUPS",
-               "h2d_bytes_per_step": int(hb.h2d_bytes()), "d2h_bytes_per_step": int(hb.d2h_bytes()),
-               "ms_per_step": dt / steps * 1e3, "slices": ctx.stats()["n_slices"],
-               "timer": "host wall clock around the synchronous C-ABI call"}
+               "h2d_bytes_per_step": int(hb[0].h2d_bytes()), "d2h_bytes_per_step": int(hb[0].d2h_bytes()),
+               "ms_per_step": dt / steps * 1e3,
+               "mode": "phmm_forward_batch_host_async / phmm_wait_host, two calls in flight, pinned host buffers",
+               "timer": "host wall clock from the first submit to the last wait (results of every step on the host)",
+               "sync_value": tot_cells / (dt_sync / steps) / 1e9, "sync_ms_per_step": dt_sync / steps * 1e3,
+               "sync_slices": n_slices_sync,
+               "sync_mode": "phmm_forward_batch_host, one synchronous call after the other"}
         del hb
     if rank != 0:
         return None

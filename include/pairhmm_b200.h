@@ -160,9 +160,30 @@ int phmm_forward_batch(phmm_ctx* ctx, const phmm_batch* b, int precision, double
  * the results back and synchronises.  This is the end-to-end entry ("with transfer").
  * The reads are processed in slices (at least one per 48 MB of read payload, and as many as the table budget asks for):
  * the copy of a slice's reads and its host plan run under the kernels of the slice before; results and flags are the
- * same as for one call with device buffers.  phmm_get_stats afterwards reports the sums over the slices. */
+ * same as for one call with device buffers.  phmm_get_stats afterwards reports the sums over the slices.  The device work
+ * runs on a stream of the context, not on the caller's. */
 int phmm_forward_batch_host(phmm_ctx* ctx, const phmm_batch* b, int precision, double* h_out_log10,
                             uint8_t* h_out_flags);
+
+/* The streaming form of phmm_forward_batch_host (the "with transfer" convention; SURVEY.md section 8(f)
+ * item 2): enqueues the copies in, the kernels and the copies out of one batch and returns with a ticket; the results are
+ * in h_out_log10 / h_out_flags once phmm_wait_host(ctx, ticket) has returned.  Up to two calls are in flight per context:
+ * a third call first waits for the oldest one.  With a second call submitted before the first is waited for, the copies
+ * and the host plan of one batch run under the kernels of the batch before it (the context keeps two device copies of
+ * payload and outputs); the reads of a call are then not sliced unless the table budget asks for it.
+ *   - Every host array of `b` (offsets, pair lists and the payload), h_out_log10 and h_out_flags must stay valid and
+ *     unchanged / unread until the ticket has been waited for.  The payload and the output arrays should be pinned
+ *     (cudaHostAlloc / cudaHostRegister) memory: with pageable memory the copies are staged by the driver and the call does
+ *     not return before they are done, so nothing overlaps (the results are the same).
+ *   - Results, flags and error codes are those of phmm_forward_batch_host.  An error is reported by the call that finds it
+ *     (arguments, offsets, allocation: the submitting call, which then leaves nothing in flight for its ticket).
+ *   - phmm_get_stats reports the batch of the most recently waited ticket (per-family kernel times: of the most recently
+ *     submitted call that has completed).
+ *   - phmm_wait_host on a ticket that has already been waited for (or whose set a later call has taken over, which
+ *     implies it completed) returns PHMM_OK at once.  One caller thread at a time per context, as for every entry. */
+int phmm_forward_batch_host_async(phmm_ctx* ctx, const phmm_batch* b, int precision, double* h_out_log10,
+                                  uint8_t* h_out_flags, int* ticket);
+int phmm_wait_host(phmm_ctx* ctx, int ticket);
 
 /* Statistics of the most recent call on the context.  Waits for that call's device work to complete (the rescue count and
  * the per-family times are only known then), on whatever stream the call was issued. */

@@ -21,7 +21,8 @@ PHMM_E_CUDA, PHMM_E_NOMEM, PHMM_E_UNSUPPORTED = -5, -6, -7
 PHMM_FP32_RESCUE, PHMM_FP64 = 0, 1
 PHMM_FLAG_RESCUED, PHMM_FLAG_LONG, PHMM_FLAG_RANGE = 1, 2, 4
 
-EXPORTS = ["phmm_create", "phmm_destroy", "phmm_forward_batch", "phmm_forward_batch_host", "phmm_get_stats",
+EXPORTS = ["phmm_create", "phmm_destroy", "phmm_forward_batch", "phmm_forward_batch_host",
+           "phmm_forward_batch_host_async", "phmm_wait_host", "phmm_get_stats",
            "phmm_strerror", "phmm_last_cuda_error", "phmm_measure_peak", "phmm_plan_host", "phmm_plan_slices_host",
            "phmm_noalloc_setup", "phmm_noalloc_limits", "phmm_forward_batch_noalloc"]
 
@@ -86,6 +87,11 @@ def lib() -> ctypes.CDLL:
         L.phmm_forward_batch_host.argtypes = [ctypes.c_void_p, ctypes.POINTER(phmm_batch), ctypes.c_int,
                                               ctypes.c_void_p, ctypes.c_void_p]
         L.phmm_forward_batch_host.restype = ctypes.c_int
+        L.phmm_forward_batch_host_async.argtypes = [ctypes.c_void_p, ctypes.POINTER(phmm_batch), ctypes.c_int,
+                                                    ctypes.c_void_p, ctypes.c_void_p, ctypes.POINTER(ctypes.c_int)]
+        L.phmm_forward_batch_host_async.restype = ctypes.c_int
+        L.phmm_wait_host.argtypes = [ctypes.c_void_p, ctypes.c_int]
+        L.phmm_wait_host.restype = ctypes.c_int
         L.phmm_get_stats.argtypes = [ctypes.c_void_p, ctypes.POINTER(phmm_stats)]
         L.phmm_get_stats.restype = ctypes.c_int
         L.phmm_strerror.argtypes = [ctypes.c_int]
@@ -296,6 +302,23 @@ class Context:
         if rc != PHMM_OK:
             raise PhmmError(rc, lib().phmm_last_cuda_error(self._h))
         return out, flags
+
+    def forward_batch_host_async(self, batch: "HostBatch", precision: int = PHMM_FP32_RESCUE) -> int:
+        """phmm_forward_batch_host_async: enqueue one HostBatch (pinned buffers) and return its ticket; the results are
+        in ``batch.out`` / ``batch.flags`` after ``wait_host(ticket)``.  Up to two calls in flight; the batch object must
+        stay alive and untouched until then."""
+        cb = batch.c_struct()
+        t = ctypes.c_int(-1)
+        rc = lib().phmm_forward_batch_host_async(self._h, ctypes.byref(cb), precision, batch.out.data_ptr(),
+                                                 batch.flags.data_ptr(), ctypes.byref(t))
+        if rc != PHMM_OK:
+            raise PhmmError(rc, lib().phmm_last_cuda_error(self._h))
+        return t.value
+
+    def wait_host(self, ticket: int) -> None:
+        rc = lib().phmm_wait_host(self._h, ticket)
+        if rc != PHMM_OK:
+            raise PhmmError(rc, lib().phmm_last_cuda_error(self._h))
 
     def stats(self) -> dict:
         s = phmm_stats()

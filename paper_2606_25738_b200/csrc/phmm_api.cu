@@ -87,7 +87,20 @@ struct phmm_ctx {
     DevBuf d_lut, d_table;
     DevBuf d_counters, d_rescue, d_boundary, d_progress, d_scratch, d_totals, d_acc, d_risk;
     DevBuf d_rq, d_rq_queue, d_rq_sorted, d_rq_plan;  // fp64 sub-warp recomputation: counters, queue, ordered queue, plan
-    DevBuf d_payload, d_out, d_flags;  // phmm_forward_batch_host only
+    // Host entries (phmm_forward_batch_host, phmm_forward_batch_host_async): two sets of device copies of the payload and of
+    // the outputs, so that the copies and the host plan of one call run under the kernels of the call before it.
+    struct HostSet {
+        DevBuf d_payload, d_out, d_flags;
+        PinBuf h_flags;              // where the caller passes no flags array
+        cudaEvent_t done = nullptr;  // the call's outputs are in the caller's host arrays
+        bool pending = false;
+        int ticket = -1;
+        int64_t np = 0;
+        const uint8_t* fl = nullptr;
+        phmm_stats stats;
+    } hset[2];
+    int host_calls = 0;
+    cudaStream_t host_stream = nullptr;  // the kernels of the host entries
     std::vector<uint8_t> is_short, read_slice;
     std::vector<int> sorted_all, slice_ids, short_ids;
     ShortPlan plan;
@@ -147,6 +160,9 @@ extern "C" int phmm_create(phmm_ctx** out, int device, const phmm_options* opt) 
             cudaEventCreateWithFlags(&ctx->cset[i].ev_free, cudaEventDisableTiming) != cudaSuccess ||
             cudaEventCreateWithFlags(&ctx->cset[i].ev_up, cudaEventDisableTiming) != cudaSuccess) { phmm_destroy(ctx); return PHMM_E_CUDA; }
     if (cudaStreamCreateWithFlags(&ctx->copy_stream, cudaStreamNonBlocking) != cudaSuccess) { phmm_destroy(ctx); return PHMM_E_CUDA; }
+    if (cudaStreamCreateWithFlags(&ctx->host_stream, cudaStreamNonBlocking) != cudaSuccess) { phmm_destroy(ctx); return PHMM_E_CUDA; }
+    for (int i = 0; i < 2; i++)
+        if (cudaEventCreateWithFlags(&ctx->hset[i].done, cudaEventDisableTiming) != cudaSuccess) { phmm_destroy(ctx); return PHMM_E_CUDA; }
     // 10^(-q/10) for every quality byte, the paper's "q64" table: [0..255] for insertion, deletion and
     // continuation qualities, [256..511] for base qualities (with the optional floor), both after the optional offset
     if (ctx->opt.qual_offset < 0 || ctx->opt.qual_offset > 255 || ctx->opt.min_base_qual < 0) { phmm_destroy(ctx); return PHMM_E_ARG; }
@@ -172,8 +188,14 @@ extern "C" int phmm_destroy(phmm_ctx* ctx) {
     DeviceGuard guard(ctx->device);
     cudaDeviceSynchronize();
     DevBuf* bufs[] = {&ctx->d_lut, &ctx->d_table, &ctx->d_counters, &ctx->d_rescue, &ctx->d_boundary, &ctx->d_progress, &ctx->d_scratch, &ctx->d_totals, &ctx->d_acc, &ctx->d_risk,
-                      &ctx->d_payload, &ctx->d_out, &ctx->d_flags, &ctx->d_rq, &ctx->d_rq_queue, &ctx->d_rq_sorted, &ctx->d_rq_plan};
+                      &ctx->d_rq, &ctx->d_rq_queue, &ctx->d_rq_sorted, &ctx->d_rq_plan};
     for (DevBuf* b : bufs) b->release();
+    for (int i = 0; i < 2; i++) {
+        phmm_ctx::HostSet& hs = ctx->hset[i];
+        hs.d_payload.release(); hs.d_out.release(); hs.d_flags.release(); hs.h_flags.release();
+        if (hs.done) cudaEventDestroy(hs.done);
+    }
+    if (ctx->host_stream) cudaStreamDestroy(ctx->host_stream);
     for (int i = 0; i < 2; i++) {
         phmm_ctx::PlanSet& ps = ctx->set[i];
         DevBuf* sb[] = {&ps.d_tasks, &ps.d_warp_first, &ps.d_srt_ent, &ps.d_srt_out, &ps.d_items, &ps.d_rq_enq, &ps.d_seq};
@@ -770,11 +792,36 @@ extern "C" int phmm_forward_batch(phmm_ctx* ctx, const phmm_batch* b, int precis
     return forward_impl(ctx, b, precision, d_out, d_flags, (cudaStream_t)cuda_stream, nullptr, 1);
 }
 
-// ---------------------------------------------------------------- end-to-end entry with host buffers
-extern "C" int phmm_forward_batch_host(phmm_ctx* ctx, const phmm_batch* b, int precision, double* h_out, uint8_t* h_flags) {
+// ---------------------------------------------------------------- end-to-end entries with host buffers
+// Completion of a host call: its outputs are in the caller's arrays; the statistics become those of this call.
+static int host_wait(phmm_ctx* ctx, int set) {
+    phmm_ctx::HostSet& hs = ctx->hset[set];
+    if (!hs.pending) return PHMM_OK;
+    DeviceGuard guard(ctx->device);
+    if (!guard.ok) return PHMM_E_CUDA;
+    hs.pending = false;
+    CK(cudaEventSynchronize(hs.done));
+    int64_t n_resc = 0;
+    for (int64_t p = 0; p < hs.np; p++) n_resc += hs.fl[p] & PHMM_FLAG_RESCUED;
+    hs.stats.n_rescued = n_resc;
+    ctx->stats = hs.stats;
+    ctx->stats_final = true;
+    return PHMM_OK;
+}
+
+// Enqueues everything of one host call (copies in, plan, kernels, copies out) and returns; `pipelined`: the call is one of a
+// stream of calls, so the copies and the plan of the next one will overlap this one's kernels and slices within the call
+// buy nothing.
+static int host_submit(phmm_ctx* ctx, const phmm_batch* b, int precision, double* h_out, uint8_t* h_flags, bool pipelined, int* ticket) {
     if (!ctx || !b) return PHMM_E_ARG;
     if (precision != PHMM_FP32_RESCUE && precision != PHMM_FP64) return PHMM_E_ARG;
     if (b->n_pairs < 0 || b->n_reads < 0 || b->n_haps < 0) return PHMM_E_ARG;
+    const int set = ctx->host_calls & 1;
+    phmm_ctx::HostSet& hs = ctx->hset[set];
+    RC(host_wait(ctx, set));  // the call that used this set two calls ago (its outputs are complete, its statistics superseded)
+    if (ticket) *ticket = ctx->host_calls;
+    hs.ticket = ctx->host_calls;
+    ctx->host_calls = (ctx->host_calls + 1) & 0x3fffffff;
     memset(&ctx->stats, 0, sizeof(ctx->stats));
     ctx->stats_final = false;
     ctx->prof_used.clear();
@@ -786,10 +833,13 @@ extern "C" int phmm_forward_batch_host(phmm_ctx* ctx, const phmm_batch* b, int p
     if (!guard.ok) return PHMM_E_CUDA;
     const size_t R = (size_t)b->h_read_off[b->n_reads], H = (size_t)b->h_hap_off[b->n_haps];
     const size_t Ra = (R + 255) & ~(size_t)255, Ha = (H + 255) & ~(size_t)255;
-    CK(ctx->d_payload.need(5 * Ra + Ha + 256));
-    CK(ctx->d_out.need((size_t)b->n_pairs * 8));
-    CK(ctx->d_flags.need((size_t)b->n_pairs));
-    uint8_t* base = (uint8_t*)ctx->d_payload.p;
+    const int64_t np = b->n_pairs;
+    CK(hs.d_payload.need(5 * Ra + Ha + 256));
+    CK(hs.d_out.need((size_t)np * 8));
+    CK(hs.d_flags.need((size_t)np));
+    uint8_t* fl = h_flags;
+    if (!fl) { CK(hs.h_flags.need((size_t)np)); fl = (uint8_t*)hs.h_flags.p; }
+    uint8_t* base = (uint8_t*)hs.d_payload.p;
     HostPayload hp;
     const uint8_t* src[5] = {b->d_read_bases, b->d_qual_base, b->d_qual_ins, b->d_qual_del, b->d_qual_gcp};
     for (int i = 0; i < 5; i++) {
@@ -798,17 +848,15 @@ extern "C" int phmm_forward_batch_host(phmm_ctx* ctx, const phmm_batch* b, int p
         hp.dst[i] = base + i * Ra - b->h_read_off[0];
     }
     if (!b->d_hap_bases) return PHMM_E_ARG;
-    cudaStream_t st = nullptr;
-    // the payload buffer may still be read by the kernels of an earlier call: the copy stream waits for them
-    CK(cudaStreamWaitEvent(ctx->copy_stream, ctx->ev_last, 0));
+    cudaStream_t st = ctx->host_stream;
+    // (this set's payload buffer is free: the call that read it was waited for above)
     CK(cudaMemcpyAsync(base + 5 * Ra, b->d_hap_bases, H, cudaMemcpyHostToDevice, ctx->copy_stream));
     phmm_batch db = *b;
     db.d_read_bases = hp.dst[0]; db.d_qual_base = hp.dst[1]; db.d_qual_ins = hp.dst[2]; db.d_qual_del = hp.dst[3];
     db.d_qual_gcp = hp.dst[4]; db.d_hap_bases = base + 5 * Ra - b->h_hap_off[0];
-    // The reads are processed in slices (at least one per 48 MB of read payload, up to 16): the copy of slice s+1 and its
-    // host plan run while the GPU works on slice s (the "with transfers" convention).
-    const int min_slices = (int)std::max<size_t>(1, std::min<size_t>(16, 5 * R / ((size_t)48 << 20)));  // (configs[1]: 1 / 2 / 4 / 7 / 10 slices: 53.6 / 51.5 / 48.6 / 50.7 / 50.0 ms)
-    const int64_t np = b->n_pairs;
+    // A call on its own: the reads are processed in slices (at least one per 48 MB of read payload, up to 16), so that the copy
+    // of slice s+1 and its host plan run while the GPU works on slice s (the "with transfers" convention).
+    const int min_slices = pipelined ? 1 : (int)std::max<size_t>(1, std::min<size_t>(16, 5 * R / ((size_t)48 << 20)));  // (configs[1]: 1 / 2 / 4 / 7 / 10 slices: 53.6 / 51.5 / 48.6 / 50.7 / 50.0 ms)
     const HostPayload* hpp = &hp;
     if (ctx->opt.validate) {  // the whole payload first, then the check: nothing may be written for a bad batch
         CK(cudaStreamWaitEvent(st, ctx->ev_last, 0));
@@ -817,17 +865,31 @@ extern "C" int phmm_forward_batch_host(phmm_ctx* ctx, const phmm_batch* b, int p
         RC(validate_payload(ctx, &db, st));
         hpp = nullptr;
     }
-    int rc = forward_impl(ctx, &db, precision, (double*)ctx->d_out.p, (uint8_t*)ctx->d_flags.p, st, hpp, min_slices);
+    int rc = forward_impl(ctx, &db, precision, (double*)hs.d_out.p, (uint8_t*)hs.d_flags.p, st, hpp, min_slices);
     if (rc != PHMM_OK) { cudaStreamSynchronize(st); return rc; }
-    std::vector<uint8_t> tmp_flags;
-    uint8_t* fl = h_flags;
-    if (!fl) { tmp_flags.resize((size_t)np); fl = tmp_flags.data(); }
-    CK(cudaMemcpyAsync(h_out, ctx->d_out.p, (size_t)np * 8, cudaMemcpyDeviceToHost, st));
-    CK(cudaMemcpyAsync(fl, ctx->d_flags.p, (size_t)np, cudaMemcpyDeviceToHost, st));
-    CK(cudaStreamSynchronize(st));
-    int64_t n_resc = 0;
-    for (int64_t p = 0; p < np; p++) n_resc += fl[p] & PHMM_FLAG_RESCUED;
-    ctx->stats.n_rescued = n_resc;
-    ctx->stats_final = true;
+    CK(cudaMemcpyAsync(h_out, hs.d_out.p, (size_t)np * 8, cudaMemcpyDeviceToHost, st));
+    CK(cudaMemcpyAsync(fl, hs.d_flags.p, (size_t)np, cudaMemcpyDeviceToHost, st));
+    CK(cudaEventRecord(hs.done, st));
+    hs.pending = true;
+    hs.np = np;
+    hs.fl = fl;
+    hs.stats = ctx->stats;
     return PHMM_OK;
+}
+
+extern "C" int phmm_forward_batch_host(phmm_ctx* ctx, const phmm_batch* b, int precision, double* h_out, uint8_t* h_flags) {
+    int ticket = 0;
+    RC(host_submit(ctx, b, precision, h_out, h_flags, false, &ticket));
+    return host_wait(ctx, ticket & 1);
+}
+
+extern "C" int phmm_forward_batch_host_async(phmm_ctx* ctx, const phmm_batch* b, int precision, double* h_out, uint8_t* h_flags, int* ticket) {
+    if (!ticket) return PHMM_E_ARG;
+    return host_submit(ctx, b, precision, h_out, h_flags, true, ticket);
+}
+
+extern "C" int phmm_wait_host(phmm_ctx* ctx, int ticket) {
+    if (!ctx || ticket < 0) return PHMM_E_ARG;
+    if (ctx->hset[ticket & 1].ticket != ticket) return PHMM_OK;  // completed already: a later call took over its set
+    return host_wait(ctx, ticket & 1);
 }

@@ -355,6 +355,50 @@ def test_host_entry_matches_device_entry(B, ctx):
     assert hb.h2d_bytes() > 5 * len(b.read_bases) and hb.d2h_bytes() == 9 * b.n_pairs
 
 
+def test_host_stream_two_calls_in_flight(B, ctx):
+    """phmm_forward_batch_host_async / phmm_wait_host: a stream of different batches (short-read regions with rescued pairs,
+    a long-read batch, a mixed one, in both precisions), two calls in flight, every result equal to the synchronous entry's
+    and within tolerance of the oracle; sets are reused (5 calls on 2 sets), tickets can be waited for late, twice or never."""
+    batches = [W.generate(1, n=6, seed=31), W.generate(3, n=3, seed=32), W.generate(2, n=3000, seed=33),
+               W.generate(1, n=4, seed=34), W.generate(0, seed=35)]
+    precs = [B.PHMM_FP32_RESCUE, B.PHMM_FP32_RESCUE, B.PHMM_FP32_RESCUE, B.PHMM_FP64, B.PHMM_FP32_RESCUE]
+    want = []
+    for b, pr in zip(batches, precs):
+        o, f = ctx.forward_batch_host(b, pr)
+        want.append((o.copy(), f.copy()))
+    hbs = [B.HostBatch(b) for b in batches]
+    for hb in hbs:
+        hb.out.fill_(float("nan"))
+    c = B.Context(0)
+    try:
+        tickets = []
+        for i, (hb, pr) in enumerate(zip(hbs, precs)):
+            tickets.append(c.forward_batch_host_async(hb, pr))
+            if i >= 1 and i != 3:
+                c.wait_host(tickets[i - 1])  # (ticket 2 is never waited for: the fifth call takes over its set)
+        c.wait_host(tickets[-1])
+        c.wait_host(tickets[0])   # long completed
+        c.wait_host(tickets[-1])  # twice
+        assert c.stats()["n_pairs"] == batches[-1].n_pairs
+        for i, (hb, (o, f)) in enumerate(zip(hbs, want)):
+            assert np.array_equal(hb.out.numpy(), o), "batch %d" % i
+            assert np.array_equal(hb.flags.numpy(), f), "batch %d" % i
+        ref = oracle.forward_batch(batches[4])
+        assert np.all(np.abs(hbs[4].out.numpy() - ref) <= TOL32)
+        assert (hbs[4].flags.numpy() & 1).sum() > 0 and (hbs[0].flags.numpy() & 1).sum() > 0
+        # a bad batch is refused by the submitting call and leaves nothing in flight
+        bad = B.HostBatch(batches[0])
+        bad.pair_read[0] = 10 ** 6
+        with pytest.raises(B.PhmmError) as ei:
+            c.forward_batch_host_async(bad, B.PHMM_FP32_RESCUE)
+        assert ei.value.code == B.PHMM_E_OFFSETS
+        t = c.forward_batch_host_async(hbs[1], precs[1])
+        c.wait_host(t)
+        assert np.array_equal(hbs[1].out.numpy(), want[1][0])
+    finally:
+        c.close()
+
+
 # ------------------------------------------------------------------ randomized batches (the fuzzer that found round 2's bugs)
 def _fz_rs(rng, n): return "".join(rng.choice(list("ACGT"), n))
 def _fz_make(rng, npairs, kmax, lmax):
