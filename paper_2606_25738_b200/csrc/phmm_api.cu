@@ -105,7 +105,7 @@ struct phmm_ctx {
     std::vector<int> sorted_all, slice_ids, short_ids;
     ShortPlan plan;
     int chain_grid[2] = {0, 0};  // resident CTAs of the fp64 chain kernel ([1]; [0] unused)
-    int long_grid = 0, rescue_grid = 0;  // resident CTAs of the fp32 long kernel / of the fp64 sub-warp kernel on this device
+    int long_grid = 0, rescue_grid = 0, long64_grid = 0;  // resident CTAs of the fp32 long kernel / of the fp64 sub-warp kernel on this device
     // profile_events: per slice s and kernel family f (0 table, 1 short, 2 rescue, 3 long) the events [8s + 2f], [8s + 2f + 1]
     std::vector<cudaEvent_t> ev_prof;
     std::vector<uint8_t> prof_used;  // [4s + f]
@@ -179,6 +179,7 @@ extern "C" int phmm_create(phmm_ctx** out, int device, const phmm_options* opt) 
     ctx->chain_grid[1] = chain_ctas_per_sm(true) * ctx->n_sm;
     ctx->long_grid = long_ctas_per_sm() * ctx->n_sm;
     ctx->rescue_grid = rescue_ctas_per_sm() * ctx->n_sm;
+    ctx->long64_grid = long64_ctas_per_sm() * ctx->n_sm;
     *out = ctx;
     return PHMM_OK;
 }
@@ -537,7 +538,7 @@ static int run_slice(phmm_ctx* ctx, const phmm_batch* b, const HostBatchView& hv
     // producer still holds an earlier ticket (forward progress), but it is far ahead or done by the time the
     // consumer starts, so consumers do not run in lock step with their producers and hardly ever poll (pair-major
     // order: 4.6 polls per step, 19 % of the stall samples; profiles/).  Boundary buffers are full-length per strip.
-    const int strip_cols = chain_strip_cols(fp64);
+    const int strip_cols = fp64 ? long64_strip_cols() : chain_strip_cols(false);
     std::vector<ChainItem> items;
     int64_t n_bnd_blocks = 0;
     int n_prog = 0;
@@ -609,12 +610,12 @@ static int run_slice(phmm_ctx* ctx, const phmm_batch* b, const HostBatchView& hv
     const int* d_pair_hap = (const int*)cs.d_pair_hap.p;
     int* counters = (int*)ctx->d_counters.p;
     const bool long32 = !fp64 && !items.empty();
-    if (fp64 && !sw.sub_pairs.empty()) {  // PHMM_FP64: the same table in double, for the sub-warp kernel
+    if (fp64 && (!sw.sub_pairs.empty() || !items.empty())) {  // PHMM_FP64: the same table in double, for the sub-warp kernel and the strips
         const size_t table_bytes = (size_t)sw.table_entries * 64;
         CK(ctx->d_table.need(table_bytes));
         ctx->stats.table_bytes = std::max<int64_t>(ctx->stats.table_bytes, (int64_t)table_bytes);
         PROF(0, 0);
-        CK(launch_table_f64(db, (const double*)ctx->d_lut.p, (double*)ctx->d_table.p, sw.r0, sw.r1, max_seq_l, st));
+        CK(launch_table_f64(db, (const double*)ctx->d_lut.p, (double*)ctx->d_table.p, sw.r0, sw.r1, std::max(max_seq_l, max_long_l), st));
         PROF(0, 1);
         launches++;
     }
@@ -641,17 +642,17 @@ static int run_slice(phmm_ctx* ctx, const phmm_batch* b, const HostBatchView& hv
         launches++;
     }
     // ---- long path.  fp32: table-driven strips with per-lane exponents (phmm_long.cu); what it cannot represent joins
-    // the rescue list of the fp64 chain launch below.  fp64: concurrent strips of the chain kernel.
+    // the rescue list of the fp64 chain launch below.  fp64: table-driven strips in double with per-thread exponents (phmm_long64.cu).
     if (!items.empty()) {
         CK(ctx->d_progress.need((size_t)n_prog * 4 + 4));
         CK(cudaMemsetAsync(ctx->d_progress.p, 0, (size_t)n_prog * 4 + 4, st));
         // no more CTAs than there are strips: with fewer strips than resident warps the block scheduler would fill
         // some SMs completely and leave others empty (configs[4]: 1648 strips, 2368 slots: 1.36 vs 1.76 TCUPS)
-        const int wpc = fp64 ? chain_warps_per_cta(true) : long_warps_per_cta();
+        const int wpc = fp64 ? 1 : long_warps_per_cta();
         const int need_ctas = (int)((items.size() + (size_t)wpc - 1) / (size_t)wpc);
         PROF(3, 0);
         if (fp64) {
-            CK(ctx->d_boundary.need((size_t)(n_bnd_blocks + 1) * chain_block_bytes(true)));
+            CK(ctx->d_boundary.need((size_t)(n_bnd_blocks + 1) * long64_block_bytes()));
             ChainLaunch cl;
             memset(&cl, 0, sizeof(cl));
             cl.items = (const ChainItem*)ps.d_items.p;
@@ -667,7 +668,7 @@ static int run_slice(phmm_ctx* ctx, const phmm_batch* b, const HostBatchView& hv
             cl.flags = d_flags;
             cl.flag_bits = PHMM_FLAG_LONG;
             cl.log2C = 0;
-            CK(launch_chain(db, cl, true, false, std::min(ctx->chain_grid[1], need_ctas), st));
+            CK(launch_long_f64(db, cl, (const double*)ctx->d_table.p, std::min(ctx->long64_grid, need_ctas), st));
         } else {
             CK(ctx->d_boundary.need((size_t)(n_bnd_blocks + 1) * 16));
             CK(ctx->d_totals.need((size_t)n_prog * 16 + 16));

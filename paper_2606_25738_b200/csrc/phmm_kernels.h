@@ -190,5 +190,11 @@ int chain_ctas_per_sm(bool fp64);
 int chain_warps_per_cta(bool fp64);
 size_t chain_block_bytes(bool fp64);  // bytes of one 32-row boundary block
 int chain_strip_cols(bool fp64);      // haplotype columns covered by one strip (fp32 long kernel: SHORT_MAX_K)
+// PHMM_FP64 long pairs as concurrent strips (phmm_long64.cu): ChainLaunch as for the chain kernel (items, progress, boundary
+// blocks of long64_block_bytes()), constants from the double table of launch_table_f64
+cudaError_t launch_long_f64(const DevBatch& b, const ChainLaunch& p, const double* table, int grid_ctas, cudaStream_t st);
+int long64_ctas_per_sm();
+size_t long64_block_bytes();
+int long64_strip_cols();
 
 }  // namespace phmm
