@@ -15,7 +15,7 @@ e2e        same metric through the host entries: all buffers in pinned HOST memo
            payload and the device->host copy of the results of every step inside the timed region (PAPER.md:346
            "with transfers").  value = the streaming entry (phmm_forward_batch_host_async, two calls in flight);
            sync_value = phmm_forward_batch_host, one synchronous call after the other.
-roofline   dominant kernel (short: k_short_f32, long: k_long_f32, fp64: k_rescue_f64t / k_chain<double>) against the FP32 (FP64)
+roofline   dominant kernel (short: k_short_f32, long: k_long_f32, fp64: k_rescue_f64t / k_long_f64) against the FP32 (FP64)
            non-tensor peak; flops = 10 per cell; duration from the library's CUDA events.
 cpu_baseline  the oracle (oracle/, as it stands) on the host cores on a bounded sample of the same batch.
 
@@ -308,7 +308,7 @@ def measure(args, workload, steps, rank, world, local, with_cpu):
         meas = binding.measure_peak(2, local)
     peak = prop.multi_processor_count * lanes * 2 * sm_max * 1e6 / 1e12
     if st["n_long_pairs"] * 2 > st["n_pairs"]:
-        kname = "k_long_f32" if args.precision == "fp32" else "k_chain<double> (concurrent strips)"
+        kname = "k_long_f32" if args.precision == "fp32" else "k_long_f64"
         kms, kcells = fam["ms_long"], cells * 1.0
     elif args.precision == "fp64":
         kname, kms, kcells = "k_rescue_f64t<double> (+ chain fallback)", fam["ms_rescue"], cells * 1.0

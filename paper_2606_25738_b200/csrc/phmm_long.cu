@@ -45,10 +45,25 @@ namespace phmm {
 #define LONG_MIN_CTAS 3
 #endif
 constexpr int LONG_WPC = 4;       // warps per CTA
-constexpr int LONG_TGT = 40;      // a lane's maximum is brought back to 2^TGT at every event: 166 bits of range below it
-constexpr int LONG_KTOT = 80;     // a lane's exponent is at most this much below that of any lane to its left
-constexpr int LONG_EVERY = 16;    // steps between two events
-constexpr int LONG_DROP = 126;    // a lane's own maximum may fall by 2^LONG_DROP between two events before the pair is sent to fp64
+#ifndef LONG_HOPNUM_
+#define LONG_HOPNUM_ 85  // 0.332 x 256
+#endif
+#ifndef LONG_TGT_
+#define LONG_TGT_ 40
+#endif
+constexpr int LONG_TGT = LONG_TGT_;      // a lane's maximum is brought back to 2^TGT at every event: 166 bits of range below it
+#ifndef LONG_KTOT_
+#define LONG_KTOT_ 80
+#endif
+constexpr int LONG_KTOT = LONG_KTOT_;     // a lane's exponent is at most this much below that of any lane to its left
+#ifndef LONG_EVERY_
+#define LONG_EVERY_ 16
+#endif
+constexpr int LONG_EVERY = LONG_EVERY_;    // steps between two events
+#ifndef LONG_DROP_
+#define LONG_DROP_ 126
+#endif
+constexpr int LONG_DROP = LONG_DROP_;    // a lane's own maximum may fall by 2^LONG_DROP between two events before the pair is sent to fp64
 constexpr int LONG_FLOOR = -(1 << 28);  // "no proposal" (a lane that holds nothing but zeros)
 
 __device__ __forceinline__ int ld_relaxed_gpu(const int* p) {
@@ -128,7 +143,8 @@ __global__ void __launch_bounds__(LONG_WPC * 32, LONG_MIN_CTAS) k_long_f32(DevBa
         const int nstrips = (k + STRIP - 1) / STRIP;
         const bool has_in = strip > 0, has_out = strip + 1 < nstrips;
         const int risk = p.risk[r];  // k_read_risk: 255 = fp32's range per lane may not do for this read, else its smallest GCP quality
-        const int hop = (risk * 32 * 85) >> 8;  // bits the running sum loses per lane it crosses: 32 columns x 0.332 GCP_min (rounded down)
+        const int hop = (risk * 32 * LONG_HOPNUM_) >> 8;  // bits the running sum loses per lane it crosses: 32 columns x 0.332 GCP_min (rounded down)
+        const int hcs = ((risk * LONG_HOPNUM_) >> 8) << 23;  // the same per column (rounded down), as a step of the fp32 exponent field
         if (risk == 255) {  // the pair's last strip hands it to fp64
             if (!has_out && lane == 0) {
                 const int idx = atomicAdd(p.fallback_count, 1);
@@ -231,11 +247,35 @@ __global__ void __launch_bounds__(LONG_WPC * 32, LONG_MIN_CTAS) k_long_f32(DevBa
                     pre = s2;
                 }
             }
-            // 2. own proposal (none for a lane that holds nothing)
-            float m = fmax3(ln.outS.x, ln.outS.y, fmaxf(ln.outT.x, ln.outT.y));
+            // 2. own proposal (none for a lane that holds nothing) and what can LEAVE this lane on its right within the next 16
+            // steps: the .y half (columns 16..31) as it stands; a value in column x < 16 moves at most 16 columns along
+            // diagonals in 16 rows and has to be deleted across the other 16 - x (gamma_max per column; charged per group of
+            // four columns, at the group's last).  All values are >= 0, so float order is integer order and a power of two is a
+            // step of the exponent field.  (Proposing the lane maximum instead, as until late in round 2, charges a lane
+            // whose large values sit at its left edge -- every lane of a deletion corridor -- 32 columns = 106 bits too little,
+            // and the lanes to its right were pushed up until the cells at their own right edge, 103 bits below their maximum,
+            // fell off fp32's range: M states inside a long deletion that split it in two, worth 0.6 % of the likelihood of a
+            // two-stretch read.)
+            static_assert(NV == 16, "the exit bound below groups the 16 columns of the .x half by four");
+            const int hcs_now = s < 64 + LONG_EVERY ? 0 : hcs;  // (no loss per column while the run-in entry is in the strip, see hop_now)
+            int gy0 = max(__float_as_int(ln.outS.y), __float_as_int(ln.outT.y)), gy1 = max(__float_as_int(ln.outS.x), __float_as_int(ln.outT.x));
+            int gx[4];
 #pragma unroll
-            for (int x = 0; x < NV; x++) m = fmax3(m, fmaxf(ln.Tt[x].x, ln.Tt[x].y), fmaxf(ln.J[x].x, ln.J[x].y));
+            for (int q = 0; q < 4; q++) {
+                gx[q] = max(__float_as_int(ln.Tt[4 * q].x), __float_as_int(ln.J[4 * q].x));
+#pragma unroll
+                for (int x = 4 * q + 1; x < 4 * q + 4; x++) gx[q] = max(gx[q], max(__float_as_int(ln.Tt[x].x), __float_as_int(ln.J[x].x)));
+            }
+#pragma unroll
+            for (int x = 0; x < NV; x += 2) {
+                gy0 = max(gy0, max(__float_as_int(ln.Tt[x].y), __float_as_int(ln.J[x].y)));
+                gy1 = max(gy1, max(__float_as_int(ln.Tt[x + 1].y), __float_as_int(ln.J[x + 1].y)));
+            }
+            const int gy = max(gy0, gy1);
+            const float m = __int_as_float(max(max(gx[0], gx[1]), max(max(gx[2], gx[3]), gy)));
             int c = m > 0.f ? ex + max(Fx<float>::ilogb(m) - LONG_TGT, -127) : LONG_FLOOR;  // (the shift 2^(ex - ex') stays one factor)
+            const int mo = max(max(max(gx[0] - 13 * hcs_now, gx[1] - 9 * hcs_now), max(gx[2] - 5 * hcs_now, gx[3] - hcs_now)), gy);
+            const int cout = mo >= 0x00800000 ? ex + (mo >> 23) - 127 - LONG_TGT : LONG_FLOOR;
             // Soundness of the 16-step interval: a lane whose own maximum stood at 2^TGT one event ago and has dropped by more
             // than LONG_DROP bits since (it takes gap-continuation qualities above 20, i.e. more than ~7 bits lost per row on every
             // path) may have flushed values that were NOT negligible (less than 166 - LONG_DROP bits below that maximum): the pair is
@@ -254,27 +294,32 @@ __global__ void __launch_bounds__(LONG_WPC * 32, LONG_MIN_CTAS) k_long_f32(DevBa
                 for (int o = 8; o > 0; o >>= 1) bmax = max(bmax, __shfl_xor_sync(PHMM_FULL, bmax, o));
                 bmax = __shfl_sync(PHMM_FULL, bmax, 0);
             }
-            // 3. ex'_L = max(c_L, max over m < L of c_m - KTOT - (L - 1 - m) HOP), the boundary records counting as a lane to the
-            //    left of lane 0.  What lane m holds can reach lane L within the next 16 steps only through the running sum, which
-            //    loses HOP = 32 log2(1 / gamma_max) bits per full lane it crosses (a deletion per column; values moving
-            //    diagonally cross at most 16 columns): nothing that can reach lane L is stored above 2^(TGT+KTOT) there.
-            //    And what is flushed in lane L -- a cell more than 2^-(126+TGT+KTOT) 2^-((L-1-m) HOP) below lane m's maximum
-            //    A -- can never matter later: A's path reaches that cell's continuation by a deletion of at most
-            //    32 (L - 1 - m) + 62 columns, which costs less.  (A constraint without the HOP term, as first written,
-            //    flushes the start of a second matching stretch a few hundred columns to the right of the first one: reads
-            //    with a long deletion against the haplotype came out too small by up to 240 in log10.)
+            // 3. ex'_L = max(c_L, max over the 8 lanes m < L of o_m - KTOT - (L - 1 - m) HOP), o_m = the exponent of what can
+            //    leave lane m (above), the boundary records counting as a lane to the left of lane 0.  What lane m holds can
+            //    reach lane L within the next 16 steps only through the running sum, which loses HOP = 32 log2(1 / gamma_max)
+            //    bits per full lane it crosses (a deletion per column), and crossing a lane takes two steps: nothing that
+            //    reaches lane L before the next event is stored above 2^(TGT+KTOT) there -- up to the 16 columns a value
+            //    may cover along diagonals instead, which a stretch that starts abruptly could turn into an overflow: inf and
+            //    NaN persist into Eq.4's total and send the pair to fp64 (below).  And what is flushed in lane L -- a cell more
+            //    than 2^-(126+TGT+KTOT) 2^-((L-1-m) HOP) below what leaves lane m -- is negligible against lane m's own
+            //    continuation into lane L.  (A constraint without the HOP term, as first written, flushes the start of a
+            //    second matching stretch a few hundred columns to the right of the first one: reads with a long deletion against
+            //    the haplotype came out too small by up to 240 in log10; with the HOP term but the lane MAXIMUM as o_m, over the
+            //    whole prefix of lanes instead of 8, the far ends of the lanes inside such a deletion were flushed: 0.6 %.)
             const int bsrc = bmax > LONG_FLOOR ? bmax - LONG_TGT : LONG_FLOOR;
             // (the run-in entry -- row 0 of Eq.1 -- carries C/k through every column undiminished, gamma := 1: no HOP until it
             // has left the strip's last lane, at step 63)
             const int hop_now = s < 64 + LONG_EVERY ? 0 : hop;
-            int pm = lane == 0 ? max(c, bsrc) : c;
+            // (a window of 8 lanes: crossing a lane takes two steps, so nothing further to the left arrives before the next event)
+            int pm = cout;
 #pragma unroll
-            for (int o = 1; o < 32; o <<= 1) {
+            for (int o = 1; o < 8; o <<= 1) {
                 const int t = __shfl_up_sync(PHMM_FULL, pm, o) - o * hop_now;
                 if (lane >= o) pm = max(pm, t);
             }
             pm = __shfl_up_sync(PHMM_FULL, pm, 1);
-            if (lane == 0) pm = bsrc;
+            if (lane == 0) pm = LONG_FLOOR;
+            if (lane < 8) pm = max(pm, bsrc - lane * hop_now);
             if (pm > LONG_FLOOR / 2) c = max(c, pm - LONG_KTOT);
             const int exn = c < LONG_FLOOR / 2 ? ex : c;  // nothing held, nothing to the left: keep the exponent
             sm.own[lane] = m > 0.f && exn == ex + Fx<float>::ilogb(m) - LONG_TGT;  // (a clamped proposal does not count)

@@ -301,6 +301,43 @@ def test_reads_with_a_long_deletion_against_the_haplotype(B, ctx):
     assert np.max(np.abs(out64 - ref)) <= TOL64
 
 
+def test_m_states_inside_a_long_deletion(B, ctx):
+    """Where opening a gap costs about what extending one does (deletion quality 10), a long deletion can be split by an M
+    state in any column whose base happens to match: together those paths carry percents of the likelihood, and each of their
+    cells sits up to 103 bits below the largest cell of its 32-column lane.  The fp32 long kernel flushed the ones at the far
+    end of the lanes inside the deletion (0.6 % of the likelihood, found by the randomized batches: generator seed 600227,
+    a 2559-base read against a 4407-base haplotype) until what a lane proposes to its right neighbours became what can
+    LEAVE it within an interval instead of its maximum (csrc/phmm_long.cu).  Reference: the log-space companion (the C
+    oracle drops cells 2^-1074 below their row maximum and loses the second stretch altogether)."""
+    from oracle import logspace
+    rng = np.random.default_rng(600227)
+    b = _fz_make(rng, 12, 6000, 3000)
+    sel = [i for i in range(b.n_pairs) if b.read_len()[b.pair_read[i]] == 2559 and b.hap_len()[b.pair_hap[i]] == 4407]
+    assert sel, "the generator no longer reproduces the batch of seed 600227"
+    out, fl = run(B, ctx, b, B.PHMM_FP32_RESCUE)
+    out64, _ = run(B, ctx, b, B.PHMM_FP64)
+    for i in sel:
+        pp = b.pair(i)
+        ref = logspace.log10_likelihood(pp[0], pp[5], pp[1], pp[2], pp[3], pp[4])
+        assert abs(out64[i] - ref) <= TOL64 and abs(out[i] - ref) <= TOL32 / 10, (out[i], out64[i], ref, fl[i])
+    rng = np.random.default_rng(52)
+    hap = _rand_seq(rng, 4300)
+    pairs, refs = [], []
+    for gap in (150, 333, 597, 801, 1100, 2050):
+        for a0 in (700, 711, 733):
+            cut, l = 400 + int(rng.integers(0, 30)), 900
+            read = hap[a0:a0 + cut] + hap[a0 + cut + gap:a0 + gap + l]
+            qb = list(rng.integers(2, 42, l)) if a0 != 711 else [30] * l
+            pairs.append((read, hap, qb, 40, 10, 10))
+    b = W.from_strings(pairs)
+    ref = np.array([logspace.log10_likelihood(*[b.pair(i)[j] for j in (0, 5, 1, 2, 3, 4)]) for i in range(b.n_pairs)])
+    out, fl = run(B, ctx, b, B.PHMM_FP32_RESCUE)
+    out64, _ = run(B, ctx, b, B.PHMM_FP64)
+    assert np.all(np.abs(out64 - ref) <= TOL64), np.abs(out64 - ref).max()
+    assert np.all(np.abs(out - ref) <= TOL32 / 10), (np.abs(out - ref).max(), fl)
+    assert np.all((fl & B.PHMM_FLAG_LONG) != 0)
+
+
 def test_async_calls_back_to_back_bitwise(B, ctx):
     """The call only enqueues: different batches issued back to back on one stream (plan uploads of call s+1 run
     on the context's copy stream under the kernels of call s, two plan sets alternate) must give exactly what each
