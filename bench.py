@@ -228,6 +228,7 @@ def measure(args, workload, steps, rank, world, local, with_cpu):
     s = ctx.stats()  # per-family CUDA-event durations of the last timed call
     fam = {k: s[k] for k in ("ms_table", "ms_short", "ms_rescue", "ms_long")}
     host_ms = s["host_batch_ms"]
+    fam_samples = [dict(fam)]
     # ---- SURVEY 8(d) protocol: 5 calls timed one by one (host batcher inside, nothing to overlap with): median and best
     single = []
     for _ in range(5):
@@ -239,6 +240,11 @@ def measure(args, workload, steps, rank, world, local, with_cpu):
         a1.record()
         torch.cuda.synchronize()
         single.append((a0.elapsed_time(a1), (time.perf_counter() - t_host) * 1e3))
+        s1 = ctx.stats()
+        fam_samples.append({k: s1[k] for k in fam})
+    # kernel durations: CUDA events the library records around each kernel family, averaged over the last call of the timed
+    # region and these five launches (same kernels, same inputs)
+    fam = {k: sum(f[k] for f in fam_samples) / len(fam_samples) for k in fam}
     clocks = sampler.stop() if sampler else None
     ms, tot_cells, tot_pairs = replicas.aggregate(ms, cells, n_pairs, dist if world > 1 else None, dev)
     ms_step = ms / steps
@@ -327,6 +333,8 @@ def measure(args, workload, steps, rank, world, local, with_cpu):
                 "whole_step_frac_at_executed_flops": step_tflops / peak * FLOPS_PER_CELL_EXECUTED[args.precision] / FLOPS_PER_CELL,
                 "kernel_ms_per_launch": kms, "kernel_gcups": kcells / (kms * 1e-3) / 1e9 if kms > 0 else 0.0,
                 "kernel_share_of_step": kms / ms_step if ms_step > 0 else None,
+                "kernel_timer": "CUDA events recorded by the library around each kernel family on the launching stream; mean of "
+                                "%d launches (the last call of the timed region and the individually timed calls)" % len(fam_samples),
                 "hbm_gbs_achieved": None, "family_ms": fam, "host_batch_ms": host_ms}
     if roofline["traffic"] and kms > 0:  # DRAM bytes of the committed ncu capture of this very workload and scale / this run's kernel time
         roofline["hbm_gbs_achieved"] = roofline["traffic"] / (kms * 1e-3) / 1e9

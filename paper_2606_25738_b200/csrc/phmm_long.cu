@@ -256,12 +256,13 @@ __global__ void __launch_bounds__(LONG_WPC * 32, LONG_MIN_CTAS) k_long_f32(DevBa
             // and the lanes to its right were pushed up until the cells at their own right edge, 103 bits below their maximum,
             // fell off fp32's range: M states inside a long deletion that split it in two, worth 0.6 % of the likelihood of a
             // two-stretch read.)
-            static_assert(NV == 16, "the exit bound below groups the 16 columns of the .x half by four");
+            static_assert(NV % 4 == 0, "the exit bound below groups the columns of the .x half by four");
+            constexpr int NG = NV / 4;
             const int hcs_now = s < 64 + LONG_EVERY ? 0 : hcs;  // (no loss per column while the run-in entry is in the strip, see hop_now)
             int gy0 = max(__float_as_int(ln.outS.y), __float_as_int(ln.outT.y)), gy1 = max(__float_as_int(ln.outS.x), __float_as_int(ln.outT.x));
-            int gx[4];
+            int gx[NG];
 #pragma unroll
-            for (int q = 0; q < 4; q++) {
+            for (int q = 0; q < NG; q++) {
                 gx[q] = max(__float_as_int(ln.Tt[4 * q].x), __float_as_int(ln.J[4 * q].x));
 #pragma unroll
                 for (int x = 4 * q + 1; x < 4 * q + 4; x++) gx[q] = max(gx[q], max(__float_as_int(ln.Tt[x].x), __float_as_int(ln.J[x].x)));
@@ -272,9 +273,15 @@ __global__ void __launch_bounds__(LONG_WPC * 32, LONG_MIN_CTAS) k_long_f32(DevBa
                 gy1 = max(gy1, max(__float_as_int(ln.Tt[x + 1].y), __float_as_int(ln.J[x + 1].y)));
             }
             const int gy = max(gy0, gy1);
-            const float m = __int_as_float(max(max(gx[0], gx[1]), max(max(gx[2], gx[3]), gy)));
+            int mall = gy, mo = gy;
+#pragma unroll
+            for (int q = 0; q < NG; q++) {  // the group's last column, 4q + 3, is 2NV - 4q - 3 columns from the lane's right edge: 16 of them may be diagonal
+                const int del = 2 * NV - 19 - 4 * q;
+                mall = max(mall, gx[q]);
+                mo = max(mo, gx[q] - (del > 0 ? del : 0) * hcs_now);
+            }
+            const float m = __int_as_float(mall);
             int c = m > 0.f ? ex + max(Fx<float>::ilogb(m) - LONG_TGT, -127) : LONG_FLOOR;  // (the shift 2^(ex - ex') stays one factor)
-            const int mo = max(max(max(gx[0] - 13 * hcs_now, gx[1] - 9 * hcs_now), max(gx[2] - 5 * hcs_now, gx[3] - hcs_now)), gy);
             const int cout = mo >= 0x00800000 ? ex + (mo >> 23) - 127 - LONG_TGT : LONG_FLOOR;
             // Soundness of the 16-step interval: a lane whose own maximum stood at 2^TGT one event ago and has dropped by more
             // than LONG_DROP bits since (it takes gap-continuation qualities above 20, i.e. more than ~7 bits lost per row on every
