@@ -1,4 +1,6 @@
-// Rescaled fp64 path ("chain" kernel; the fp32 long path is phmm_long.cu): one warp = one strip of 32 lanes x 2NV haplotype columns of
+// Rescaled fp64 path ("chain" kernel; the fp32 long path is phmm_long.cu, the PHMM_FP64 long path phmm_long64.cu, which took over
+// this kernel's concurrent mode late in round 2: the library now launches it only in its sequential mode, as the last resort
+// for pairs no other kernel could represent): one warp = one strip of 32 lanes x 2NV haplotype columns of
 // one pair; the strips of a pair are chained left to right through boundary-column buffers in
 // global memory (per stream entry: the running sum s and the T that drop out of the strip's last
 // column, and the producing thread's block exponent), either concurrently (one strip per
